@@ -1,0 +1,160 @@
+"""ORACLE (test infrastructure, not the product): ctypes front-end of oracle/tbpm_oracle.c plus numpy post-processing.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may import this package.
+It imports nothing from paper_2509_26309_b200 (the CUDA path) and shares no code with it.  All arrays are numpy,
+complex128 viewed as (re, im) float64 pairs.  See the header of tbpm_oracle.c for the algorithm and its citations.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_DIR, "tbpm_oracle.c")
+_LIB = os.path.join(_DIR, "libtbpm_oracle.so")
+TOL = 1e-15   # truncation |J_k(tau)| < 1e-15 (BASELINE.json:configs[0])
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-shared", "-fPIC", _SRC, "-o", _LIB, "-lm"])
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+    return _lib
+
+
+def _p(a, t=C.c_double):
+    return None if a is None else a.ctypes.data_as(C.POINTER(t))
+
+
+def _c128(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.complex128))
+
+
+def bessel_j(x: float, kmax: int) -> np.ndarray:
+    out = np.empty(kmax + 1, dtype=np.float64)
+    rc = lib().oracle_bessel_j(C.c_double(x), C.c_int(kmax), _p(out))
+    if rc:
+        raise ValueError(f"oracle_bessel_j rc={rc}")
+    return out
+
+
+def cheb_coeff(tau: float, tol: float = TOL, kcap: int = 4096) -> np.ndarray:
+    """complex128 [K] coefficients c_k = (2-delta_k0)(-i)^k J_k(tau)."""
+    buf = np.empty(2 * kcap, dtype=np.float64)
+    K = C.c_int(0)
+    rc = lib().oracle_cheb_coeff(C.c_double(tau), C.c_double(tol), C.c_int(kcap), C.byref(K), _p(buf))
+    if rc:
+        raise ValueError(f"oracle_cheb_coeff rc={rc}")
+    return buf[: 2 * K.value].view(np.complex128).copy()
+
+
+def _hops(hop_i, hop_j, hop_val):
+    hi = np.ascontiguousarray(np.asarray(hop_i, dtype=np.int32))
+    hj = np.ascontiguousarray(np.asarray(hop_j, dtype=np.int32))
+    hv = _c128(hop_val)
+    assert hi.shape == hj.shape == hv.shape and hi.ndim == 1
+    return hi, hj, hv
+
+
+def build_csr(n_orb, onsite, hop_i, hop_j, hop_val, hops_full=False):
+    """Canonical CSR (rowptr int64[n+1], col int32[nnz], val complex128[nnz])."""
+    hi, hj, hv = _hops(hop_i, hop_j, hop_val)
+    on = None if onsite is None else np.ascontiguousarray(np.asarray(onsite, dtype=np.float64))
+    nnz = hi.size * (1 if hops_full else 2) + (n_orb if on is not None else 0)
+    rowptr = np.empty(n_orb + 1, dtype=np.int64)
+    col = np.empty(max(nnz, 1), dtype=np.int32)
+    val = np.empty(max(nnz, 1), dtype=np.complex128)
+    rc = lib().oracle_build_csr(C.c_int64(n_orb), _p(on), C.c_int64(hi.size), _p(hi, C.c_int32), _p(hj, C.c_int32),
+                                _p(hv.view(np.float64)), C.c_int(int(hops_full)), _p(rowptr, C.c_int64),
+                                _p(col, C.c_int32), _p(val.view(np.float64)))
+    if rc:
+        raise ValueError(f"oracle_build_csr rc={rc}")
+    return rowptr, col[:nnz], val[:nnz]
+
+
+def apply_h(n_orb, onsite, hop_i, hop_j, hop_val, x, hops_full=False):
+    hi, hj, hv = _hops(hop_i, hop_j, hop_val)
+    on = None if onsite is None else np.ascontiguousarray(np.asarray(onsite, dtype=np.float64))
+    x = _c128(x)
+    y = np.empty(n_orb, dtype=np.complex128)
+    rc = lib().oracle_apply_h(C.c_int64(n_orb), _p(on), C.c_int64(hi.size), _p(hi, C.c_int32), _p(hj, C.c_int32),
+                              _p(hv.view(np.float64)), C.c_int(int(hops_full)), _p(x.view(np.float64)), _p(y.view(np.float64)))
+    if rc:
+        raise ValueError(f"oracle_apply_h rc={rc}")
+    return y
+
+
+def propagate(n_orb, onsite, hop_i, hop_j, hop_val, psi0, n_step, dt, rescale, *, psi_start=None, hops_full=False,
+              tol=TOL, form="hops", return_state=False):
+    """corr[n_state][n_step], norm2[n_state][n_step] (and final states) for psi0[n_state][n_orb].
+
+    form="hops": serial hop-list scatter form (authoritative).  form="csr": OpenMP row form on the canonical CSR.
+    psi_start (same shape) starts the window from a later state while the bra stays psi0 (windowed parity)."""
+    hi, hj, hv = _hops(hop_i, hop_j, hop_val)
+    on = None if onsite is None else np.ascontiguousarray(np.asarray(onsite, dtype=np.float64))
+    psi0 = np.atleast_2d(_c128(psi0))
+    start = psi0 if psi_start is None else np.atleast_2d(_c128(psi_start))
+    B = psi0.shape[0]
+    assert psi0.shape == (B, n_orb) and start.shape == (B, n_orb)
+    corr = np.zeros((B, n_step), dtype=np.complex128)
+    norm2 = np.zeros((B, n_step), dtype=np.float64)
+    final = np.empty((B, n_orb), dtype=np.complex128)
+    if form == "csr":
+        rowptr, col, val = build_csr(n_orb, on, hi, hj, hv, hops_full)
+    for b in range(B):
+        s, z, f = np.ascontiguousarray(start[b]), np.ascontiguousarray(psi0[b]), final[b]
+        if form == "hops":
+            rc = lib().oracle_propagate(C.c_int64(n_orb), _p(on), C.c_int64(hi.size), _p(hi, C.c_int32), _p(hj, C.c_int32),
+                                        _p(hv.view(np.float64)), C.c_int(int(hops_full)), _p(s.view(np.float64)),
+                                        _p(z.view(np.float64)), C.c_int(n_step), C.c_double(dt), C.c_double(rescale),
+                                        C.c_double(tol), _p(corr[b].view(np.float64)), _p(norm2[b]), _p(f.view(np.float64)))
+        elif form == "csr":
+            rc = lib().oracle_propagate_csr(C.c_int64(n_orb), _p(rowptr, C.c_int64), _p(col, C.c_int32),
+                                            _p(val.view(np.float64)), _p(s.view(np.float64)), _p(z.view(np.float64)),
+                                            C.c_int(n_step), C.c_double(dt), C.c_double(rescale), C.c_double(tol),
+                                            _p(corr[b].view(np.float64)), _p(norm2[b]), _p(f.view(np.float64)))
+        else:
+            raise ValueError(form)
+        if rc:
+            raise ValueError(f"oracle_propagate rc={rc}")
+    return (corr, norm2, final) if return_state else (corr, norm2)
+
+
+def ldos(n_orb, onsite, hop_i, hop_j, hop_val, sites, n_step, dt, rescale, **kw):
+    """TBPM-style LDOS correlation: psi0 = e_site (reading #25), corr_n = psi_site(n dt)."""
+    sites = np.asarray(sites, dtype=np.int64)
+    psi0 = np.zeros((sites.size, n_orb), dtype=np.complex128)
+    psi0[np.arange(sites.size), sites] = 1.0
+    return propagate(n_orb, onsite, hop_i, hop_j, hop_val, psi0, n_step, dt, rescale, **kw)
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def dos_from_corr(corr: np.ndarray, rescale: float):
+    """DOS post-processing (NEXT-1; `Analyzer.calc_dos(corr)`, PAPER.md:980-982 gives no formula; reading #27):
+    C_0 = 1, C_{-n} = conj(C_n), Hann window w_n = (1 + cos(pi n/N_t))/2 and, for tau = pi (sampling interval
+    pi/s <-> energy window [-s, s]),  D(E) = (1/2s) [1 + 2 Re sum_{n=1}^{N_t} w_n C_n exp(i n pi E/s)]  on
+    E_j = -s + j s/N_t, j = 0..2N_t.  Plain direct DFT, no FFT.  corr is 1-D (average over states beforehand)."""
+    corr = np.asarray(corr, dtype=np.complex128).ravel()
+    nt = corr.size
+    n = np.arange(1, nt + 1)
+    w = 0.5 * (1.0 + np.cos(np.pi * n / nt))
+    E = -rescale + np.arange(2 * nt + 1) * (rescale / nt)
+    ph = np.exp(1j * np.pi * np.outer(E / rescale, n))
+    D = (1.0 + 2.0 * np.real(ph @ (w * corr))) / (2.0 * rescale)
+    return E, D
