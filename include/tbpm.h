@@ -1,0 +1,136 @@
+/*
+ * tbpm.h -- C ABI of libtbpm.so: the B200-native (sm_100a) hot path of TBPLaS 2.0's tight-binding propagation
+ * method (TBPM), arxiv 2509.26309.  Citations are "PAPER.md:LINE" of the paper text plus the section.
+ *
+ * The path:
+ *   a0  tbpm_build      hopping list (each conjugate pair once) -> canonical CSR on the device
+ *                       (+ the internal compressed layout the kernels read)
+ *   a1  coefficients    c_k = (2 - delta_k0)(-i)^k J_k(tau), truncated at |J_k| < 1e-15 ("the imaginary
+ *                       factor ... has been merged into the Chebyshev coefficients"; values: BASELINE.json:configs[0])
+ *   a2-a7 tbpm_propagate  per time step  psi <- sum_k c_k T_k(H/s) psi  by the recursion of PAPER.md:437-443
+ *                       (p2 = p0; amxsy(2.0, p1, p0); axpy(coeff[n], p2, wf_out); rotate), then
+ *                       corr[n] = <psi0|psi(t_n)> and norm2[n] = <psi|psi>   (calc_corr_dos)
+ *   a8  tbpm_ldos       the same with psi0 = unit vectors on the given sites
+ *
+ * Conventions
+ *   - "device" pointers are CUDA device memory of the current device; "host" pointers are ordinary host memory.
+ *   - complex128 values are (re, im) pairs of doubles.  hbar = 1: dt is in 1/(energy unit of H); tau = rescale*dt.
+ *   - Ownership: every buffer is allocated and freed by the caller (PyTorch in this repository).  The library
+ *     allocates no device memory.  `persist` must outlive the handle; `scratch` may be released when tbpm_build
+ *     returns; `workspace` holds the states of the last tbpm_propagate / tbpm_ldos call (see tbpm_get_state).
+ *   - All device pointers must be 16-byte aligned; `persist`, `scratch`, `workspace` 256-byte aligned.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - Every function returns TBPM_OK (0) or a negative TBPM_E* code; no C++ exception crosses the ABI.
+ *   - There is NO CPU fallback: without a usable CUDA device every device entry point returns TBPM_ECUDA.
+ */
+#ifndef TBPM_H
+#define TBPM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tbpm_ham tbpm_ham; /* opaque host handle pointing into caller-owned device memory */
+
+/* error codes */
+#define TBPM_OK 0
+#define TBPM_EINVAL (-1)  /* NULL / negative / misaligned argument, n_orb >= 2^31, rescale <= 0, ...                 */
+#define TBPM_EINDEX (-2)  /* hop index out of [0, n_orb)                                   (TBPM_VALIDATE only)      */
+#define TBPM_EDIAG (-3)   /* hop with i == j: illegal, on-site energy is an orbital attribute    */
+#define TBPM_EDUP (-4)    /* the same (row, col) produced twice (the paper's dict-update semantic, PAPER.md:190-191,
+                             has no meaning for a flat list; SURVEY reading #15)          (TBPM_VALIDATE only)      */
+#define TBPM_ENOMEM (-5)  /* a caller-provided buffer is too small                                                   */
+#define TBPM_ECUDA (-6)   /* CUDA runtime error (no device, launch failure, sticky error)                            */
+#define TBPM_EBOUND (-7)  /* Gershgorin bound max_i(|onsite_i| + sum_j |H_ij|) > rescale (strictly): the Chebyshev
+                             recursion would diverge.  Returned by tbpm_check_bound only; never fatal elsewhere.     */
+
+/* flags of tbpm_build */
+#define TBPM_VALIDATE 1u    /* run the precondition checks (index range, i != j, duplicates); following the paper's
+                               "bugs vs exceptions" split they are off by default         */
+#define TBPM_HOPS_FULL 2u   /* the list already holds both orientations of every pair (default: each pair once and
+                               the conjugate partner H_ji = conj(H_ij) is generated)                    */
+#define TBPM_NO_TABLE 4u    /* keep complex128 values in the kernel layout instead of 16-bit indices into a table of
+                               distinct hopping values (the table is the default whenever <= 65536 values occur)      */
+
+const char *tbpm_strerror(int code);
+const char *tbpm_version(void);
+
+/* ---- a1: Chebyshev coefficients (host only, needs no GPU) -----------------------------------------------------------
+ * tau >= 0.  K = first k >= ceil(tau) with |J_k(tau)| < tol (strict); coefficients k = 0..K-1 are written to
+ * coeff[k][2].  K(pi) = 21 at tol = 1e-15, i.e. 20 H-applications per time step.  TBPM_ENOMEM if K > kcap (K is still
+ * reported).  The library uses tol = 1e-15 (BASELINE.json:configs[0]). */
+int tbpm_cheb_coeff(double tau, double tol, int kcap, int *K, double *coeff /* host [kcap][2] */);
+
+/* ---- a0: build -----------------------------------------------------------------------------------------------------
+ * Sizes of the two caller-provided device buffers for a model with n_orb orbitals and n_hop list entries. */
+int tbpm_build_bytes(int64_t n_orb, int64_t n_hop, int has_onsite, uint32_t flags, size_t *persist_bytes,
+                     size_t *scratch_bytes);
+
+/* Entry h of the list means <hop_i[h]| H |hop_j[h]> = hop_val[h] (the paper's <i,0|H|j,R>); unless
+ * TBPM_HOPS_FULL is set the partner <j|H|i> = conj(val) is added.  onsite (real, may be NULL) adds a diagonal entry
+ * (onsite_i, 0) to EVERY row; onsite == NULL stores no diagonal.  Result: canonical CSR (rows ascending, columns
+ * strictly ascending within a row), bit-exact whatever the order of the list, plus the internal kernel layout.
+ * Rows without entries are legal.  The call enqueues its kernels on `stream` and synchronises it before returning
+ * (it must read back the status word and the size of the hopping-value table). */
+int tbpm_build(int64_t n_orb, const double *onsite /* device [n_orb] or NULL */, int64_t n_hop,
+               const int32_t *hop_i /* device [n_hop] */, const int32_t *hop_j /* device [n_hop] */,
+               const double *hop_val /* device [n_hop][2] */, uint32_t flags, void *persist /* device */,
+               size_t persist_bytes, void *scratch /* device */, size_t scratch_bytes, void *stream, tbpm_ham **out);
+
+/* nnz = stored entries of the canonical CSR; matrix_bytes_per_term = bytes of H the kernels read per Chebyshev term
+ * (the "matrix bytes as stored" of the roofline count); n_table = distinct off-diagonal values (0: table not used);
+ * gershgorin = max_i (|onsite_i| + sum_j |H_ij|).  Any output pointer may be NULL. */
+int tbpm_ham_info(const tbpm_ham *H, int64_t *n_orb, int64_t *nnz, int32_t *max_row_nnz, size_t *matrix_bytes_per_term,
+                  int32_t *n_table, double *gershgorin);
+
+/* TBPM_EBOUND if gershgorin > rescale (test is '>' : config 4 sits exactly at equality), else TBPM_OK. */
+int tbpm_check_bound(const tbpm_ham *H, double rescale);
+
+/* Canonical CSR in caller order, copied device -> device: rowptr int64[n_orb+1], col int32[nnz], val [nnz][2]. */
+int tbpm_export_csr(const tbpm_ham *H, int64_t *rowptr, int32_t *col, double *val, void *stream);
+
+void tbpm_free(tbpm_ham *H); /* frees only the host struct */
+
+/* ---- a2-a7: propagate ------------------------------------------------------------------------------------------------ */
+int tbpm_propagate_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes);
+
+/* psi0: device [n_state][n_orb][2], state-major (one random initial state per row; one independent propagation per
+ * state).  corr: device out [n_state][n_step][2], entry n is t = (n+1)*dt (t = 0, value <psi0|psi0>, is
+ * not stored).  norm2: device out [n_state][n_step] or NULL.  rescale = s > 0 must bound the spectrum, ||H|| <= s
+ * (config.rescale).  n_step == 0 or n_state == 0: success, outputs untouched.  Asynchronous on `stream`.
+ * Deterministic: the same inputs give bit-identical outputs, and the first m entries do not depend on n_step. */
+int tbpm_propagate(const tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale,
+                   double *corr, double *norm2, void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- a8: TBPM-style LDOS correlation: psi0_b = e_{sites[b]}, corr[b][n] = <site_b| psi_b(t_n) > -------------------- */
+int tbpm_ldos(const tbpm_ham *H, const int64_t *sites /* host [n_site] */, int n_site, int n_step, double dt,
+              double rescale, double *corr, double *norm2, void *workspace, size_t workspace_bytes, void *stream);
+
+/* State `state` as left in `workspace` by the last tbpm_propagate / tbpm_ldos call on it (psi after its n_step steps),
+ * caller order, device out [n_orb][2].  A snapshot at step j is a call with n_step = j. */
+int tbpm_get_state(const tbpm_ham *H, const void *workspace, int state, double *psi_out, void *stream);
+
+/* Number of kernels the last tbpm_propagate / tbpm_ldos call launched (host counter kept in the handle's library). */
+int64_t tbpm_last_launch_count(void);
+/* Kernels launched by this library in this process since it was loaded (build + propagate + get_state). */
+int64_t tbpm_total_launch_count(void);
+
+/* ---- end to end with HOST buffers ------------------------------------------------------------------------------------
+ * Whole path for host-resident inputs: H2D of the list and psi0, tbpm_build, tbpm_propagate, D2H of corr/norm2, then a
+ * stream synchronise.  `arena` is caller-owned device memory of at least tbpm_corr_host_bytes(); host buffers should be
+ * pinned for full copy bandwidth.  h2d_bytes / d2h_bytes (may be NULL) report what was copied. */
+int tbpm_corr_host_bytes(int64_t n_orb, int64_t n_hop, int has_onsite, int n_state, int n_step, uint32_t flags,
+                         size_t *arena_bytes);
+int tbpm_corr_host(int64_t n_orb, const double *onsite /* host or NULL */, int64_t n_hop, const int32_t *hop_i /* host */,
+                   const int32_t *hop_j /* host */, const double *hop_val /* host */, uint32_t flags,
+                   const double *psi0 /* host [n_state][n_orb][2] */, int n_state, int n_step, double dt, double rescale,
+                   double *corr /* host out */, double *norm2 /* host out or NULL */, void *arena /* device */,
+                   size_t arena_bytes, void *stream, size_t *h2d_bytes, size_t *d2h_bytes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TBPM_H */

@@ -1,0 +1,534 @@
+// build.cu -- step a0 of the path: hopping list -> canonical CSR -> kernel layout, all on the device.
+//
+// Conventions (PAPER.md, sections 2.1-3.2):
+//   * entry (i, j, v) is <i,0|H|j,R> = v; the list holds each pair once, "hopping terms reduced by
+//     the conjugate relation H_ij(R) = H_ji*(-R)", so both (i, j, v) and (j, i, conj v) are emitted
+//     unless TBPM_HOPS_FULL;
+//   * a hop with i == j is illegal, on-site energies are an orbital attribute: `onsite`
+//     gives one real diagonal entry per row;
+//   * Sample.init_array / build_ham_csr is the paper's "terms -> arrays" step.
+//
+// Algorithm (integer work; the result is unique, so bit-exact parity with the oracle is well defined):
+//   1. count entries per row with integer atomics                    k_count
+//   2. exclusive scan of the counts -> rowptr (int64)                scan_exclusive (3 kernels)
+//   3. scatter entries into their row segment (order within the row is arbitrary at this point)   k_fill
+//   4. one thread per row: insertion sort by column, duplicate check, Gershgorin row sum, max row length   k_sort_rows
+//   5. kernel layout: off-diagonal CSR with 32-bit row offsets + real diagonal                     k_strip
+//   6. table of distinct off-diagonal values (open-addressing hash on the 128-bit pattern), 16-bit index per entry
+//      k_tab_insert / scan / k_tab_number / k_tab_lookup   ("hopping-table index for uniform lattices", north_star)
+#include <algorithm>
+#include <cstring>
+#include <new>
+
+#include "tbpm_internal.h"
+
+using namespace tbpm_detail;
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kScanItems = 8;                       // items per thread in the scan kernels
+constexpr int kScanTile = kThreads * kScanItems;    // 2048 items per block
+
+inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)((n + per_block - 1) / per_block); }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// exclusive scan int32 -> int64 over n items (out[i] = sum_{k<i} in[k]); three kernels, deterministic
+// ---------------------------------------------------------------------------------------------------------------------
+__global__ void k_scan_block_sums(const int32_t *__restrict__ in, int64_t n, int64_t *__restrict__ bsum)
+{
+    __shared__ int64_t warp_sum[kThreads / 32];
+    int64_t base = (int64_t)blockIdx.x * kScanTile;
+    int64_t s = 0;
+    for (int k = 0; k < kScanItems; ++k) {
+        int64_t i = base + (int64_t)k * kThreads + threadIdx.x;
+        if (i < n) s += in[i];
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) warp_sum[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int64_t t = 0;
+        for (int w = 0; w < kThreads / 32; ++w) t += warp_sum[w];
+        bsum[blockIdx.x] = t;
+    }
+}
+
+// single block: in-place exclusive scan of nb block sums
+__global__ void k_scan_of_sums(int64_t *bsum, int64_t nb)
+{
+    __shared__ int64_t warp_tot[32];
+    __shared__ int64_t carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int64_t base = 0; base < nb; base += blockDim.x) {
+        int64_t i = base + threadIdx.x;
+        int64_t v = i < nb ? bsum[i] : 0;
+        int64_t incl = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            int64_t t = __shfl_up_sync(0xffffffffu, incl, o);
+            if ((threadIdx.x & 31) >= o) incl += t;
+        }
+        if ((threadIdx.x & 31) == 31) warp_tot[threadIdx.x >> 5] = incl;
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            int nw = blockDim.x >> 5;
+            int64_t w = threadIdx.x < nw ? warp_tot[threadIdx.x] : 0;
+            int64_t wi = w;
+            for (int o = 1; o < 32; o <<= 1) {
+                int64_t t = __shfl_up_sync(0xffffffffu, wi, o);
+                if (threadIdx.x >= o) wi += t;
+            }
+            warp_tot[threadIdx.x] = wi - w;          // exclusive prefix of warp totals
+        }
+        __syncthreads();
+        int64_t carry = carry_s;
+        int64_t excl = carry + warp_tot[threadIdx.x >> 5] + incl - v;
+        if (i < nb) bsum[i] = excl;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry_s = excl + v;
+        __syncthreads();
+    }
+}
+
+__global__ void k_scan_apply(const int32_t *__restrict__ in, int64_t n, const int64_t *__restrict__ bsum,
+                             int64_t *__restrict__ out)
+{
+    // each thread owns kScanItems CONSECUTIVE items so that a simple thread-level prefix works
+    __shared__ int64_t warp_tot[kThreads / 32];
+    int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
+    int32_t v[kScanItems];
+    int64_t s = 0;
+    for (int k = 0; k < kScanItems; ++k) {
+        int64_t i = base + k;
+        v[k] = i < n ? in[i] : 0;
+        s += v[k];
+    }
+    int64_t incl = s;
+    for (int o = 1; o < 32; o <<= 1) {
+        int64_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((threadIdx.x & 31) >= o) incl += t;
+    }
+    if ((threadIdx.x & 31) == 31) warp_tot[threadIdx.x >> 5] = incl;
+    __syncthreads();
+    int64_t woff = 0;
+    for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) woff += warp_tot[w];
+    int64_t run = bsum[blockIdx.x] + woff + incl - s;
+    for (int k = 0; k < kScanItems; ++k) {
+        int64_t i = base + k;
+        if (i < n) out[i] = run;
+        run += v[k];
+    }
+}
+
+// bsum must hold blocks_for(n, kScanTile) int64
+int scan_exclusive(const int32_t *in, int64_t n, int64_t *out, int64_t *bsum, cudaStream_t st)
+{
+    if (n <= 0) return TBPM_OK;
+    unsigned nb = blocks_for(n, kScanTile);
+    k_scan_block_sums<<<nb, kThreads, 0, st>>>(in, n, bsum);
+    k_scan_of_sums<<<1, 1024, 0, st>>>(bsum, nb);
+    k_scan_apply<<<nb, kThreads, 0, st>>>(in, n, bsum, out);
+    count_launches(3);
+    TBPM_CUDA_TRY(cudaGetLastError());
+    return TBPM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// 1. counts.  cnt has n_orb + 1 entries; cnt[r] starts at has_onsite, cnt[n_orb] = 0.
+// ---------------------------------------------------------------------------------------------------------------------
+__global__ void k_init_counts(int32_t *cnt, int64_t n_orb, int has_onsite)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < n_orb) cnt[r] = has_onsite;
+    else if (r == n_orb) cnt[r] = 0;
+}
+
+__device__ __forceinline__ bool hop_ok(int32_t i, int32_t j, int64_t n_orb, int32_t *status)
+{
+    if (i < 0 || j < 0 || i >= n_orb || j >= n_orb) { atomicOr(&status[ST_ERR], 1); return false; }
+    if (i == j) { atomicOr(&status[ST_ERR], 2); return false; }
+    return true;
+}
+
+__global__ void k_count(int64_t n_hop, const int32_t *__restrict__ hop_i, const int32_t *__restrict__ hop_j, int64_t n_orb,
+                        int full, int32_t *cnt, int32_t *status)
+{
+    int64_t h = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= n_hop) return;
+    int32_t i = hop_i[h], j = hop_j[h];
+    if (!hop_ok(i, j, n_orb, status)) return;
+    atomicAdd(&cnt[i], 1);
+    if (!full) atomicAdd(&cnt[j], 1);
+}
+
+// 3. scatter.  cur[r] counts the entries already placed in row r (starts at has_onsite: slot 0 holds the diagonal).
+__global__ void k_fill_diag(int64_t n_orb, const double *__restrict__ onsite, const int64_t *__restrict__ rowptr, int32_t *col,
+                            double2 *val, int32_t *cur)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_orb) return;
+    if (onsite) {
+        int64_t p = rowptr[r];
+        col[p] = (int32_t)r;
+        val[p] = make_double2(onsite[r], 0.0);
+        cur[r] = 1;
+    } else {
+        cur[r] = 0;
+    }
+}
+
+__global__ void k_fill(int64_t n_hop, const int32_t *__restrict__ hop_i, const int32_t *__restrict__ hop_j,
+                       const double2 *__restrict__ hop_val, int64_t n_orb, int full, const int64_t *__restrict__ rowptr,
+                       int32_t *cur, int32_t *col, double2 *val, int32_t *status)
+{
+    int64_t h = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= n_hop) return;
+    int32_t i = hop_i[h], j = hop_j[h];
+    if (i < 0 || j < 0 || i >= n_orb || j >= n_orb || i == j) return;   // already flagged by k_count
+    double2 v = hop_val[h];
+    int64_t p = rowptr[i] + atomicAdd(&cur[i], 1);
+    col[p] = j;
+    val[p] = v;
+    if (!full) {
+        int64_t q = rowptr[j] + atomicAdd(&cur[j], 1);
+        col[q] = i;
+        val[q] = make_double2(v.x, -v.y);                               // conj: flips the sign bit of im (-0.0 possible)
+    }
+}
+
+// 4. per-row insertion sort by column + checks
+__global__ void k_sort_rows(int64_t n_orb, const int64_t *__restrict__ rowptr, int32_t *col, double2 *val, int32_t *status)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int len = 0;
+    double rowsum = 0.0;
+    bool dup = false;
+    if (r < n_orb) {
+        int64_t b = rowptr[r], e = rowptr[r + 1];
+        len = (int)(e - b);
+        for (int64_t p = b + 1; p < e; ++p) {
+            int32_t c = col[p];
+            double2 v = val[p];
+            int64_t q = p - 1;
+            while (q >= b && col[q] > c) {
+                col[q + 1] = col[q];
+                val[q + 1] = val[q];
+                --q;
+            }
+            col[q + 1] = c;
+            val[q + 1] = v;
+        }
+        for (int64_t p = b; p < e; ++p) {
+            double2 v = val[p];
+            rowsum += sqrt(v.x * v.x + v.y * v.y);
+            if (p > b && col[p] == col[p - 1]) dup = true;
+        }
+    }
+    // block-level max to keep the number of global atomics small
+    for (int o = 16; o > 0; o >>= 1) {
+        len = max(len, __shfl_xor_sync(0xffffffffu, len, o));
+        rowsum = fmax(rowsum, __shfl_xor_sync(0xffffffffu, rowsum, o));
+    }
+    if (__any_sync(0xffffffffu, dup) && (threadIdx.x & 31) == 0) atomicOr(&status[ST_ERR], 4);
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(&status[ST_MAX_ROW], len);
+        atomicMax(reinterpret_cast<unsigned long long *>(&status[ST_GERSH_LO]), (unsigned long long)__double_as_longlong(rowsum));
+    }
+}
+
+// 5. kernel layout.  has_onsite: every row holds exactly one diagonal entry -> off-diagonal offset = rowptr[r] - r.
+__global__ void k_strip(int64_t n_orb, int has_onsite, const int64_t *__restrict__ rowptr, const int32_t *__restrict__ col,
+                        const double2 *__restrict__ val, uint32_t *orp, int32_t *ocol, double *diag)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r > n_orb) return;
+    int64_t b = rowptr[r];
+    if (!has_onsite) { orp[r] = (uint32_t)b; return; }
+    int64_t ob = b - r;
+    orp[r] = (uint32_t)ob;
+    if (r == n_orb) return;
+    int64_t e = rowptr[r + 1];
+    for (int64_t p = b; p < e; ++p) {
+        int32_t c = col[p];
+        if (c == (int32_t)r) diag[r] = val[p].x;
+        else ocol[ob++] = c;
+    }
+}
+
+// 6. distinct-value table
+__device__ __forceinline__ uint64_t mix64(uint64_t z)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+__device__ __forceinline__ bool same_bits(double2 a, double2 b)
+{
+    return __double_as_longlong(a.x) == __double_as_longlong(b.x) && __double_as_longlong(a.y) == __double_as_longlong(b.y);
+}
+__device__ __forceinline__ uint32_t slot_of(double2 v)
+{
+    return (uint32_t)(mix64((uint64_t)__double_as_longlong(v.x) ^ mix64((uint64_t)__double_as_longlong(v.y) + 0x9E3779B97F4A7C15ull))) &
+           (kHashSlots - 1);
+}
+
+constexpr uint32_t kEmpty = 0xFFFFFFFFu;
+
+// slots[h] = canonical position of a representative entry with that value
+__global__ void k_tab_insert(int64_t n_orb, int has_onsite, const int64_t *__restrict__ rowptr, const int32_t *__restrict__ col,
+                             const double2 *__restrict__ val, uint32_t *slots, int32_t *status)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_orb) return;
+    for (int64_t p = rowptr[r]; p < rowptr[r + 1]; ++p) {
+        if (has_onsite && col[p] == (int32_t)r) continue;
+        double2 v = val[p];
+        uint32_t h = slot_of(v);
+        for (int probe = 0;; ++probe) {
+            if (probe >= kHashSlots || *(volatile int32_t *)&status[ST_TAB_OVERFLOW]) { status[ST_TAB_OVERFLOW] = 1; return; }
+            uint32_t cur = *(volatile uint32_t *)&slots[h];
+            if (cur == kEmpty) {
+                cur = atomicCAS(&slots[h], kEmpty, (uint32_t)p);
+                if (cur == kEmpty) {
+                    if (atomicAdd(&status[ST_NTAB], 1) + 1 > kTableMax) status[ST_TAB_OVERFLOW] = 1;
+                    break;
+                }
+            }
+            if (same_bits(val[cur], v)) break;
+            h = (h + 1) & (kHashSlots - 1);
+        }
+    }
+}
+
+__global__ void k_tab_flags(const uint32_t *__restrict__ slots, int32_t *flag)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < kHashSlots) flag[i] = slots[i] != kEmpty;
+    else if (i == kHashSlots) flag[i] = 0;
+}
+
+__global__ void k_tab_number(const uint32_t *__restrict__ slots, const int64_t *__restrict__ slot_id, const double2 *__restrict__ val,
+                             double2 *vtab)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= kHashSlots) return;
+    uint32_t s = slots[i];
+    if (s != kEmpty && slot_id[i] < kTableMax) vtab[slot_id[i]] = val[s];
+}
+
+__global__ void k_tab_lookup(int64_t n_orb, int has_onsite, const int64_t *__restrict__ rowptr, const int32_t *__restrict__ col,
+                             const double2 *__restrict__ val, const uint32_t *__restrict__ slots, const int64_t *__restrict__ slot_id,
+                             uint16_t *oidx)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_orb) return;
+    int64_t q = rowptr[r] - (has_onsite ? r : 0);
+    for (int64_t p = rowptr[r]; p < rowptr[r + 1]; ++p) {
+        if (has_onsite && col[p] == (int32_t)r) continue;
+        double2 v = val[p];
+        uint32_t h = slot_of(v);
+        while (!same_bits(val[slots[h]], v)) h = (h + 1) & (kHashSlots - 1);
+        oidx[q++] = (uint16_t)slot_id[h];
+    }
+}
+
+struct PersistLayout {
+    size_t status, rowptr, col, val, orp, ocol, oidx, vtab, diag, total;
+};
+
+PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint32_t flags)
+{
+    PersistLayout L{};
+    const size_t nnz_off = (size_t)n_hop * ((flags & TBPM_HOPS_FULL) ? 1 : 2);
+    const size_t nnz = nnz_off + (has_onsite ? (size_t)n_orb : 0);
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes ? bytes : 1); return at; };
+    L.status = take(sizeof(int32_t) * kStatusWords);
+    L.rowptr = take(sizeof(int64_t) * ((size_t)n_orb + 1));
+    L.col = take(sizeof(int32_t) * nnz);
+    L.val = take(sizeof(double2) * nnz);
+    L.orp = take(sizeof(uint32_t) * ((size_t)n_orb + 1));
+    L.ocol = has_onsite ? take(sizeof(int32_t) * nnz_off) : L.col;
+    L.oidx = take(sizeof(uint16_t) * nnz_off);
+    L.vtab = take(sizeof(double2) * kTableMax);
+    L.diag = has_onsite ? take(sizeof(double) * (size_t)n_orb) : 0;
+    L.total = o;
+    return L;
+}
+
+struct ScratchLayout {
+    size_t cnt, cur, bsum, slots, flag, slot_id, total;
+};
+
+ScratchLayout scratch_layout(int64_t n_orb)
+{
+    ScratchLayout L{};
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes ? bytes : 1); return at; };
+    const size_t scan_n = (size_t)std::max<int64_t>(n_orb + 1, kHashSlots + 1);
+    L.cnt = take(sizeof(int32_t) * ((size_t)n_orb + 1));
+    L.cur = take(sizeof(int32_t) * ((size_t)n_orb + 1));
+    L.bsum = take(sizeof(int64_t) * (scan_n / kScanTile + 2));
+    L.slots = take(sizeof(uint32_t) * kHashSlots);
+    L.flag = take(sizeof(int32_t) * (kHashSlots + 1));
+    L.slot_id = take(sizeof(int64_t) * (kHashSlots + 1));
+    L.total = o;
+    return L;
+}
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+bool aligned256(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 255u) == 0; }
+
+}  // namespace
+
+extern "C" int tbpm_build_bytes(int64_t n_orb, int64_t n_hop, int has_onsite, uint32_t flags, size_t *persist_bytes,
+                                size_t *scratch_bytes)
+{
+    if (n_orb < 0 || n_hop < 0 || n_orb >= (int64_t(1) << 31)) return TBPM_EINVAL;
+    const int64_t nnz = n_hop * ((flags & TBPM_HOPS_FULL) ? 1 : 2) + (has_onsite ? n_orb : 0);
+    if (nnz >= (int64_t(1) << 32) - 1) return TBPM_EINVAL;   // 32-bit row offsets in the kernel layout
+    if (persist_bytes) *persist_bytes = persist_layout(n_orb, n_hop, has_onsite != 0, flags).total;
+    if (scratch_bytes) *scratch_bytes = scratch_layout(n_orb).total;
+    return TBPM_OK;
+}
+
+extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, const int32_t *hop_i, const int32_t *hop_j,
+                          const double *hop_val, uint32_t flags, void *persist, size_t persist_bytes, void *scratch,
+                          size_t scratch_bytes, void *stream, tbpm_ham **out)
+{
+    if (!out) return TBPM_EINVAL;
+    *out = nullptr;
+    size_t need_p = 0, need_s = 0;
+    int rc = tbpm_build_bytes(n_orb, n_hop, onsite != nullptr, flags, &need_p, &need_s);
+    if (rc) return rc;
+    if (!persist || !scratch || !aligned256(persist) || !aligned256(scratch)) return TBPM_EINVAL;
+    if (n_hop > 0 && (!hop_i || !hop_j || !hop_val || !aligned16(hop_val))) return TBPM_EINVAL;
+    if (persist_bytes < need_p || scratch_bytes < need_s) return TBPM_ENOMEM;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int has_onsite = onsite != nullptr;
+    const int full = (flags & TBPM_HOPS_FULL) ? 1 : 0;
+
+    tbpm_ham *H = new (std::nothrow) tbpm_ham();
+    if (!H) return TBPM_ENOMEM;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { delete H; note_cuda_error(cudaGetLastError()); return TBPM_ECUDA; }
+    cudaDeviceGetAttribute(&H->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    H->device = dev;
+    H->n_orb = n_orb;
+    H->n_hop = n_hop;
+    H->has_onsite = has_onsite;
+    H->flags = flags;
+    H->nnz_off = n_hop * (full ? 1 : 2);
+    H->nnz = H->nnz_off + (has_onsite ? n_orb : 0);
+
+    char *P = static_cast<char *>(persist), *S = static_cast<char *>(scratch);
+    PersistLayout PL = persist_layout(n_orb, n_hop, has_onsite, flags);
+    ScratchLayout SL = scratch_layout(n_orb);
+    H->status = reinterpret_cast<int32_t *>(P + PL.status);
+    H->rowptr = reinterpret_cast<int64_t *>(P + PL.rowptr);
+    H->col = reinterpret_cast<int32_t *>(P + PL.col);
+    H->val = reinterpret_cast<double2 *>(P + PL.val);
+    H->orp = reinterpret_cast<uint32_t *>(P + PL.orp);
+    H->ocol = reinterpret_cast<int32_t *>(P + PL.ocol);
+    H->oidx = reinterpret_cast<uint16_t *>(P + PL.oidx);
+    H->vtab = reinterpret_cast<double2 *>(P + PL.vtab);
+    H->diag = has_onsite ? reinterpret_cast<double *>(P + PL.diag) : nullptr;
+    int32_t *cnt = reinterpret_cast<int32_t *>(S + SL.cnt);
+    int32_t *cur = reinterpret_cast<int32_t *>(S + SL.cur);
+    int64_t *bsum = reinterpret_cast<int64_t *>(S + SL.bsum);
+    uint32_t *slots = reinterpret_cast<uint32_t *>(S + SL.slots);
+    int32_t *flag = reinterpret_cast<int32_t *>(S + SL.flag);
+    int64_t *slot_id = reinterpret_cast<int64_t *>(S + SL.slot_id);
+
+    auto fail = [&](int code) { delete H; return code; };
+#define TRY_OR_FAIL(expr)                                                       \
+    do {                                                                        \
+        cudaError_t e__ = (expr);                                               \
+        if (e__ != cudaSuccess) { note_cuda_error(e__); return fail(TBPM_ECUDA); } \
+    } while (0)
+
+    TRY_OR_FAIL(cudaMemsetAsync(H->status, 0, sizeof(int32_t) * kStatusWords, st));
+    const unsigned gr = blocks_for(n_orb + 1, kThreads), gh = blocks_for(n_hop, kThreads);
+    k_init_counts<<<gr, kThreads, 0, st>>>(cnt, n_orb, has_onsite);
+    count_launches(1 + (n_hop > 0 ? 2 : 0) + (n_orb > 0 ? 2 : 0) + 1);   // init, count, fill, fill_diag, sort, strip
+    if (n_hop > 0) k_count<<<gh, kThreads, 0, st>>>(n_hop, hop_i, hop_j, n_orb, full, cnt, H->status);
+    if ((rc = scan_exclusive(cnt, n_orb + 1, H->rowptr, bsum, st)) != TBPM_OK) return fail(rc);
+    if (n_orb > 0) k_fill_diag<<<gr, kThreads, 0, st>>>(n_orb, onsite, H->rowptr, H->col, H->val, cur);
+    if (n_hop > 0)
+        k_fill<<<gh, kThreads, 0, st>>>(n_hop, hop_i, hop_j, reinterpret_cast<const double2 *>(hop_val), n_orb, full, H->rowptr,
+                                        cur, H->col, H->val, H->status);
+    if (n_orb > 0) k_sort_rows<<<gr, kThreads, 0, st>>>(n_orb, H->rowptr, H->col, H->val, H->status);
+    k_strip<<<gr, kThreads, 0, st>>>(n_orb, has_onsite, H->rowptr, H->col, H->val, H->orp, H->ocol, H->diag);
+    const bool want_table = !(flags & TBPM_NO_TABLE) && H->nnz_off > 0;
+    if (want_table) {
+        TRY_OR_FAIL(cudaMemsetAsync(slots, 0xFF, sizeof(uint32_t) * kHashSlots, st));
+        k_tab_insert<<<gr, kThreads, 0, st>>>(n_orb, has_onsite, H->rowptr, H->col, H->val, slots, H->status);
+        count_launches(1);
+    }
+    TRY_OR_FAIL(cudaGetLastError());
+
+    int32_t hst[kStatusWords];
+    TRY_OR_FAIL(cudaMemcpyAsync(hst, H->status, sizeof(hst), cudaMemcpyDeviceToHost, st));
+    TRY_OR_FAIL(cudaStreamSynchronize(st));
+    if (hst[ST_ERR] & 1) return fail(TBPM_EINDEX);
+    if (hst[ST_ERR] & 2) return fail(TBPM_EDIAG);
+    if (hst[ST_ERR] & 4) return fail(TBPM_EDUP);
+    H->max_row_nnz = hst[ST_MAX_ROW];
+    uint64_t gb = (uint64_t)(uint32_t)hst[ST_GERSH_LO] | ((uint64_t)(uint32_t)hst[ST_GERSH_HI] << 32);
+    std::memcpy(&H->gershgorin, &gb, sizeof(double));
+    H->n_table = 0;
+    if (want_table && !hst[ST_TAB_OVERFLOW] && hst[ST_NTAB] <= kTableMax) {
+        k_tab_flags<<<blocks_for(kHashSlots + 1, kThreads), kThreads, 0, st>>>(slots, flag);
+        if ((rc = scan_exclusive(flag, kHashSlots + 1, slot_id, bsum, st)) != TBPM_OK) return fail(rc);
+        k_tab_number<<<blocks_for(kHashSlots, kThreads), kThreads, 0, st>>>(slots, slot_id, H->val, H->vtab);
+        k_tab_lookup<<<gr, kThreads, 0, st>>>(n_orb, has_onsite, H->rowptr, H->col, H->val, slots, slot_id, H->oidx);
+        count_launches(3);
+        TRY_OR_FAIL(cudaGetLastError());
+        TRY_OR_FAIL(cudaStreamSynchronize(st));
+        H->n_table = hst[ST_NTAB];
+    }
+#undef TRY_OR_FAIL
+    *out = H;
+    return TBPM_OK;
+}
+
+extern "C" int tbpm_ham_info(const tbpm_ham *H, int64_t *n_orb, int64_t *nnz, int32_t *max_row_nnz, size_t *matrix_bytes_per_term,
+                             int32_t *n_table, double *gershgorin)
+{
+    if (!H) return TBPM_EINVAL;
+    if (n_orb) *n_orb = H->n_orb;
+    if (nnz) *nnz = H->nnz;
+    if (max_row_nnz) *max_row_nnz = H->max_row_nnz;
+    if (matrix_bytes_per_term) {
+        if (H->n_table > 0)   // 32-bit row offsets + (int32 column + uint16 value index) per off-diagonal entry + real diagonal
+            *matrix_bytes_per_term = sizeof(uint32_t) * ((size_t)H->n_orb + 1) + (size_t)H->nnz_off * (sizeof(int32_t) + sizeof(uint16_t)) +
+                                     (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0) + sizeof(double2) * (size_t)H->n_table;
+        else                  // canonical CSR: int64 row pointers + (int32 column + complex128 value) per entry
+            *matrix_bytes_per_term = sizeof(int64_t) * ((size_t)H->n_orb + 1) + (size_t)H->nnz * (sizeof(int32_t) + sizeof(double2));
+    }
+    if (n_table) *n_table = H->n_table;
+    if (gershgorin) *gershgorin = H->gershgorin;
+    return TBPM_OK;
+}
+
+extern "C" int tbpm_check_bound(const tbpm_ham *H, double rescale)
+{
+    if (!H || !(rescale > 0.0)) return TBPM_EINVAL;
+    // the row sums are rounded: allow a few ulps so that an exact equality (config 4: 4*1 + 4*0.2 = 4.8) passes
+    return H->gershgorin > rescale * (1.0 + 8 * 2.220446049250313e-16) ? TBPM_EBOUND : TBPM_OK;
+}
+
+extern "C" int tbpm_export_csr(const tbpm_ham *H, int64_t *rowptr, int32_t *col, double *val, void *stream)
+{
+    if (!H || !rowptr || (H->nnz > 0 && (!col || !val))) return TBPM_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    TBPM_CUDA_TRY(cudaMemcpyAsync(rowptr, H->rowptr, sizeof(int64_t) * ((size_t)H->n_orb + 1), cudaMemcpyDeviceToDevice, st));
+    if (H->nnz > 0) {
+        TBPM_CUDA_TRY(cudaMemcpyAsync(col, H->col, sizeof(int32_t) * (size_t)H->nnz, cudaMemcpyDeviceToDevice, st));
+        TBPM_CUDA_TRY(cudaMemcpyAsync(val, H->val, sizeof(double2) * (size_t)H->nnz, cudaMemcpyDeviceToDevice, st));
+    }
+    return TBPM_OK;
+}
+
+extern "C" void tbpm_free(tbpm_ham *H) { delete H; }

@@ -1,0 +1,136 @@
+// capi.cu -- the remaining C-ABI entry points: error strings and the end-to-end call on HOST buffers.
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+
+#include "tbpm_internal.h"
+
+using namespace tbpm_detail;
+
+namespace {
+thread_local char g_cuda_msg[256] = "CUDA runtime error";
+std::atomic<long long> g_total_launches{0};
+}
+
+void tbpm_detail::note_cuda_error(cudaError_t e)
+{
+    std::snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA runtime error: %s (%s)", cudaGetErrorName(e), cudaGetErrorString(e));
+}
+
+void tbpm_detail::count_launches(int n) { g_total_launches.fetch_add(n, std::memory_order_relaxed); }
+
+extern "C" int64_t tbpm_total_launch_count(void) { return (int64_t)g_total_launches.load(std::memory_order_relaxed); }
+
+extern "C" const char *tbpm_strerror(int code)
+{
+    switch (code) {
+    case TBPM_OK: return "success";
+    case TBPM_EINVAL: return "invalid argument (null, negative, misaligned, n_orb >= 2^31 or nnz >= 2^32 - 1)";
+    case TBPM_EINDEX: return "hop or site index out of range";
+    case TBPM_EDIAG: return "hop with i == j is illegal; on-site energies go into `onsite` (PAPER.md:177-179)";
+    case TBPM_EDUP: return "duplicate (row, col) pair in the hopping list";
+    case TBPM_ENOMEM: return "caller-provided buffer too small";
+    case TBPM_ECUDA: return g_cuda_msg;
+    case TBPM_EBOUND: return "Gershgorin bound of H exceeds rescale: the Chebyshev recursion would diverge";
+    }
+    return "unknown error code";
+}
+
+extern "C" const char *tbpm_version(void) { return "tbpm-b200 0.1 (sm_100a)"; }
+
+namespace {
+
+struct Arena {
+    size_t hop_i, hop_j, hop_val, onsite, psi0, corr, norm2, persist, scratch, workspace, total;
+    size_t persist_bytes, scratch_bytes, workspace_bytes;
+};
+
+int arena_layout(int64_t n_orb, int64_t n_hop, int has_onsite, int n_state, int n_step, uint32_t flags, Arena *A)
+{
+    if (n_state < 0 || n_step < 0) return TBPM_EINVAL;
+    int rc = tbpm_build_bytes(n_orb, n_hop, has_onsite, flags, &A->persist_bytes, &A->scratch_bytes);
+    if (rc) return rc;
+    tbpm_ham tmp;                                        // only n_orb matters for the workspace size
+    tmp.n_orb = n_orb;
+    if ((rc = tbpm_propagate_bytes(&tmp, n_state, &A->workspace_bytes))) return rc;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes ? bytes : 1); return at; };
+    A->hop_i = take(sizeof(int32_t) * (size_t)n_hop);
+    A->hop_j = take(sizeof(int32_t) * (size_t)n_hop);
+    A->hop_val = take(sizeof(double) * 2 * (size_t)n_hop);
+    A->onsite = take(has_onsite ? sizeof(double) * (size_t)n_orb : 0);
+    A->psi0 = take(sizeof(double) * 2 * (size_t)n_orb * (size_t)n_state);
+    A->corr = take(sizeof(double) * 2 * (size_t)n_state * (size_t)n_step);
+    A->norm2 = take(sizeof(double) * (size_t)n_state * (size_t)n_step);
+    A->persist = take(A->persist_bytes);
+    A->scratch = take(A->scratch_bytes);
+    A->workspace = take(A->workspace_bytes);
+    A->total = o;
+    return TBPM_OK;
+}
+
+}  // namespace
+
+extern "C" int tbpm_corr_host_bytes(int64_t n_orb, int64_t n_hop, int has_onsite, int n_state, int n_step, uint32_t flags,
+                                    size_t *arena_bytes)
+{
+    if (!arena_bytes) return TBPM_EINVAL;
+    Arena A{};
+    int rc = arena_layout(n_orb, n_hop, has_onsite, n_state, n_step, flags, &A);
+    if (rc) return rc;
+    *arena_bytes = A.total;
+    return TBPM_OK;
+}
+
+extern "C" int tbpm_corr_host(int64_t n_orb, const double *onsite, int64_t n_hop, const int32_t *hop_i, const int32_t *hop_j,
+                              const double *hop_val, uint32_t flags, const double *psi0, int n_state, int n_step, double dt,
+                              double rescale, double *corr, double *norm2, void *arena, size_t arena_bytes, void *stream,
+                              size_t *h2d_bytes, size_t *d2h_bytes)
+{
+    Arena A{};
+    int rc = arena_layout(n_orb, n_hop, onsite != nullptr, n_state, n_step, flags, &A);
+    if (rc) return rc;
+    if (!arena || (reinterpret_cast<uintptr_t>(arena) & 255u)) return TBPM_EINVAL;
+    if (arena_bytes < A.total) return TBPM_ENOMEM;
+    if (n_hop > 0 && (!hop_i || !hop_j || !hop_val)) return TBPM_EINVAL;
+    if (n_state > 0 && n_step > 0 && (!psi0 || !corr)) return TBPM_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    char *D = static_cast<char *>(arena);
+    size_t up = 0, down = 0;
+    auto h2d = [&](size_t off, const void *src, size_t bytes) -> int {
+        if (bytes == 0) return TBPM_OK;
+        TBPM_CUDA_TRY(cudaMemcpyAsync(D + off, src, bytes, cudaMemcpyHostToDevice, st));
+        up += bytes;
+        return TBPM_OK;
+    };
+    if ((rc = h2d(A.hop_i, hop_i, sizeof(int32_t) * (size_t)n_hop))) return rc;
+    if ((rc = h2d(A.hop_j, hop_j, sizeof(int32_t) * (size_t)n_hop))) return rc;
+    if ((rc = h2d(A.hop_val, hop_val, sizeof(double) * 2 * (size_t)n_hop))) return rc;
+    if (onsite && (rc = h2d(A.onsite, onsite, sizeof(double) * (size_t)n_orb))) return rc;
+    if ((rc = h2d(A.psi0, psi0, sizeof(double) * 2 * (size_t)n_orb * (size_t)n_state))) return rc;
+
+    tbpm_ham *H = nullptr;
+    rc = tbpm_build(n_orb, onsite ? reinterpret_cast<const double *>(D + A.onsite) : nullptr, n_hop,
+                    reinterpret_cast<const int32_t *>(D + A.hop_i), reinterpret_cast<const int32_t *>(D + A.hop_j),
+                    reinterpret_cast<const double *>(D + A.hop_val), flags, D + A.persist, A.persist_bytes, D + A.scratch,
+                    A.scratch_bytes, stream, &H);
+    if (rc) return rc;
+    rc = tbpm_propagate(H, reinterpret_cast<const double *>(D + A.psi0), n_state, n_step, dt, rescale,
+                        reinterpret_cast<double *>(D + A.corr), reinterpret_cast<double *>(D + A.norm2), D + A.workspace,
+                        A.workspace_bytes, stream);
+    tbpm_free(H);
+    if (rc) return rc;
+    const size_t nc = (size_t)n_state * (size_t)n_step;
+    if (nc > 0) {
+        TBPM_CUDA_TRY(cudaMemcpyAsync(corr, D + A.corr, sizeof(double) * 2 * nc, cudaMemcpyDeviceToHost, st));
+        down += sizeof(double) * 2 * nc;
+        if (norm2) {
+            TBPM_CUDA_TRY(cudaMemcpyAsync(norm2, D + A.norm2, sizeof(double) * nc, cudaMemcpyDeviceToHost, st));
+            down += sizeof(double) * nc;
+        }
+    }
+    TBPM_CUDA_TRY(cudaStreamSynchronize(st));
+    if (h2d_bytes) *h2d_bytes = up;
+    if (d2h_bytes) *d2h_bytes = down;
+    return TBPM_OK;
+}

@@ -1,0 +1,493 @@
+// propagate.cu -- steps a2-a8 of the path: Chebyshev time propagation with the per-step correlation fused in.
+//
+// What one time step computes (section 2.2.1; coefficients PAPER.md:434):
+//     T_0 = psi,  T_1 = (1/s) H T_0,  T_k = (2/s) H T_{k-1} - T_{k-2}   [amxsy, in place over T_{k-2}]
+//     psi' = sum_{k<K} c_k T_k                                           [axpy with the complex coefficient]
+//     corr = <psi0|psi'>,  norm2 = <psi'|psi'>                           [calc_corr_dos, PAPER.md:965-971]
+//
+// B200 design (differs from the paper's amxsy + axpy pair):
+//   * ONE kernel per Chebyshev term does the SpMV, the subtraction, the accumulation into psi' and (last term) the
+//     two dot products.  Vectors of a tile of BT states are interleaved [row][state] so that H is read once per row
+//     for all BT states (SpMM) and every gather of x[col] is BT*16 contiguous bytes (128-bit loads).
+//   * psi' is touched only every third term: at term k the thread already holds T_k (just computed) and T_{k-2}
+//     (the y it read) and reads T_{k-1}[row] (an L1/L2 hit: the same line is being gathered by the neighbouring
+//     rows), so three terms are added at once.  Vector traffic falls from 5 to 3.67 streams per term.
+//   * H is read from the compressed kernel layout built by build.cu (32-bit row offsets, int32 column, 16-bit index
+//     into the table of distinct hopping values, real diagonal).
+//   * Persistent grid (blocks = SMs x resident blocks), rows handed out grid-strided so that all SMs sweep one moving
+//     window of the vectors (L2 locality of the gather); streaming operands use evict-first loads/stores.
+//   * Reductions are deterministic: per-thread sums -> warp shuffles -> shared memory -> one partial per block, then a
+//     second tiny kernel adds the block partials in a fixed order.  No floating-point atomics anywhere.
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <vector>
+
+#include "tbpm_internal.h"
+
+using namespace tbpm_detail;
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kMaxBT = 32;
+constexpr int kMaxGrid = 4096;                       // upper bound on the persistent grid (partials are sized for it)
+constexpr size_t kHeaderBytes = 256;
+constexpr size_t kPartialBytes = sizeof(double) * 3 * kMaxBT * kMaxGrid;
+
+thread_local int64_t g_launches = 0;
+
+enum TermFlags { F_SUB_Y = 1, F_WRITE_Y = 2, F_SKIP_H = 4, F_ACC_INIT = 8, F_REDUCE = 16 };
+
+struct TermParams {
+    // matrix (kernel layout or canonical CSR)
+    const uint32_t *orp;
+    const int32_t *ocol;
+    const uint16_t *oidx;
+    const double2 *vtab;
+    const double *diag;
+    const int64_t *rowptr;
+    const int32_t *col;
+    const double2 *val;
+    int64_t n_orb;
+    // vectors of this tile, [row][BT]
+    const double2 *x;      // T_{k-1}
+    double2 *y;            // T_{k-2} in, T_k out (in place)
+    double2 *acc;          // psi'
+    const double2 *psi0;   // bra of the correlation
+    double *partial;       // [grid][BT][3]
+    double a;              // 1/s (k = 1) or 2/s
+    double2 ca, cb, cc;    // coefficients of T_k, T_{k-1}, T_{k-2} in this flush
+    int n_acc;             // 0: psi' untouched; 1..3 terms added
+    int flags;
+};
+
+struct WsHeader {          // first bytes of the workspace; read by tbpm_get_state's kernel
+    int64_t n_orb;
+    int32_t n_state;
+    int32_t tile;          // states per full tile
+    int64_t vec0_off;      // byte offset of the first tile's buffers
+    int32_t final_slot;    // which of the three rotating buffers holds psi
+    int32_t pad;
+};
+
+__device__ __forceinline__ double2 ld_stream(const double2 *p)
+{
+    double2 r;
+    asm volatile("ld.global.cs.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream(double2 *p, double2 v)
+{
+    asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void cfma(double2 &h, double2 v, double2 x)
+{
+    h.x = fma(v.x, x.x, h.x);
+    h.x = fma(-v.y, x.y, h.x);
+    h.y = fma(v.x, x.y, h.y);
+    h.y = fma(v.y, x.x, h.y);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// The fused Chebyshev term.  Thread -> (row, state b): BT consecutive threads share a row.
+// ---------------------------------------------------------------------------------------------------------------------
+template <int BT, bool TABLE>
+__global__ void __launch_bounds__(kThreads) k_cheb_term(const TermParams p)
+{
+    constexpr int kRowsPerBlock = kThreads / BT;
+    const int b = threadIdx.x % BT;
+    const int64_t stride = (int64_t)gridDim.x * kRowsPerBlock;
+    const int flags = p.flags;
+    const int n_acc = p.n_acc;
+    double s_re = 0.0, s_im = 0.0, s_nn = 0.0;
+
+    for (int64_t row = (int64_t)blockIdx.x * kRowsPerBlock + threadIdx.x / BT; row < p.n_orb; row += stride) {
+        const int64_t e = row * BT + b;
+        double2 h = make_double2(0.0, 0.0);
+        double2 xrow = make_double2(0.0, 0.0);
+        const bool need_xrow = (flags & F_SKIP_H) || n_acc >= 2 || (TABLE && p.diag != nullptr);
+        if (need_xrow) xrow = __ldg(p.x + e);
+        if (!(flags & F_SKIP_H)) {
+            if (TABLE) {
+                const uint32_t q0 = __ldg(p.orp + row), q1 = __ldg(p.orp + row + 1);
+                uint32_t q = q0;
+                for (; q + 4 <= q1; q += 4) {            // batches of 4 independent gathers
+                    int32_t c[4];
+                    uint16_t vi[4];
+                    double2 xv[4], vv[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { c[u] = __ldg(p.ocol + q + u); vi[u] = __ldg(p.oidx + q + u); }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { xv[u] = __ldg(p.x + (int64_t)c[u] * BT + b); vv[u] = __ldg(p.vtab + vi[u]); }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) cfma(h, vv[u], xv[u]);
+                }
+                {
+                    int32_t c[3];
+                    uint16_t vi[3];
+                    double2 xv[3], vv[3];
+                    const int rem = (int)(q1 - q);
+#pragma unroll
+                    for (int u = 0; u < 3; ++u)
+                        if (u < rem) { c[u] = __ldg(p.ocol + q + u); vi[u] = __ldg(p.oidx + q + u); }
+#pragma unroll
+                    for (int u = 0; u < 3; ++u)
+                        if (u < rem) { xv[u] = __ldg(p.x + (int64_t)c[u] * BT + b); vv[u] = __ldg(p.vtab + vi[u]); }
+#pragma unroll
+                    for (int u = 0; u < 3; ++u)
+                        if (u < rem) cfma(h, vv[u], xv[u]);
+                }
+                if (p.diag != nullptr) {
+                    const double d = __ldg(p.diag + row);
+                    h.x = fma(d, xrow.x, h.x);
+                    h.y = fma(d, xrow.y, h.y);
+                }
+            } else {
+                const int64_t q0 = __ldg(p.rowptr + row), q1 = __ldg(p.rowptr + row + 1);
+                int64_t q = q0;
+                for (; q + 4 <= q1; q += 4) {
+                    int32_t c[4];
+                    double2 xv[4], vv[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { c[u] = __ldg(p.col + q + u); vv[u] = __ldg(p.val + q + u); }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) xv[u] = __ldg(p.x + (int64_t)c[u] * BT + b);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) cfma(h, vv[u], xv[u]);
+                }
+                for (; q < q1; ++q) {
+                    const int32_t c = __ldg(p.col + q);
+                    cfma(h, __ldg(p.val + q), __ldg(p.x + (int64_t)c * BT + b));
+                }
+            }
+            h.x *= p.a;
+            h.y *= p.a;
+        } else {
+            h = xrow;
+        }
+        double2 yold = make_double2(0.0, 0.0);
+        if ((flags & F_SUB_Y) || n_acc == 3) yold = ld_stream(p.y + e);
+        if (flags & F_SUB_Y) { h.x -= yold.x; h.y -= yold.y; }
+        if (flags & F_WRITE_Y) p.y[e] = h;                // T_k: gathered by the next term, keep it cacheable
+        if (n_acc > 0) {
+            double2 s = make_double2(0.0, 0.0);
+            if (!(flags & F_ACC_INIT)) s = ld_stream(p.acc + e);
+            cfma(s, p.ca, h);
+            if (n_acc >= 2) cfma(s, p.cb, xrow);
+            if (n_acc == 3) cfma(s, p.cc, yold);
+            if (flags & F_REDUCE) {
+                const double2 z = ld_stream(p.psi0 + e);
+                s_re = fma(z.x, s.x, s_re);               // conj(z) * s
+                s_re = fma(z.y, s.y, s_re);
+                s_im = fma(z.x, s.y, s_im);
+                s_im = fma(-z.y, s.x, s_im);
+                s_nn = fma(s.x, s.x, s_nn);
+                s_nn = fma(s.y, s.y, s_nn);
+                p.acc[e] = s;                             // psi': T_0 of the next step, gathered right away
+            } else {
+                st_stream(p.acc + e, s);
+            }
+        }
+    }
+
+    if (flags & F_REDUCE) {
+        __shared__ double sm[kThreads / 32][kMaxBT][3];
+#pragma unroll
+        for (int o = 16; o >= BT; o >>= 1) {              // lanes with equal (lane % BT) hold the same state
+            s_re += __shfl_xor_sync(0xffffffffu, s_re, o);
+            s_im += __shfl_xor_sync(0xffffffffu, s_im, o);
+            s_nn += __shfl_xor_sync(0xffffffffu, s_nn, o);
+        }
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        if (lane < BT) { sm[warp][lane][0] = s_re; sm[warp][lane][1] = s_im; sm[warp][lane][2] = s_nn; }
+        __syncthreads();
+        if (threadIdx.x < BT * 3) {
+            const int bb = threadIdx.x / 3, c = threadIdx.x % 3;
+            double t = 0.0;
+#pragma unroll
+            for (int w = 0; w < kThreads / 32; ++w) t += sm[w][bb][c];
+            p.partial[((int64_t)blockIdx.x * BT + bb) * 3 + c] = t;
+        }
+    }
+}
+
+// Sum the block partials in a fixed order: block = state, warp = component, lanes stride over the partials.
+__global__ void k_reduce_final(const double *__restrict__ partial, int n_blocks, int bt, int n_valid, int state0, int n_step, int step,
+                               double *corr, double *norm2)
+{
+    const int bb = blockIdx.x, c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (bb >= n_valid) return;
+    double t = 0.0;
+    for (int k = lane; k < n_blocks; k += 32) t += partial[((int64_t)k * bt + bb) * 3 + c];
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (lane == 0) {
+        const int64_t at = (int64_t)(state0 + bb) * n_step + step;
+        if (c < 2) corr[2 * at + c] = t;
+        else if (norm2) norm2[at] = t;
+    }
+}
+
+// a2: state-major psi0 -> interleaved tile buffers (psi and the bra); states beyond n_valid are zero padding.
+__global__ void k_interleave(const double2 *__restrict__ psi0, int64_t n_orb, int state0, int n_valid, int bt, double2 *psi, double2 *bra)
+{
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_orb * bt) return;
+    const int b = (int)(t % bt);
+    const int64_t row = t / bt;
+    double2 v = make_double2(0.0, 0.0);
+    if (b < n_valid) v = psi0[(int64_t)(state0 + b) * n_orb + row];
+    psi[t] = v;
+    bra[t] = v;
+}
+
+// a8: unit vectors on the given sites
+__global__ void k_unit_states(const int64_t *__restrict__ sites, int state0, int n_valid, int bt, double2 *psi, double2 *bra)
+{
+    int b = threadIdx.x;
+    if (b >= n_valid) return;
+    const int64_t at = sites[state0 + b] * bt + b;
+    psi[at] = make_double2(1.0, 0.0);
+    bra[at] = make_double2(1.0, 0.0);
+}
+
+__global__ void k_write_header(WsHeader *h, WsHeader v) { *h = v; }
+
+__global__ void k_get_state(const char *ws, int state, double2 *out)
+{
+    const WsHeader h = *reinterpret_cast<const WsHeader *>(ws);
+    const int tile = state / h.tile;
+    const int n_rest = h.n_state - tile * h.tile;
+    int bt = h.tile;
+    if (n_rest < h.tile) { bt = 1; while (bt < n_rest) bt <<= 1; }
+    const size_t full_vec = ((size_t)h.n_orb * h.tile * sizeof(double2) + kAlign - 1) / kAlign * kAlign;
+    const size_t this_vec = ((size_t)h.n_orb * bt * sizeof(double2) + kAlign - 1) / kAlign * kAlign;
+    const char *base = ws + h.vec0_off + (size_t)tile * 4 * full_vec + (size_t)h.final_slot * this_vec;
+    const double2 *psi = reinterpret_cast<const double2 *>(base);
+    const int b = state - tile * h.tile;
+    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < h.n_orb; row += (int64_t)gridDim.x * blockDim.x)
+        out[row] = psi[row * bt + b];
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------------------
+int tile_max()
+{
+    int t = 8;                                           // default: 8 states = one 128-byte line per row
+    if (const char *e = std::getenv("TBPM_TILE")) {
+        int v = std::atoi(e);
+        if (v == 1 || v == 2 || v == 4 || v == 8 || v == 16 || v == 32) t = v;
+    }
+    return t;
+}
+
+int pow2_ceil(int n)
+{
+    int p = 1;
+    while (p < n) p <<= 1;
+    return p;
+}
+
+struct Plan {
+    int tile;            // states per full tile
+    int n_tile;
+    int last_bt;         // padded size of the last tile
+    size_t full_vec;     // bytes of one vector buffer of a full tile
+    size_t sites_off, partial_off, vec0_off, total;
+};
+
+Plan make_plan(int64_t n_orb, int n_state)
+{
+    Plan P{};
+    P.tile = std::min(tile_max(), pow2_ceil(std::max(n_state, 1)));
+    P.n_tile = (std::max(n_state, 1) + P.tile - 1) / P.tile;
+    const int rest = std::max(n_state, 1) - (P.n_tile - 1) * P.tile;
+    P.last_bt = pow2_ceil(rest);
+    P.full_vec = align_up((size_t)n_orb * P.tile * sizeof(double2));
+    size_t o = kHeaderBytes;
+    P.sites_off = o;
+    o += align_up(sizeof(int64_t) * (size_t)std::max(n_state, 1));
+    P.partial_off = o;
+    o += kPartialBytes;
+    P.vec0_off = o;
+    o += (size_t)P.n_tile * 4 * P.full_vec;
+    P.total = o;
+    return P;
+}
+
+template <int BT, bool TABLE>
+int launch_term_t(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
+{
+    static int blocks_per_sm = 0;
+    if (blocks_per_sm == 0) {
+        int nb = 0;
+        TBPM_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_cheb_term<BT, TABLE>, kThreads, 0));
+        blocks_per_sm = std::max(nb, 1);
+    }
+    constexpr int kRowsPerBlock = kThreads / BT;
+    const int64_t need = (p.n_orb + kRowsPerBlock - 1) / kRowsPerBlock;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>({need, (int64_t)num_sms * blocks_per_sm, (int64_t)kMaxGrid}));
+    k_cheb_term<BT, TABLE><<<grid, kThreads, 0, st>>>(p);
+    ++g_launches; count_launches(1);
+    *grid_out = grid;
+    return TBPM_OK;
+}
+
+int launch_term(int bt, bool table, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
+{
+#define TBPM_CASE(B)                                                                     \
+    case B:                                                                              \
+        return table ? launch_term_t<B, true>(p, num_sms, st, grid_out) : launch_term_t<B, false>(p, num_sms, st, grid_out);
+    switch (bt) {
+        TBPM_CASE(1)
+        TBPM_CASE(2)
+        TBPM_CASE(4)
+        TBPM_CASE(8)
+        TBPM_CASE(16)
+        TBPM_CASE(32)
+    }
+#undef TBPM_CASE
+    return TBPM_EINVAL;
+}
+
+// Shared body of tbpm_propagate (psi0 != NULL) and tbpm_ldos (sites != NULL).
+int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int n_step, double dt, double rescale, double *corr,
+        double *norm2, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!H || n_state < 0 || n_step < 0 || !(rescale > 0.0) || !(dt >= 0.0) || !std::isfinite(dt) || !std::isfinite(rescale))
+        return TBPM_EINVAL;
+    g_launches = 0;
+    if (n_state == 0 || n_step == 0) return TBPM_OK;
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || !corr || (!psi0 && !sites)) return TBPM_EINVAL;
+    if (psi0 && (reinterpret_cast<uintptr_t>(psi0) & 15u)) return TBPM_EINVAL;
+    if (sites)
+        for (int b = 0; b < n_state; ++b)
+            if (sites[b] < 0 || sites[b] >= H->n_orb) return TBPM_EINDEX;
+    const Plan P = make_plan(H->n_orb, n_state);
+    if (workspace_bytes < P.total) return TBPM_ENOMEM;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+
+    // a1: coefficients (host, once per call)
+    std::vector<double> cf(2 * 8192);
+    int K = 0;
+    int rc = tbpm_cheb_coeff(rescale * dt, 1e-15, 8192, &K, cf.data());
+    if (rc) return rc;
+    auto C = [&](int k) { return make_double2(cf[2 * k], cf[2 * k + 1]); };
+
+    char *W = static_cast<char *>(workspace);
+    double *partial = reinterpret_cast<double *>(W + P.partial_off);
+    int64_t *d_sites = reinterpret_cast<int64_t *>(W + P.sites_off);
+    if (sites) TBPM_CUDA_TRY(cudaMemcpyAsync(d_sites, sites, sizeof(int64_t) * (size_t)n_state, cudaMemcpyHostToDevice, st));
+
+    // psi sits in slot p_n at the start of step n and moves p -> (p + 2) % 3 every step; start so that it ends in slot 0
+    const int start_slot = n_step % 3;
+    WsHeader hdr{H->n_orb, n_state, P.tile, (int64_t)P.vec0_off, 0, 0};
+    k_write_header<<<1, 1, 0, st>>>(reinterpret_cast<WsHeader *>(W), hdr);
+    ++g_launches; count_launches(1);
+
+    const bool table = H->n_table > 0;
+    TermParams tp{};
+    tp.orp = H->orp; tp.ocol = H->ocol; tp.oidx = H->oidx; tp.vtab = H->vtab; tp.diag = H->diag;
+    tp.rowptr = H->rowptr; tp.col = H->col; tp.val = H->val;
+    tp.n_orb = H->n_orb;
+    tp.partial = partial;
+
+    for (int t = 0; t < P.n_tile; ++t) {
+        const int state0 = t * P.tile;
+        const int n_valid = std::min(P.tile, n_state - state0);
+        const int bt = (t == P.n_tile - 1) ? P.last_bt : P.tile;
+        const size_t vec = align_up((size_t)H->n_orb * bt * sizeof(double2));
+        char *base = W + P.vec0_off + (size_t)t * 4 * P.full_vec;
+        double2 *buf[3] = {reinterpret_cast<double2 *>(base), reinterpret_cast<double2 *>(base + vec),
+                           reinterpret_cast<double2 *>(base + 2 * vec)};
+        double2 *bra = reinterpret_cast<double2 *>(base + 3 * vec);
+        const int64_t n_el = H->n_orb * bt;
+        if (n_el > 0) {
+            if (psi0) {
+                k_interleave<<<(unsigned)((n_el + kThreads - 1) / kThreads), kThreads, 0, st>>>(
+                    reinterpret_cast<const double2 *>(psi0), H->n_orb, state0, n_valid, bt, buf[start_slot], bra);
+            } else {
+                TBPM_CUDA_TRY(cudaMemsetAsync(buf[start_slot], 0, sizeof(double2) * (size_t)n_el, st));
+                TBPM_CUDA_TRY(cudaMemsetAsync(bra, 0, sizeof(double2) * (size_t)n_el, st));
+                k_unit_states<<<1, kMaxBT, 0, st>>>(d_sites, state0, n_valid, bt, buf[start_slot], bra);
+            }
+            ++g_launches; count_launches(1);
+        }
+        tp.psi0 = bra;
+        int slot = start_slot;
+        for (int n = 0; n < n_step; ++n) {
+            double2 *psi = buf[slot], *t1 = buf[(slot + 1) % 3], *acc = buf[(slot + 2) % 3];
+            int grid = 1;
+            if (K == 1) {                                 // tau = 0: psi' = c_0 psi, no H application
+                tp.x = psi; tp.y = t1; tp.acc = acc; tp.a = 0.0;
+                tp.ca = C(0); tp.n_acc = 1; tp.flags = F_SKIP_H | F_ACC_INIT | F_REDUCE;
+                if ((rc = launch_term(bt, table, tp, H->num_sms, st, &grid))) return rc;
+            }
+            int flushed = -1;                             // highest term already added to psi'
+            for (int k = 1; k < K; ++k) {
+                // buffers: T_k overwrites T_{k-2}; T_0 = psi, T_1 = t1, T_2 -> psi's buffer, ...
+                tp.x = (k % 2 == 1) ? psi : t1;           // T_{k-1}
+                tp.y = (k % 2 == 1) ? t1 : psi;           // T_{k-2} -> T_k
+                tp.acc = acc;
+                tp.a = (k == 1 ? 1.0 : 2.0) / rescale;
+                int flags = F_WRITE_Y | (k >= 2 ? F_SUB_Y : 0);
+                const bool last = (k == K - 1);
+                tp.n_acc = 0;
+                if (k % 3 == 2 || last) {                 // flush terms flushed+1 .. k (at most 3)
+                    tp.n_acc = k - flushed;
+                    tp.ca = C(k);
+                    tp.cb = tp.n_acc >= 2 ? C(k - 1) : make_double2(0.0, 0.0);
+                    tp.cc = tp.n_acc == 3 ? C(k - 2) : make_double2(0.0, 0.0);
+                    if (flushed < 0) flags |= F_ACC_INIT;
+                    flushed = k;
+                }
+                if (last) { flags |= F_REDUCE; flags &= ~F_WRITE_Y; }   // T_{K-1} is never read again
+                tp.flags = flags;
+                if ((rc = launch_term(bt, table, tp, H->num_sms, st, &grid))) return rc;
+            }
+            k_reduce_final<<<bt, 96, 0, st>>>(partial, grid, bt, n_valid, state0, n_step, n, corr, norm2);
+            ++g_launches; count_launches(1);
+            slot = (slot + 2) % 3;                        // psi' (acc) is the next step's psi
+        }
+    }
+    TBPM_CUDA_TRY(cudaGetLastError());
+    return TBPM_OK;
+}
+
+}  // namespace
+
+extern "C" int tbpm_propagate_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes)
+{
+    if (!H || n_state < 0 || !workspace_bytes) return TBPM_EINVAL;
+    *workspace_bytes = make_plan(H->n_orb, n_state).total;
+    return TBPM_OK;
+}
+
+extern "C" int tbpm_propagate(const tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale, double *corr,
+                              double *norm2, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (n_state > 0 && n_step > 0 && !psi0) return TBPM_EINVAL;
+    return run(H, psi0, nullptr, n_state, n_step, dt, rescale, corr, norm2, workspace, workspace_bytes, stream);
+}
+
+extern "C" int tbpm_ldos(const tbpm_ham *H, const int64_t *sites, int n_site, int n_step, double dt, double rescale, double *corr,
+                         double *norm2, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (n_site > 0 && n_step > 0 && !sites) return TBPM_EINVAL;
+    return run(H, nullptr, sites, n_site, n_step, dt, rescale, corr, norm2, workspace, workspace_bytes, stream);
+}
+
+extern "C" int tbpm_get_state(const tbpm_ham *H, const void *workspace, int state, double *psi_out, void *stream)
+{
+    if (!H || !workspace || !psi_out || state < 0) return TBPM_EINVAL;
+    if (H->n_orb == 0) return TBPM_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int grid = (int)std::min<int64_t>((H->n_orb + kThreads - 1) / kThreads, 4096);
+    k_get_state<<<grid, kThreads, 0, st>>>(static_cast<const char *>(workspace), state, reinterpret_cast<double2 *>(psi_out));
+    count_launches(1);
+    TBPM_CUDA_TRY(cudaGetLastError());
+    return TBPM_OK;
+}
+
+extern "C" int64_t tbpm_last_launch_count(void) { return g_launches; }

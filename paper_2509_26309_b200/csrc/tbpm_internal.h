@@ -1,0 +1,68 @@
+// tbpm_internal.h -- private declarations of libtbpm.so (not part of the C ABI, not shared with oracle/).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/tbpm.h"
+
+#define TBPM_CUDA_TRY(expr)                      \
+    do {                                         \
+        cudaError_t e__ = (expr);                \
+        if (e__ != cudaSuccess) {                \
+            tbpm_detail::note_cuda_error(e__);   \
+            return TBPM_ECUDA;                   \
+        }                                        \
+    } while (0)
+
+namespace tbpm_detail {
+
+void note_cuda_error(cudaError_t e);
+void count_launches(int n);   // process-wide kernel-launch counter (tbpm_total_launch_count)
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a; }
+
+constexpr int kTableMax = 65536;        // distinct hopping values addressable by a 16-bit index
+constexpr int kHashSlots = 1 << 18;     // open-addressing table used while collecting distinct values
+constexpr int kStatusWords = 64;
+
+// status words written by the build kernels (device int32[kStatusWords] at the start of `persist`)
+enum StatusWord {
+    ST_ERR = 0,          // bit 0: index out of range, bit 1: diagonal hop, bit 2: duplicate (row, col)
+    ST_MAX_ROW = 1,      // max entries in a row of the canonical CSR
+    ST_GERSH_LO = 2,     // bits of the double max_i (|onsite_i| + sum_j |H_ij|)   (non-negative doubles order as u64)
+    ST_GERSH_HI = 3,
+    ST_NTAB = 4,         // number of distinct off-diagonal values inserted into the hash table
+    ST_TAB_OVERFLOW = 5  // more than kTableMax distinct values (or a probe sequence gave up)
+};
+
+}  // namespace tbpm_detail
+
+// The handle: a host struct of device pointers into `persist`.
+struct tbpm_ham {
+    int64_t n_orb = 0;
+    int64_t n_hop = 0;
+    int64_t nnz = 0;       // canonical CSR entries
+    int64_t nnz_off = 0;   // off-diagonal entries
+    int has_onsite = 0;
+    uint32_t flags = 0;
+    int32_t max_row_nnz = 0;
+    double gershgorin = 0.0;
+    int32_t n_table = 0;   // 0: kernels read complex128 values from the canonical CSR
+    int device = 0;
+    int num_sms = 0;
+
+    // canonical CSR (device)
+    int64_t *rowptr = nullptr;
+    int32_t *col = nullptr;
+    double2 *val = nullptr;
+    // kernel layout (device): off-diagonal part with 32-bit row offsets, 16-bit value indices and a real diagonal
+    uint32_t *orp = nullptr;
+    int32_t *ocol = nullptr;
+    uint16_t *oidx = nullptr;
+    double2 *vtab = nullptr;
+    double *diag = nullptr;
+    int32_t *status = nullptr;
+};

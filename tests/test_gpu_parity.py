@@ -1,0 +1,324 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle on the same seeded inputs (`-m gpu`).
+
+Bar (BASELINE.json:north_star): hopping-to-sparse index build bit-exact; max |delta corr| <= 1e-10 absolute in fp64;
+|norm2 - 1| <= 1e-12.  Small cases compare every element against the authoritative serial oracle; the full-size
+configs use prefix parity on a sample of states (the first m steps do not depend on n_step, reading #7) against the
+OpenMP row form of the oracle (itself pinned to the serial form), closed-form eigenstates at full size, and the
+norm invariant.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2509_26309_b200 import tbpm, workloads as W
+
+pytestmark = pytest.mark.gpu
+
+CORR_TOL = 1e-10     # north_star
+NORM_TOL = 1e-12     # north_star
+
+
+@pytest.fixture(scope="module")
+def dev():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch.device("cuda:0")
+
+
+def to_np(w):
+    return (w.hop_i.cpu().numpy(), w.hop_j.cpu().numpy(), w.hop_val.cpu().numpy(),
+            None if w.onsite is None else w.onsite.cpu().numpy())
+
+
+def assert_csr_bit_exact(H, oracle_mod, w, hops_full=False):
+    hi, hj, hv, on = to_np(w)
+    orow, ocol, oval = oracle_mod.build_csr(w.n_orb, on, hi, hj, hv, hops_full)
+    rowptr, col, val = tbpm.tbpm_export_csr(H)
+    torch.cuda.synchronize()
+    assert np.array_equal(rowptr.cpu().numpy(), orow)
+    assert np.array_equal(col.cpu().numpy(), ocol)
+    assert np.array_equal(val.cpu().numpy().view(np.uint64), oval.view(np.uint64))   # raw 64-bit patterns (-0.0 matters)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# a0: builder
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,over", [
+    (1, {}),                                           # config 1 at full size
+    (2, dict(Na=96, Nb=70)),                           # with on-site diagonal
+    (3, dict(Na=128, Nb=96)),                          # vacancies: rows of 0..3 entries, empty rows
+    (4, dict(Lx=64, Ly=48, phi_den=32)),               # complex values, 8 per row
+    (5, dict(L=17)),                                   # 7 per row incl. diagonal, ragged tail (4913 rows)
+])
+@pytest.mark.parametrize("flags", [0, tbpm.TBPM_NO_TABLE])
+def test_build_bit_exact(dev, oracle_mod, cfg, over, flags):
+    w = W.make_workload(cfg, device=dev, **over)
+    # the result must not depend on the order of the list
+    perm = torch.randperm(w.n_hop, generator=torch.Generator().manual_seed(cfg)).to(dev)
+    w.hop_i, w.hop_j, w.hop_val = w.hop_i[perm].contiguous(), w.hop_j[perm].contiguous(), w.hop_val[perm].contiguous()
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val, flags | tbpm.TBPM_VALIDATE)
+    assert H.nnz == w.nnz
+    assert_csr_bit_exact(H, oracle_mod, w)
+    hi, hj, hv, on = to_np(w)
+    rowsum = np.zeros(w.n_orb)
+    np.add.at(rowsum, hi, np.abs(hv))
+    np.add.at(rowsum, hj, np.abs(hv))
+    if on is not None:
+        rowsum += np.abs(on)
+    assert H.gershgorin == pytest.approx(rowsum.max(), rel=1e-12)
+    assert tbpm.tbpm_check_bound(H, w.rescale) == tbpm.TBPM_OK        # config 4: equality is allowed
+    assert tbpm.tbpm_check_bound(H, 0.5 * w.rescale) == tbpm.TBPM_EBOUND
+    if flags & tbpm.TBPM_NO_TABLE:
+        assert H.n_table == 0
+    else:
+        assert H.n_table == len(set(zip(np.concatenate([hv.real, hv.real]).view(np.uint64).tolist(),
+                                        np.concatenate([hv.imag, -hv.imag]).view(np.uint64).tolist())))
+
+
+def test_build_edge_cases(dev, oracle_mod):
+    i32 = lambda a: torch.tensor(a, dtype=torch.int32, device=dev)
+    c128 = lambda a: torch.tensor(a, dtype=torch.complex128, device=dev)
+    # both orientations supplied by the caller
+    w = W.Workload("full", 3, i32([0, 1, 1, 2]), i32([1, 0, 2, 1]), c128([1 + 2j, 1 - 2j, 3j, -3j]), None, 1, 1, 1.0)
+    H = tbpm.tbpm_build(3, None, w.hop_i, w.hop_j, w.hop_val, tbpm.TBPM_HOPS_FULL)
+    assert_csr_bit_exact(H, oracle_mod, w, hops_full=True)
+    # no hops at all, with and without diagonal; zero orbitals
+    e = W.Workload("empty", 5, i32([]), i32([]), c128([]), None, 1, 1, 1.0)
+    H = tbpm.tbpm_build(5, None, e.hop_i, e.hop_j, e.hop_val)
+    assert H.nnz == 0 and tbpm.tbpm_export_csr(H)[0].tolist() == [0] * 6
+    e.onsite = torch.linspace(-1, 1, 5, dtype=torch.float64, device=dev)
+    H = tbpm.tbpm_build(5, e.onsite, e.hop_i, e.hop_j, e.hop_val)
+    assert_csr_bit_exact(H, oracle_mod, e)
+    H = tbpm.tbpm_build(0, None, e.hop_i, e.hop_j, e.hop_val)
+    assert H.nnz == 0 and H.n_orb == 0
+    # one long row (star graph): max_row_nnz, sorting of a long segment
+    n = 3000
+    star = W.Workload("star", n, i32(list(range(1, n))[::-1]), i32([0] * (n - 1)),
+                      torch.full((n - 1,), 0.001 + 0.002j, dtype=torch.complex128, device=dev), None, 1, 1, 10.0)
+    H = tbpm.tbpm_build(n, None, star.hop_i, star.hop_j, star.hop_val)
+    assert H.max_row_nnz == n - 1
+    assert_csr_bit_exact(H, oracle_mod, star)
+    # errors
+    for hi, hj, code in (([1], [1], tbpm.TBPM_EDIAG), ([0, 1], [1, 0], tbpm.TBPM_EDUP), ([0, 0], [1, 1], tbpm.TBPM_EDUP),
+                         ([0], [3], tbpm.TBPM_EINDEX), ([-1], [2], tbpm.TBPM_EINDEX)):
+        with pytest.raises(tbpm.TbpmError) as ei:
+            tbpm.tbpm_build(3, None, i32(hi), i32(hj), c128([1.0] * len(hi)), tbpm.TBPM_VALIDATE)
+        assert ei.value.code == code
+
+
+def test_table_overflow_falls_back_to_full_values(dev, oracle_mod):
+    # > 65536 distinct hopping values: the kernels must read complex128 values from the canonical CSR
+    n = 70001
+    i = torch.arange(n - 1, dtype=torch.int32, device=dev)
+    vals = torch.complex(torch.linspace(0.1, 0.9, n - 1, dtype=torch.float64, device=dev),
+                         torch.linspace(-0.3, 0.3, n - 1, dtype=torch.float64, device=dev))
+    w = W.Workload("many", n, i, i + 1, vals, None, 2, 8, 2.0)
+    H = tbpm.tbpm_build(n, None, w.hop_i, w.hop_j, w.hop_val)
+    assert H.n_table == 0
+    assert_csr_bit_exact(H, oracle_mod, w)
+    psi0 = w.psi0(device=dev)
+    corr, norm2, _ = tbpm.tbpm_propagate(H, psi0, 8, w.dt, w.rescale)
+    hi, hj, hv, on = to_np(w)
+    ref, _ = oracle_mod.propagate(n, on, hi, hj, hv, psi0.cpu().numpy(), 8, w.dt, w.rescale)
+    assert np.abs(corr.cpu().numpy() - ref).max() <= CORR_TOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# a1-a7: propagate, every element against the serial oracle
+# ---------------------------------------------------------------------------------------------------------------------
+def run_parity(dev, oracle_mod, w, n_state, n_step, flags=0, dt=None, check_state=True):
+    dt = w.dt if dt is None else dt
+    psi0 = w.psi0(device=dev, n_state=n_state)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val, flags)
+    corr, norm2, ws = tbpm.tbpm_propagate(H, psi0, n_step, dt, w.rescale)
+    hi, hj, hv, on = to_np(w)
+    ref, refn, reff = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0.cpu().numpy(), n_step, dt, w.rescale, return_state=True)
+    assert np.abs(corr.cpu().numpy() - ref).max() <= CORR_TOL
+    assert np.abs(norm2.cpu().numpy() - refn).max() <= NORM_TOL
+    assert np.abs(norm2.cpu().numpy() - 1).max() <= NORM_TOL
+    if check_state:
+        for b in sorted({0, n_state - 1}):
+            got = tbpm.tbpm_get_state(H, ws, b).cpu().numpy()
+            assert np.abs(got - reff[b]).max() <= 1e-12
+    return H, psi0, corr, norm2
+
+
+def test_config1_full_length(dev, oracle_mod):
+    """BASELINE.json:configs[0] exactly: honeycomb 64x64, 1 state, 256 steps, s = 9, tau = pi."""
+    w = W.make_workload(1, device=dev)
+    H, _, corr, _ = run_parity(dev, oracle_mod, w, 1, 256)
+    assert corr.shape == (1, 256)
+    assert H.n_table == 2                                            # t and conj(t) = (t, -0.0)
+    assert tbpm.tbpm_last_launch_count() == 256 * 21 + 2             # 20 terms + 1 final reduction per step
+
+
+@pytest.mark.parametrize("cfg,over,n_state,n_step", [
+    (2, dict(Na=96, Nb=70), 4, 24),                                  # 13440 rows: several blocks + ragged tail
+    (2, dict(Na=33, Nb=35), 3, 9),                                   # 3 states -> padded tile of 4
+    (3, dict(Na=128, Nb=96), 1, 24),                                 # irregular rows 0..3, empty rows
+    (3, dict(Na=100, Nb=60), 2, 7),
+    (4, dict(Lx=64, Ly=48, phi_den=32), 8, 24),                      # complex hops, SpMM tile of 8, s = ||H||
+    (4, dict(Lx=32, Ly=24, phi_den=8), 5, 6),                        # 5 states -> padded tile of 8
+    (5, dict(L=17), 32, 12),                                         # 4 tiles of 8
+    (5, dict(L=12), 11, 5),                                          # tile of 8 + padded tile of 4
+])
+@pytest.mark.parametrize("flags", [0, tbpm.TBPM_NO_TABLE])
+def test_small_configs_every_element(dev, oracle_mod, cfg, over, n_state, n_step, flags):
+    w = W.make_workload(cfg, device=dev, **over)
+    run_parity(dev, oracle_mod, w, n_state, n_step, flags)
+
+
+@pytest.mark.parametrize("tile", ["1", "2", "4", "16", "32"])
+def test_other_tile_widths(dev, oracle_mod, tile, monkeypatch):
+    monkeypatch.setenv("TBPM_TILE", tile)
+    w = W.make_workload(5, device=dev, L=13)
+    run_parity(dev, oracle_mod, w, 35 if tile in ("16", "32") else 7, 6)
+    w = W.make_workload(4, device=dev, Lx=48, Ly=32, phi_den=16)
+    run_parity(dev, oracle_mod, w, 33 if tile == "32" else 6, 5, tbpm.TBPM_NO_TABLE)
+
+
+@pytest.mark.parametrize("tau,K", [(0.0, 1), (1e-9, None), (math.pi / 2, 16), (2 * math.pi, 28), (1.0, None), (5.3, None)])
+def test_other_time_steps(dev, oracle_mod, tau, K):
+    """Different K exercise every flush pattern of the deferred accumulation (1, 2 or 3 pending terms; K = 1, 2)."""
+    w = W.make_workload(2, device=dev, Na=40, Nb=36)
+    if K is not None:
+        assert len(tbpm.tbpm_cheb_coeff(tau)) == K
+    run_parity(dev, oracle_mod, w, 2, 7, dt=tau / w.rescale)
+
+
+def test_prefix_determinism_and_edge_calls(dev, oracle_mod):
+    w = W.make_workload(4, device=dev, Lx=64, Ly=64, phi_den=64)
+    psi0 = w.psi0(device=dev, n_state=8)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    a, an, _ = tbpm.tbpm_propagate(H, psi0, 12, w.dt, w.rescale)
+    b, bn, _ = tbpm.tbpm_propagate(H, psi0, 12, w.dt, w.rescale)
+    c, cn, _ = tbpm.tbpm_propagate(H, psi0, 5, w.dt, w.rescale)
+    assert torch.equal(a, b) and torch.equal(an, bn)                 # run-to-run bit identical (no float atomics)
+    assert torch.equal(a[:, :5], c) and torch.equal(an[:, :5], cn)   # prefix property (reading #7)
+    corr, norm2, _ = tbpm.tbpm_propagate(H, psi0, 0, w.dt, w.rescale)  # n_step = 0: success, nothing written
+    assert corr.shape == (8, 0)
+    corr = torch.full((2, 3), 7.0, dtype=torch.complex128, device=dev)
+    tbpm.tbpm_propagate(H, psi0[:0], 3, w.dt, w.rescale, corr=corr)    # n_state = 0: outputs untouched
+    assert torch.all(corr == 7.0)
+    with pytest.raises(tbpm.TbpmError):
+        tbpm.tbpm_propagate(H, psi0, 3, w.dt, -1.0)
+    small = torch.empty(1024, dtype=torch.uint8, device=dev)
+    with pytest.raises(tbpm.TbpmError) as ei:
+        tbpm.tbpm_propagate(H, psi0, 3, w.dt, w.rescale, workspace=small)
+    assert ei.value.code == tbpm.TBPM_ENOMEM
+    # norm2 = NULL is allowed
+    d, dn, _ = tbpm.tbpm_propagate(H, psi0, 5, w.dt, w.rescale, want_norm=False)
+    assert dn is None and torch.equal(d, c)
+
+
+def test_windowed_parity_from_snapshot(dev, oracle_mod):
+    """Reading/§8(d)(3): download psi at a late step from the GPU, let the oracle advance it and compare the window."""
+    w = W.make_workload(2, device=dev, Na=64, Nb=48)
+    psi0 = w.psi0(device=dev, n_state=2)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    j, m = 200, 6
+    full, _, _ = tbpm.tbpm_propagate(H, psi0, j + m, w.dt, w.rescale)
+    _, _, ws = tbpm.tbpm_propagate(H, psi0, j, w.dt, w.rescale)
+    snap = torch.stack([tbpm.tbpm_get_state(H, ws, b) for b in range(2)]).cpu().numpy()
+    hi, hj, hv, on = to_np(w)
+    ref, _ = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0.cpu().numpy(), m, w.dt, w.rescale, psi_start=snap)
+    assert np.abs(full[:, j:].cpu().numpy() - ref).max() <= CORR_TOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# a8: LDOS
+# ---------------------------------------------------------------------------------------------------------------------
+def test_ldos_parity_and_closed_form(dev, oracle_mod):
+    w = W.make_workload(5, device=dev, L=14)
+    sites = W.ldos_sites(w.n_orb, 11)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    corr, norm2, _ = tbpm.tbpm_ldos(H, sites, 10, w.dt, w.rescale)
+    hi, hj, hv, on = to_np(w)
+    ref, _ = oracle_mod.ldos(w.n_orb, on, hi, hj, hv, sites.numpy(), 10, w.dt, w.rescale)
+    assert np.abs(corr.cpu().numpy() - ref).max() <= CORR_TOL
+    assert np.abs(norm2.cpu().numpy() - 1).max() <= NORM_TOL
+    with pytest.raises(tbpm.TbpmError):
+        tbpm.tbpm_ldos(H, [w.n_orb], 3, w.dt, w.rescale)
+    # clean cubic lattice, any L: corr_n = g_n^3 (reading #25) -- needs no oracle
+    L, s, nst = 48, 15.0, 40
+    n, hi, hj, hv = W.cubic_hops(L, -1.0, dev)
+    H = tbpm.tbpm_build(n, None, hi, hj, hv)
+    corr, _, _ = tbpm.tbpm_ldos(H, [0, 12345, n - 1], nst, math.pi / s, s)
+    q = np.arange(L)
+    g = np.exp(-1j * np.outer(np.arange(1, nst + 1), 2 * -1.0 * np.cos(2 * math.pi * q / L)) * math.pi / s).mean(axis=1)
+    assert np.abs(corr.cpu().numpy() - g ** 3).max() <= 1e-12
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# end-to-end host entry
+# ---------------------------------------------------------------------------------------------------------------------
+def test_corr_host_matches_device_path(dev, oracle_mod):
+    w = W.make_workload(2, Na=64, Nb=40)                              # generated on the host
+    psi0 = w.psi0(n_state=4).pin_memory()
+    n_step = 8
+    arena = torch.empty(tbpm.tbpm_corr_host_bytes(w.n_orb, w.n_hop, True, 4, n_step), dtype=torch.uint8, device=dev)
+    corr = torch.zeros((4, n_step), dtype=torch.complex128).pin_memory()
+    norm2 = torch.zeros((4, n_step), dtype=torch.float64).pin_memory()
+    up, down = tbpm.tbpm_corr_host(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val, psi0, n_step, w.dt, w.rescale, arena, corr, norm2)
+    assert up == w.n_hop * 24 + w.n_orb * 8 + 4 * w.n_orb * 16 and down == 4 * n_step * 24
+    hi, hj, hv, on = to_np(w)
+    ref, _ = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0.numpy(), n_step, w.dt, w.rescale)
+    assert np.abs(corr.numpy() - ref).max() <= CORR_TOL
+    assert np.abs(norm2.numpy() - 1).max() <= NORM_TOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# full-size configs, in the launch configuration bench.py times
+# ---------------------------------------------------------------------------------------------------------------------
+FULL = os.environ.get("TBPM_TEST_FULL", "1") != "0"
+
+
+def eigen_check(dev, w, psi, E, n_step):
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    corr, norm2, _ = tbpm.tbpm_propagate(H, psi[None, :].contiguous(), n_step, w.dt, w.rescale)
+    n = np.arange(1, n_step + 1)
+    assert np.abs(corr.cpu().numpy()[0] - np.exp(-1j * n * math.pi * E / w.rescale)).max() <= CORR_TOL
+    assert np.abs(norm2.cpu().numpy() - 1).max() <= NORM_TOL
+
+
+@pytest.mark.skipif(not FULL, reason="TBPM_TEST_FULL=0")
+def test_full_size_closed_form_eigenstates(dev):
+    """Reading #10: uniform / staggered states are exact eigenstates of the clean periodic lattices, so
+    corr_n = exp(-i n tau E/s) and norm2 = 1 at 16-33 M orbitals with no oracle at all."""
+    w = W.make_workload(3, device=dev, vac=0.0)                       # clean honeycomb 4096x4096, 33.5 M orbitals
+    N = w.n_orb
+    eigen_check(dev, w, torch.full((N,), 1 / math.sqrt(N), dtype=torch.complex128, device=dev), 3 * -2.7, 24)
+    stag = torch.where(torch.arange(N, device=dev) % 2 == 0, 1.0, -1.0).to(torch.complex128) / math.sqrt(N)
+    eigen_check(dev, w, stag, -3 * -2.7, 24)
+    del w, stag
+    n, hi, hj, hv = W.cubic_hops(256, -1.0, dev)                      # clean cubic 256^3
+    w = W.Workload("cubic-clean", n, hi, hj, hv, None, 1, 1, 15.0)
+    eigen_check(dev, w, torch.full((n,), 1 / math.sqrt(n), dtype=torch.complex128, device=dev), -6.0, 24)
+
+
+@pytest.mark.skipif(not FULL, reason="TBPM_TEST_FULL=0")
+@pytest.mark.parametrize("cfg,m,sample", [(2, 3, [0, 3]), (3, 2, [0]), (4, 2, [5]), (5, 2, [17])])
+def test_full_size_prefix_parity(dev, oracle_mod, cfg, m, sample):
+    """Configs 2-5 at BASELINE.json's full size with all their states batched as bench.py runs them; the first m steps
+    of a sample of states are compared with the oracle (OpenMP row form), the norm is checked for every state."""
+    w = W.make_workload(cfg, device=dev)
+    psi0 = w.psi0(device=dev)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    assert H.nnz == w.nnz
+    corr, norm2, _ = tbpm.tbpm_propagate(H, psi0, m, w.dt, w.rescale)
+    torch.cuda.synchronize()
+    assert np.abs(norm2.cpu().numpy() - 1).max() <= NORM_TOL
+    hi, hj, hv, on = to_np(w)
+    ref, _ = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0[sample].cpu().numpy(), m, w.dt, w.rescale, form="csr")
+    assert np.abs(corr[sample].cpu().numpy() - ref).max() <= CORR_TOL
+    if cfg == 3:
+        assert abs(w.n_orb - 30198989) < 20000 and H.max_row_nnz == 3
+    if cfg == 5:                                                      # LDOS leg of config 5 on the same H
+        sites = w.sites()
+        lc, ln, _ = tbpm.tbpm_ldos(H, sites, m, w.dt, w.rescale)
+        lref, _ = oracle_mod.ldos(w.n_orb, on, hi, hj, hv, sites[:2].numpy(), m, w.dt, w.rescale, form="csr")
+        assert np.abs(lc[:2].cpu().numpy() - lref).max() <= CORR_TOL
+        assert np.abs(ln.cpu().numpy() - 1).max() <= NORM_TOL
