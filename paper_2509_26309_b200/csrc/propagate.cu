@@ -23,48 +23,17 @@
 #include <cstdlib>
 #include <vector>
 
-#include "tbpm_internal.h"
+#include "term.h"
 
 using namespace tbpm_detail;
 
 namespace {
 
 constexpr int kThreads = 256;
-constexpr int kMaxBT = 32;
-constexpr int kMaxGrid = 4096;                       // upper bound on the persistent grid (partials are sized for it)
 constexpr size_t kHeaderBytes = 256;
 constexpr size_t kPartialBytes = sizeof(double) * 3 * kMaxBT * kMaxGrid;
 
 thread_local int64_t g_launches = 0;
-
-enum TermFlags { F_SUB_Y = 1, F_WRITE_Y = 2, F_SKIP_H = 4, F_ACC_INIT = 8, F_REDUCE = 16 };
-
-struct TermParams {
-    // matrix (kernel layout or canonical CSR)
-    const uint32_t *orp;
-    const int32_t *ocol;
-    const uint16_t *oidx;
-    const double2 *vtab;
-    const double *diag;
-    const int64_t *rowptr;
-    const int32_t *col;
-    const double2 *val;
-    int64_t n_orb;
-    // vectors of this tile, [row][BT]
-    const double2 *x;      // T_{k-1}
-    double2 *y;            // T_{k-2} in, T_k out (in place)
-    double2 *acc;          // psi'
-    const double2 *psi0;   // bra of the correlation
-    double *partial;       // [grid][BT][3]
-    double a;              // 1/s (k = 1) or 2/s
-    double2 ca, cb, cc;    // coefficients of T_k, T_{k-1}, T_{k-2} in this flush
-    int n_acc;             // 0: psi' untouched; 1..3 terms added
-    int flags;
-    int n_table;           // entries of vtab (kernel layout)
-    int max_row_off;       // longest off-diagonal row (sizes the staged index slices)
-    // staged kernel: shared-memory stage geometry (bytes), filled by launch_staged
-    int n_stage, stage_bytes, cap_entries, off_col, off_idx, off_diag, off_vec;
-};
 
 struct WsHeader {          // first bytes of the workspace; read by tbpm_get_state's kernel
     int64_t n_orb;
@@ -77,14 +46,6 @@ struct WsHeader {          // first bytes of the workspace; read by tbpm_get_sta
 
 __device__ __forceinline__ double2 ld_stream(const double2 *p) { return __ldcs(p); }     // read once: evict first
 __device__ __forceinline__ void st_stream(double2 *p, double2 v) { __stcs(p, v); }
-__device__ __forceinline__ void cfma(double2 &h, double2 v, double2 x)
-{
-    h.x = fma(v.x, x.x, h.x);
-    h.x = fma(-v.y, x.y, h.x);
-    h.y = fma(v.x, x.y, h.y);
-    h.y = fma(v.y, x.x, h.y);
-}
-
 // ---------------------------------------------------------------------------------------------------------------------
 // The fused Chebyshev term.  Thread -> (row, state b): BT consecutive threads share a row.
 // Latency structure: the streaming operands of a row (y, psi', psi0, diagonal, x[row]) do not depend on the row
@@ -212,319 +173,6 @@ __global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p
     }
 }
 
-// ---------------------------------------------------------------------------------------------------------------------
-// Staged, warp-specialised variant of the fused term (kernel layout only) -- the default hot kernel.
-//
-//   producer warp (1 elected lane)  : for every tile of R rows, kStages ahead of the compute, bulk-copies (cp.async.bulk
-//                                     + mbarrier complete_tx, the TMA 1-D bulk path; SASS UBLKCP) the row offsets, column
-//                                     indices, value indices, diagonal slice and the y / psi' / psi0 slices of the tile
-//                                     into a shared-memory stage;
-//   8 consumer warps                : wait on the stage's "full" barrier, then have a ONE-deep dependent chain per
-//                                     non-zero: index from shared memory -> gather x[col] (128/256-bit LDG through
-//                                     L1/L2), complex FMA; results go straight to global memory; each warp then arrives
-//                                     on the stage's "empty" barrier.  No block-wide barrier in the main loop.
-//
-// Thread -> (row, SPT consecutive states); SPT = 2 (one 256-bit load per gather) whenever the tile has >= 2 states.
-// Nothing the copy engine moves occupies registers while in flight, and the lanes of a row do not repeat index loads
-// from global memory.
-// ---------------------------------------------------------------------------------------------------------------------
-constexpr int kTabSmem = 256;            // hopping-value tables up to this size are copied into shared memory
-constexpr int kConsumers = 256;          // 8 consumer warps
-constexpr int kWsThreads = kConsumers + 32;
-constexpr int kMaxStages = 8;
-
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
-                 "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-
-// SPT consecutive complex128 values
-template <int SPT> struct CVec;
-template <> struct CVec<1> {
-    double2 v[1];
-    __device__ __forceinline__ void ldg(const double2 *p) { v[0] = __ldg(p); }
-    __device__ __forceinline__ void lds(const double2 *p) { v[0] = *p; }
-    __device__ __forceinline__ void st(double2 *p) const { *p = v[0]; }
-    __device__ __forceinline__ void st_cs(double2 *p) const { __stcs(p, v[0]); }
-};
-template <> struct CVec<2> {
-    double2 v[2];
-    __device__ __forceinline__ void ldg(const double2 *p)     // one 256-bit load (LDG.E.256)
-    {
-        asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v[0].x), "=d"(v[0].y), "=d"(v[1].x), "=d"(v[1].y) : "l"(p));
-    }
-    __device__ __forceinline__ void lds(const double2 *p) { v[0] = p[0]; v[1] = p[1]; }
-    __device__ __forceinline__ void st(double2 *p) const
-    {
-        asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v[0].x), "d"(v[0].y), "d"(v[1].x), "d"(v[1].y) : "memory");
-    }
-    __device__ __forceinline__ void st_cs(double2 *p) const
-    {
-        asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v[0].x), "d"(v[0].y), "d"(v[1].x), "d"(v[1].y) : "memory");
-    }
-};
-
-template <int BT, int SPT>
-__global__ void __launch_bounds__(kWsThreads, 2) k_cheb_term_ws(const TermParams p)
-{
-    constexpr int LPR = BT / SPT;                           // lanes per row
-    constexpr int R = kConsumers / LPR;                     // rows per tile
-    constexpr uint32_t kVecBytes = R * BT * sizeof(double2);
-    extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ uint64_t full_bar[kMaxStages], empty_bar[kMaxStages];
-    __shared__ uint32_t lo_s[kMaxStages][2];                // first column / value-index element held by each stage
-    __shared__ double2 tab_s[kTabSmem];
-    __shared__ double red_s[kConsumers / 32][kMaxBT][3];
-
-    const int tid = threadIdx.x;
-    const int flags = p.flags, n_acc = p.n_acc;
-    const bool skip_h = flags & F_SKIP_H;
-    const bool need_y = (flags & F_SUB_Y) || n_acc == 3;
-    const bool need_xrow = skip_h || n_acc >= 2 || p.diag != nullptr;
-    const bool need_acc = n_acc > 0 && !(flags & F_ACC_INIT);
-    const bool reduce = flags & F_REDUCE;
-    const bool tab_in_smem = p.n_table <= kTabSmem;
-    const int S = p.n_stage;
-    const int64_t n_tiles = (p.n_orb + R - 1) / R;
-    const int slot_acc = need_y ? 1 : 0, slot_z = slot_acc + (need_acc ? 1 : 0);   // y is slot 0
-
-    if (tid == 0) {
-        for (int s = 0; s < S; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], kConsumers / 32); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    if (tab_in_smem)
-        for (int i = tid; i < p.n_table; i += kWsThreads) tab_s[i] = __ldg(p.vtab + i);
-    __syncthreads();
-
-    if (tid >= kConsumers) {
-        // ------------------------------------------------ producer warp ------------------------------------------------
-        if (tid == kConsumers) {
-            uint32_t q_lo = 0, q_hi = 0;                    // offsets bounding the next tile to issue (prefetched)
-            int64_t tile = blockIdx.x;
-            if (tile < n_tiles && !skip_h) {
-                const int64_t r0 = tile * R;
-                q_lo = __ldg(p.orp + r0);
-                q_hi = __ldg(p.orp + min(r0 + R, p.n_orb));
-            }
-            for (int it = 0; tile < n_tiles; tile += gridDim.x, ++it) {
-                const int s = it % S;
-                const uint32_t c_lo = q_lo, c_hi = q_hi;
-                const int64_t nt = tile + gridDim.x;
-                if (nt < n_tiles && !skip_h) {              // bounds of the following tile: latency hidden behind this issue
-                    const int64_t nr0 = nt * R;
-                    q_lo = __ldg(p.orp + nr0);
-                    q_hi = __ldg(p.orp + min(nr0 + R, p.n_orb));
-                }
-                if (it >= S) mbar_wait(&empty_bar[s], (uint32_t)(it / S - 1) & 1u);
-                unsigned char *st = smem + (size_t)s * p.stage_bytes;
-                const int64_t r0 = tile * R;
-                const int rows = (int)min((int64_t)R, p.n_orb - r0);
-                uint32_t tx = 0;
-                if (!skip_h) {
-                    const uint32_t col_lo = c_lo & ~3u, idx_lo = c_lo & ~7u;
-                    const uint32_t nc = ((c_hi - col_lo) + 3u) & ~3u, ni = ((c_hi - idx_lo) + 7u) & ~7u;
-                    lo_s[s][0] = col_lo;
-                    lo_s[s][1] = idx_lo;
-                    const uint32_t orp_bytes = (uint32_t)(((rows + 1) * 4 + 15) & ~15);
-                    bulk_g2s(st, p.orp + r0, orp_bytes, &full_bar[s]);
-                    tx += orp_bytes;
-                    if (nc > 0) {
-                        bulk_g2s(st + p.off_col, p.ocol + col_lo, nc * 4, &full_bar[s]);
-                        bulk_g2s(st + p.off_idx, p.oidx + idx_lo, ni * 2, &full_bar[s]);
-                        tx += nc * 4 + ni * 2;
-                    }
-                    if (p.diag != nullptr) {
-                        const uint32_t db = (uint32_t)((rows * 8 + 15) & ~15);
-                        bulk_g2s(st + p.off_diag, p.diag + r0, db, &full_bar[s]);
-                        tx += db;
-                    }
-                }
-                const uint32_t vb = (uint32_t)rows * BT * sizeof(double2);
-                unsigned char *vec = st + p.off_vec;
-                const int64_t e0 = r0 * BT;
-                if (need_y) { bulk_g2s(vec, p.y + e0, vb, &full_bar[s]); tx += vb; }
-                if (need_acc) { bulk_g2s(vec + slot_acc * kVecBytes, p.acc + e0, vb, &full_bar[s]); tx += vb; }
-                if (reduce) { bulk_g2s(vec + slot_z * kVecBytes, p.psi0 + e0, vb, &full_bar[s]); tx += vb; }
-                mbar_expect_tx(&full_bar[s], tx);           // release: also publishes lo_s[s]
-            }
-        }
-        return;
-    }
-
-    // ---------------------------------------------------- consumer warps ----------------------------------------------------
-    const int rl = tid / LPR;                               // row within the tile
-    const int b0 = (tid % LPR) * SPT;                       // first state of this thread
-    const double2 *xb = p.x + b0;
-    double s_re[SPT], s_im[SPT], s_nn[SPT];
-#pragma unroll
-    for (int k = 0; k < SPT; ++k) s_re[k] = s_im[k] = s_nn[k] = 0.0;
-
-    int it = 0;
-    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-        const int s = it % S;
-        mbar_wait(&full_bar[s], (uint32_t)(it / S) & 1u);
-        const unsigned char *st = smem + (size_t)s * p.stage_bytes;
-        const int64_t row = tile * R + rl;
-        if (row < p.n_orb) {
-            const int64_t e = row * BT + b0;
-            const double2 *vec = reinterpret_cast<const double2 *>(st + p.off_vec);
-            const int le = rl * BT + b0;
-            CVec<SPT> xrow, h;
-#pragma unroll
-            for (int k = 0; k < SPT; ++k) h.v[k] = xrow.v[k] = make_double2(0.0, 0.0);
-            if (need_xrow) xrow.ldg(p.x + e);               // the tile's own x rows are gathered by its neighbours: L1 hit
-            if (!skip_h) {
-                const uint32_t *orp_s = reinterpret_cast<const uint32_t *>(st);
-                const uint32_t q0 = orp_s[rl], n = orp_s[rl + 1] - q0;
-                const int32_t *cs = reinterpret_cast<const int32_t *>(st + p.off_col) + (q0 - lo_s[s][0]);
-                const uint16_t *is = reinterpret_cast<const uint16_t *>(st + p.off_idx) + (q0 - lo_s[s][1]);
-                auto value = [&](uint32_t i) { return tab_in_smem ? tab_s[i] : __ldg(p.vtab + i); };
-                uint32_t j = 0;
-                for (; j + 4 <= n; j += 4) {                // 4 independent gathers in flight
-                    CVec<SPT> x0, x1, x2, x3;
-                    x0.ldg(xb + (int64_t)cs[j] * BT);
-                    x1.ldg(xb + (int64_t)cs[j + 1] * BT);
-                    x2.ldg(xb + (int64_t)cs[j + 2] * BT);
-                    x3.ldg(xb + (int64_t)cs[j + 3] * BT);
-                    const double2 v0 = value(is[j]), v1 = value(is[j + 1]), v2 = value(is[j + 2]), v3 = value(is[j + 3]);
-#pragma unroll
-                    for (int k = 0; k < SPT; ++k) { cfma(h.v[k], v0, x0.v[k]); cfma(h.v[k], v1, x1.v[k]); cfma(h.v[k], v2, x2.v[k]); cfma(h.v[k], v3, x3.v[k]); }
-                }
-                const uint32_t rem = n - j;
-                if (rem == 3) {
-                    CVec<SPT> x0, x1, x2;
-                    x0.ldg(xb + (int64_t)cs[j] * BT);
-                    x1.ldg(xb + (int64_t)cs[j + 1] * BT);
-                    x2.ldg(xb + (int64_t)cs[j + 2] * BT);
-                    const double2 v0 = value(is[j]), v1 = value(is[j + 1]), v2 = value(is[j + 2]);
-#pragma unroll
-                    for (int k = 0; k < SPT; ++k) { cfma(h.v[k], v0, x0.v[k]); cfma(h.v[k], v1, x1.v[k]); cfma(h.v[k], v2, x2.v[k]); }
-                } else if (rem == 2) {
-                    CVec<SPT> x0, x1;
-                    x0.ldg(xb + (int64_t)cs[j] * BT);
-                    x1.ldg(xb + (int64_t)cs[j + 1] * BT);
-                    const double2 v0 = value(is[j]), v1 = value(is[j + 1]);
-#pragma unroll
-                    for (int k = 0; k < SPT; ++k) { cfma(h.v[k], v0, x0.v[k]); cfma(h.v[k], v1, x1.v[k]); }
-                } else if (rem == 1) {
-                    CVec<SPT> x0;
-                    x0.ldg(xb + (int64_t)cs[j] * BT);
-                    const double2 v0 = value(is[j]);
-#pragma unroll
-                    for (int k = 0; k < SPT; ++k) cfma(h.v[k], v0, x0.v[k]);
-                }
-                if (p.diag != nullptr) {
-                    const double d = reinterpret_cast<const double *>(st + p.off_diag)[rl];
-#pragma unroll
-                    for (int k = 0; k < SPT; ++k) { h.v[k].x = fma(d, xrow.v[k].x, h.v[k].x); h.v[k].y = fma(d, xrow.v[k].y, h.v[k].y); }
-                }
-#pragma unroll
-                for (int k = 0; k < SPT; ++k) { h.v[k].x *= p.a; h.v[k].y *= p.a; }
-            } else {
-                h = xrow;
-            }
-            CVec<SPT> yold;
-#pragma unroll
-            for (int k = 0; k < SPT; ++k) yold.v[k] = make_double2(0.0, 0.0);
-            if (need_y) yold.lds(vec + le);
-            if (flags & F_SUB_Y) {
-#pragma unroll
-                for (int k = 0; k < SPT; ++k) { h.v[k].x -= yold.v[k].x; h.v[k].y -= yold.v[k].y; }
-            }
-            if (flags & F_WRITE_Y) h.st(p.y + e);           // T_k: gathered by the next term, keep it cacheable
-            if (n_acc > 0) {
-                CVec<SPT> sacc;
-#pragma unroll
-                for (int k = 0; k < SPT; ++k) sacc.v[k] = make_double2(0.0, 0.0);
-                if (need_acc) sacc.lds(vec + slot_acc * (R * BT) + le);
-#pragma unroll
-                for (int k = 0; k < SPT; ++k) {
-                    cfma(sacc.v[k], p.ca, h.v[k]);
-                    if (n_acc >= 2) cfma(sacc.v[k], p.cb, xrow.v[k]);
-                    if (n_acc == 3) cfma(sacc.v[k], p.cc, yold.v[k]);
-                }
-                if (reduce) {
-                    CVec<SPT> z;
-                    z.lds(vec + slot_z * (R * BT) + le);
-#pragma unroll
-                    for (int k = 0; k < SPT; ++k) {
-                        s_re[k] = fma(z.v[k].x, sacc.v[k].x, s_re[k]);      // conj(z) * psi'
-                        s_re[k] = fma(z.v[k].y, sacc.v[k].y, s_re[k]);
-                        s_im[k] = fma(z.v[k].x, sacc.v[k].y, s_im[k]);
-                        s_im[k] = fma(-z.v[k].y, sacc.v[k].x, s_im[k]);
-                        s_nn[k] = fma(sacc.v[k].x, sacc.v[k].x, s_nn[k]);
-                        s_nn[k] = fma(sacc.v[k].y, sacc.v[k].y, s_nn[k]);
-                    }
-                    sacc.st(p.acc + e);                     // psi': T_0 of the next step, gathered right away
-                } else {
-                    sacc.st_cs(p.acc + e);
-                }
-            }
-        }
-        __syncwarp();
-        if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);    // this warp is done with stage s
-    }
-
-    if (reduce) {
-        // lanes with equal (lane % LPR) hold the same states
-#pragma unroll
-        for (int k = 0; k < SPT; ++k) {
-#pragma unroll
-            for (int o = 16; o >= LPR; o >>= 1) {
-                s_re[k] += __shfl_xor_sync(0xffffffffu, s_re[k], o);
-                s_im[k] += __shfl_xor_sync(0xffffffffu, s_im[k], o);
-                s_nn[k] += __shfl_xor_sync(0xffffffffu, s_nn[k], o);
-            }
-        }
-        const int lane = tid & 31, warp = tid >> 5;
-        if (lane < LPR) {
-#pragma unroll
-            for (int k = 0; k < SPT; ++k) {
-                red_s[warp][lane * SPT + k][0] = s_re[k];
-                red_s[warp][lane * SPT + k][1] = s_im[k];
-                red_s[warp][lane * SPT + k][2] = s_nn[k];
-            }
-        }
-        asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");   // consumers only (the producer warp has left)
-        if (tid < BT * 3) {
-            const int bb = tid / 3, c = tid % 3;
-            double t = 0.0;
-#pragma unroll
-            for (int w = 0; w < kConsumers / 32; ++w) t += red_s[w][bb][c];
-            p.partial[((int64_t)blockIdx.x * BT + bb) * 3 + c] = t;
-        }
-    }
-}
-
 // Sum the block partials in a fixed order: block = state, warp = component, lanes stride over the partials.
 __global__ void k_reduce_final(const double *__restrict__ partial, int n_blocks, int bt, int n_valid, int state0, int n_step, int step,
                                double *corr, double *norm2)
@@ -629,12 +277,6 @@ Plan make_plan(int64_t n_orb, int n_state)
     return P;
 }
 
-int env_int(const char *name, int dflt)
-{
-    const char *e = std::getenv(name);
-    return e ? std::atoi(e) : dflt;
-}
-
 int min_blocks()
 {
     int m = 4;
@@ -675,56 +317,12 @@ int launch_term_m(const TermParams &p, int num_sms, cudaStream_t st, int *grid_o
 }
 
 
-template <int BT>
-int launch_ws_t(TermParams p, int num_sms, cudaStream_t st, int *grid_out)
-{
-    constexpr int SPT = BT >= 2 ? 2 : 1;
-    constexpr int R = kConsumers / (BT / SPT);
-    const int flags = p.flags, n_acc = p.n_acc;
-    const int nvec = (((flags & F_SUB_Y) || n_acc == 3) ? 1 : 0) + ((n_acc > 0 && !(flags & F_ACC_INIT)) ? 1 : 0) + ((flags & F_REDUCE) ? 1 : 0);
-    p.n_stage = std::min(kMaxStages, std::max(2, env_int("TBPM_STAGES", 4)));
-    p.cap_entries = ((R * std::max(p.max_row_off, 1) + 8 + 7) / 8) * 8;          // + alignment slack of the slice start
-    size_t o = (size_t)(((R + 1) * 4 + 15) & ~15);
-    p.off_col = (int)o;  o += (size_t)p.cap_entries * 4;
-    p.off_idx = (int)o;  o += (size_t)p.cap_entries * 2;
-    o = (o + 15) & ~size_t(15);
-    p.off_diag = (int)o; o += (size_t)((R * 8 + 15) & ~15);
-    o = (o + 127) & ~size_t(127);
-    p.off_vec = (int)o;  o += (size_t)nvec * R * BT * sizeof(double2);
-    p.stage_bytes = (int)((o + 127) & ~size_t(127));
-    const size_t dyn = (size_t)p.stage_bytes * p.n_stage;
-    static size_t configured = 0;
-    if (dyn > configured) {
-        const size_t want = std::max(dyn, (size_t)64 * 1024);
-        TBPM_CUDA_TRY(cudaFuncSetAttribute(k_cheb_term_ws<BT, SPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)want));
-        configured = want;
-    }
-    int nb = 0;
-    TBPM_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_cheb_term_ws<BT, SPT>, kWsThreads, dyn));
-    if (nb < 1) return TBPM_ENOMEM;
-    nb = std::min(nb, std::max(1, env_int("TBPM_MAXB", 8)));
-    const int64_t need = (p.n_orb + R - 1) / R;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>({need, (int64_t)num_sms * nb, (int64_t)kMaxGrid}));
-    k_cheb_term_ws<BT, SPT><<<grid, kWsThreads, dyn, st>>>(p);
-    ++g_launches; count_launches(1);
-    *grid_out = grid;
-    return TBPM_OK;
-}
-
 int launch_term(int bt, bool table, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
-    // staged (bulk-copy pipelined) kernel whenever the kernel layout is in use and a tile's index slice fits a stage
-    const bool staged = table && env_int("TBPM_DIRECT", 0) == 0 && (int64_t)p.max_row_off * kConsumers <= 12288;
-    if (staged) {
-        switch (bt) {
-        case 1: return launch_ws_t<1>(p, num_sms, st, grid_out);
-        case 2: return launch_ws_t<2>(p, num_sms, st, grid_out);
-        case 4: return launch_ws_t<4>(p, num_sms, st, grid_out);
-        case 8: return launch_ws_t<8>(p, num_sms, st, grid_out);
-        case 16: return launch_ws_t<16>(p, num_sms, st, grid_out);
-        case 32: return launch_ws_t<32>(p, num_sms, st, grid_out);
-        }
-        return TBPM_EINVAL;
+    // warp-specialised bulk-copy kernel (term_ws.cu) whenever it has an instantiation for this term; else the direct kernel
+    if (table && term_ws_supported(bt, p)) {
+        ++g_launches;
+        return launch_term_ws(bt, p, num_sms, st, grid_out);
     }
 #define TBPM_CASE(B)                                                                     \
     case B:                                                                              \

@@ -1,0 +1,64 @@
+// term.h -- private: parameters shared by the fused Chebyshev-term kernels (term_ws.cu, propagate.cu).
+#pragma once
+
+#include <cstdlib>
+
+#include "tbpm_internal.h"
+
+namespace tbpm_detail {
+
+constexpr int kMaxBT = 32;       // widest state tile
+constexpr int kMaxGrid = 4096;   // upper bound on the persistent grid (block partials are sized for it)
+
+enum TermFlags { F_SUB_Y = 1, F_WRITE_Y = 2, F_SKIP_H = 4, F_ACC_INIT = 8, F_REDUCE = 16 };
+
+// One launch = one Chebyshev term  T_k = a*H*T_{k-1} - T_{k-2}  on one tile of BT interleaved states
+// (amxsy of PAPER.md:434/439), plus the deferred accumulation psi' += ca*T_k + cb*T_{k-1} + cc*T_{k-2}
+// (the axpy of PAPER.md:440 for up to three terms at once) and, on the last term, <psi0|psi'> and <psi'|psi'>.
+struct TermParams {
+    // matrix: kernel layout (orp/ocol/oidx/vtab/diag) or canonical CSR (rowptr/col/val)
+    const uint32_t *orp;
+    const int32_t *ocol;
+    const uint16_t *oidx;
+    const double2 *vtab;
+    const double *diag;
+    const int64_t *rowptr;
+    const int32_t *col;
+    const double2 *val;
+    int64_t n_orb;
+    // vectors of this tile, [row][BT]
+    const double2 *x;      // T_{k-1}
+    double2 *y;            // T_{k-2} in, T_k out (in place)
+    double2 *acc;          // psi'
+    const double2 *psi0;   // bra of the correlation
+    double *partial;       // [grid][BT][3]
+    double a;              // 1/s (k = 1) or 2/s
+    double2 ca, cb, cc;    // coefficients of T_k, T_{k-1}, T_{k-2} in this flush
+    int n_acc;             // 0: psi' untouched; 1..3 terms added
+    int flags;
+    int n_table;           // entries of vtab (kernel layout)
+    int max_row_off;       // longest off-diagonal row (sizes the staged index slices)
+    // warp-specialised kernel: shared-memory stage geometry (bytes), filled by its launcher
+    int n_stage, stage_bytes, cap_entries, off_col, off_idx, off_diag, off_vec;
+};
+
+__device__ __forceinline__ void cfma(double2 &h, double2 v, double2 x)   // h += v * x (complex)
+{
+    h.x = fma(v.x, x.x, h.x);
+    h.x = fma(-v.y, x.y, h.x);
+    h.y = fma(v.x, x.y, h.y);
+    h.y = fma(v.y, x.x, h.y);
+}
+
+inline int env_int(const char *name, int dflt)
+{
+    const char *e = std::getenv(name);
+    return e ? std::atoi(e) : dflt;
+}
+
+// Warp-specialised bulk-copy (TMA) kernel, term_ws.cu.  Returns TBPM_EINVAL if (bt, flags) has no instantiation
+// (the caller then uses the direct kernel).  *grid_out = blocks launched (sizes the final reduction).
+bool term_ws_supported(int bt, const TermParams &p);
+int launch_term_ws(int bt, TermParams p, int num_sms, cudaStream_t st, int *grid_out);
+
+}  // namespace tbpm_detail
