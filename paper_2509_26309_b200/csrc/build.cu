@@ -14,8 +14,10 @@
 //   3. scatter entries into their row segment (order within the row is arbitrary at this point)   k_fill
 //   4. one thread per row: insertion sort by column, duplicate check, Gershgorin row sum, max row length   k_sort_rows
 //   5. kernel layout: off-diagonal CSR with 32-bit row offsets + real diagonal                     k_strip
-//   6. table of distinct off-diagonal values (open-addressing hash on the 128-bit pattern), 16-bit index per entry
-//      k_tab_insert / scan / k_tab_number / k_tab_lookup   ("hopping-table index for uniform lattices", north_star)
+//   6. table of distinct off-diagonal values (open-addressing hash on the 128-bit pattern), numbered by first use in
+//      (entry-within-row, row) order; 16-bit index per entry, or -- tables of <= 2 values -- bit 31 of the column word
+//      k_tab_insert / scan / k_tab_key / k_tab_compact / k_tab_rank / k_tab_number / k_tab_lookup
+//      ("hopping-table index for uniform lattices", north_star)
 #include <algorithm>
 #include <cstring>
 #include <new>
@@ -237,21 +239,21 @@ __global__ void k_sort_rows(int64_t n_orb, const int64_t *__restrict__ rowptr, i
     }
 }
 
-// 5. kernel layout.  has_onsite: every row holds exactly one diagonal entry -> off-diagonal offset = rowptr[r] - r.
+// 5. kernel layout: off-diagonal columns in a separate array (they are packed with the value index later, so they never
+//    alias the canonical CSR).  has_onsite: every row holds exactly one diagonal entry -> off-diagonal offset = rowptr[r] - r.
 __global__ void k_strip(int64_t n_orb, int has_onsite, const int64_t *__restrict__ rowptr, const int32_t *__restrict__ col,
                         const double2 *__restrict__ val, uint32_t *orp, int32_t *ocol, double *diag)
 {
     int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r > n_orb) return;
     int64_t b = rowptr[r];
-    if (!has_onsite) { orp[r] = (uint32_t)b; return; }
-    int64_t ob = b - r;
+    int64_t ob = has_onsite ? b - r : b;
     orp[r] = (uint32_t)ob;
     if (r == n_orb) return;
     int64_t e = rowptr[r + 1];
     for (int64_t p = b; p < e; ++p) {
         int32_t c = col[p];
-        if (c == (int32_t)r) diag[r] = val[p].x;
+        if (has_onsite && c == (int32_t)r) diag[r] = val[p].x;
         else ocol[ob++] = c;
     }
 }
@@ -308,18 +310,56 @@ __global__ void k_tab_flags(const uint32_t *__restrict__ slots, int32_t *flag)
     else if (i == kHashSlots) flag[i] = 0;
 }
 
-__global__ void k_tab_number(const uint32_t *__restrict__ slots, const int64_t *__restrict__ slot_id, const double2 *__restrict__ val,
-                             double2 *vtab)
+// Table order.  The index of a value is its rank by the key (j, r) of its first use, j = position among the off-diagonal
+// entries of row r, r = row: on a lattice the j-th hops of consecutive rows then sit in consecutive table entries, so the
+// eight rows a warp works on fetch their j-th values from one or two 128-byte lines instead of eight.
+__global__ void k_tab_key(int64_t n_orb, int has_onsite, const int64_t *__restrict__ rowptr, const int32_t *__restrict__ col,
+                          const double2 *__restrict__ val, const uint32_t *__restrict__ slots, unsigned long long *keys)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_orb) return;
+    unsigned long long j = 0;
+    for (int64_t p = rowptr[r]; p < rowptr[r + 1]; ++p) {
+        if (has_onsite && col[p] == (int32_t)r) continue;
+        double2 v = val[p];
+        uint32_t h = slot_of(v);
+        while (!same_bits(val[slots[h]], v)) h = (h + 1) & (kHashSlots - 1);
+        const unsigned long long key = (j << 32) | (unsigned long long)r;
+        if (*(volatile unsigned long long *)&keys[h] > key) atomicMin(&keys[h], key);   // read first: few values, many entries
+        ++j;
+    }
+}
+
+__global__ void k_tab_compact(const uint32_t *__restrict__ slots, const int64_t *__restrict__ slot_id,
+                              const unsigned long long *__restrict__ keys, unsigned long long *ckeys)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < kHashSlots && slots[i] != kEmpty && slot_id[i] < kTableMax) ckeys[slot_id[i]] = keys[i];
+}
+
+__global__ void k_tab_rank(int n_table, const unsigned long long *__restrict__ ckeys, int32_t *rank)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_table) return;
+    const unsigned long long k = ckeys[i];
+    int32_t c = 0;
+    for (int t = 0; t < n_table; ++t) c += ckeys[t] < k;
+    rank[i] = c;
+}
+
+__global__ void k_tab_number(const uint32_t *__restrict__ slots, const int64_t *__restrict__ slot_id, const int32_t *__restrict__ rank,
+                             const double2 *__restrict__ val, double2 *vtab)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= kHashSlots) return;
     uint32_t s = slots[i];
-    if (s != kEmpty && slot_id[i] < kTableMax) vtab[slot_id[i]] = val[s];
+    if (s != kEmpty && slot_id[i] < kTableMax) vtab[rank[slot_id[i]]] = val[s];
 }
 
+// oidx[q] = table index of off-diagonal entry q; pack: additionally bit 31 of ocol[q] (tables of <= 2 values)
 __global__ void k_tab_lookup(int64_t n_orb, int has_onsite, const int64_t *__restrict__ rowptr, const int32_t *__restrict__ col,
                              const double2 *__restrict__ val, const uint32_t *__restrict__ slots, const int64_t *__restrict__ slot_id,
-                             uint16_t *oidx)
+                             const int32_t *__restrict__ rank, int pack, uint16_t *oidx, int32_t *ocol)
 {
     int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n_orb) return;
@@ -329,7 +369,10 @@ __global__ void k_tab_lookup(int64_t n_orb, int has_onsite, const int64_t *__res
         double2 v = val[p];
         uint32_t h = slot_of(v);
         while (!same_bits(val[slots[h]], v)) h = (h + 1) & (kHashSlots - 1);
-        oidx[q++] = (uint16_t)slot_id[h];
+        const int32_t id = rank[slot_id[h]];
+        oidx[q] = (uint16_t)id;
+        if (pack) ocol[q] = (int32_t)((uint32_t)ocol[q] | ((uint32_t)id << 31));
+        ++q;
     }
 }
 
@@ -349,7 +392,7 @@ PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint3
     L.col = take(sizeof(int32_t) * nnz);
     L.val = take(sizeof(double2) * nnz);
     L.orp = take(sizeof(uint32_t) * ((size_t)n_orb + 1));
-    L.ocol = has_onsite ? take(sizeof(int32_t) * nnz_off) : L.col;
+    L.ocol = take(sizeof(int32_t) * nnz_off);
     L.oidx = take(sizeof(uint16_t) * nnz_off);
     L.vtab = take(sizeof(double2) * kTableMax);
     L.diag = has_onsite ? take(sizeof(double) * (size_t)n_orb) : 0;
@@ -358,7 +401,7 @@ PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint3
 }
 
 struct ScratchLayout {
-    size_t cnt, cur, bsum, slots, flag, slot_id, total;
+    size_t cnt, cur, bsum, slots, flag, slot_id, keys, ckeys, rank, total;
 };
 
 ScratchLayout scratch_layout(int64_t n_orb)
@@ -373,6 +416,9 @@ ScratchLayout scratch_layout(int64_t n_orb)
     L.slots = take(sizeof(uint32_t) * kHashSlots);
     L.flag = take(sizeof(int32_t) * (kHashSlots + 1));
     L.slot_id = take(sizeof(int64_t) * (kHashSlots + 1));
+    L.keys = take(sizeof(unsigned long long) * kHashSlots);
+    L.ckeys = take(sizeof(unsigned long long) * kTableMax);
+    L.rank = take(sizeof(int32_t) * kTableMax);
     L.total = o;
     return L;
 }
@@ -440,6 +486,9 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
     uint32_t *slots = reinterpret_cast<uint32_t *>(S + SL.slots);
     int32_t *flag = reinterpret_cast<int32_t *>(S + SL.flag);
     int64_t *slot_id = reinterpret_cast<int64_t *>(S + SL.slot_id);
+    unsigned long long *keys = reinterpret_cast<unsigned long long *>(S + SL.keys);
+    unsigned long long *ckeys = reinterpret_cast<unsigned long long *>(S + SL.ckeys);
+    int32_t *rank = reinterpret_cast<int32_t *>(S + SL.rank);
 
     auto fail = [&](int code) { delete H; return code; };
 #define TRY_OR_FAIL(expr)                                                       \
@@ -481,11 +530,18 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
     if (want_table && !hst[ST_TAB_OVERFLOW] && hst[ST_NTAB] <= kTableMax) {
         k_tab_flags<<<blocks_for(kHashSlots + 1, kThreads), kThreads, 0, st>>>(slots, flag);
         if ((rc = scan_exclusive(flag, kHashSlots + 1, slot_id, bsum, st)) != TBPM_OK) return fail(rc);
-        k_tab_number<<<blocks_for(kHashSlots, kThreads), kThreads, 0, st>>>(slots, slot_id, H->val, H->vtab);
-        k_tab_lookup<<<gr, kThreads, 0, st>>>(n_orb, has_onsite, H->rowptr, H->col, H->val, slots, slot_id, H->oidx);
-        count_launches(3);
+        const int n_table = hst[ST_NTAB];
+        const int pack = n_table <= 2;
+        TRY_OR_FAIL(cudaMemsetAsync(keys, 0xFF, sizeof(unsigned long long) * kHashSlots, st));
+        k_tab_key<<<gr, kThreads, 0, st>>>(n_orb, has_onsite, H->rowptr, H->col, H->val, slots, keys);
+        k_tab_compact<<<blocks_for(kHashSlots, kThreads), kThreads, 0, st>>>(slots, slot_id, keys, ckeys);
+        k_tab_rank<<<blocks_for(n_table, kThreads), kThreads, 0, st>>>(n_table, ckeys, rank);
+        k_tab_number<<<blocks_for(kHashSlots, kThreads), kThreads, 0, st>>>(slots, slot_id, rank, H->val, H->vtab);
+        k_tab_lookup<<<gr, kThreads, 0, st>>>(n_orb, has_onsite, H->rowptr, H->col, H->val, slots, slot_id, rank, pack, H->oidx, H->ocol);
+        count_launches(6);
         TRY_OR_FAIL(cudaGetLastError());
         TRY_OR_FAIL(cudaStreamSynchronize(st));
+        H->packed = pack;
         H->n_table = hst[ST_NTAB];
     }
 #undef TRY_OR_FAIL
@@ -502,7 +558,7 @@ extern "C" int tbpm_ham_info(const tbpm_ham *H, int64_t *n_orb, int64_t *nnz, in
     if (max_row_nnz) *max_row_nnz = H->max_row_nnz;
     if (matrix_bytes_per_term) {
         if (H->n_table > 0)   // 32-bit row offsets + (int32 column + uint16 value index) per off-diagonal entry + real diagonal
-            *matrix_bytes_per_term = sizeof(uint32_t) * ((size_t)H->n_orb + 1) + (size_t)H->nnz_off * (sizeof(int32_t) + sizeof(uint16_t)) +
+            *matrix_bytes_per_term = sizeof(uint32_t) * ((size_t)H->n_orb + 1) + (size_t)H->nnz_off * (sizeof(int32_t) + (H->packed ? 0 : sizeof(uint16_t))) +
                                      (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0) + sizeof(double2) * (size_t)H->n_table;
         else                  // canonical CSR: int64 row pointers + (int32 column + complex128 value) per entry
             *matrix_bytes_per_term = sizeof(int64_t) * ((size_t)H->n_orb + 1) + (size_t)H->nnz * (sizeof(int32_t) + sizeof(double2));

@@ -98,10 +98,10 @@ __global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p
                 const bool p1 = q + 1 < q1, p2 = q + 2 < q1, p3 = q + 3 < q1;
                 if (TABLE) {
                     uint32_t i0 = 0, i1 = 0, i2 = 0, i3 = 0;
-                    c0 = __ldg(p.ocol + q); i0 = __ldg(p.oidx + q);
-                    if (p1) { c1 = __ldg(p.ocol + q + 1); i1 = __ldg(p.oidx + q + 1); }
-                    if (p2) { c2 = __ldg(p.ocol + q + 2); i2 = __ldg(p.oidx + q + 2); }
-                    if (p3) { c3 = __ldg(p.ocol + q + 3); i3 = __ldg(p.oidx + q + 3); }
+                    c0 = __ldg(p.ocol + q) & 0x7fffffff; i0 = __ldg(p.oidx + q);
+                    if (p1) { c1 = __ldg(p.ocol + q + 1) & 0x7fffffff; i1 = __ldg(p.oidx + q + 1); }
+                    if (p2) { c2 = __ldg(p.ocol + q + 2) & 0x7fffffff; i2 = __ldg(p.oidx + q + 2); }
+                    if (p3) { c3 = __ldg(p.ocol + q + 3) & 0x7fffffff; i3 = __ldg(p.oidx + q + 3); }
                     v0 = __ldg(p.vtab + i0);
                     if (p1) v1 = __ldg(p.vtab + i1);
                     if (p2) v2 = __ldg(p.vtab + i2);
@@ -319,7 +319,17 @@ int launch_term_m(const TermParams &p, int num_sms, cudaStream_t st, int *grid_o
 
 int launch_term(int bt, bool table, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
-    // warp-specialised bulk-copy kernel (term_ws.cu) whenever it has an instantiation for this term; else the direct kernel
+    // phased kernel (term_ph.cuh) whenever it has an instantiation for this term; TBPM_KERNEL=0: the earlier
+    // warp-specialised kernel with staged vectors (term_ws.cu); else the direct kernel below
+    if (table && env_int("TBPM_KERNEL", 1) != 0 && term_ph_supported(bt, p)) {
+        ++g_launches;
+        switch (bt) {
+        case 1: return launch_term_ph_bt1(p, num_sms, st, grid_out);
+        case 2: return launch_term_ph_bt2(p, num_sms, st, grid_out);
+        case 4: return launch_term_ph_bt4(p, num_sms, st, grid_out);
+        case 8: return launch_term_ph_bt8(p, num_sms, st, grid_out);
+        }
+    }
     if (table && term_ws_supported(bt, p)) {
         ++g_launches;
         return launch_term_ws(bt, p, num_sms, st, grid_out);
@@ -381,6 +391,7 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     tp.n_orb = H->n_orb;
     tp.partial = partial;
     tp.n_table = H->n_table;
+    tp.packed = H->packed;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
 
     for (int t = 0; t < P.n_tile; ++t) {

@@ -51,6 +51,7 @@ struct tbpm_ham {
     int32_t max_row_nnz = 0;
     double gershgorin = 0.0;
     int32_t n_table = 0;   // 0: kernels read complex128 values from the canonical CSR
+    int32_t packed = 0;    // n_table <= 2: bit 31 of every ocol word holds the value index (oidx is not read by the kernels)
     int device = 0;
     int num_sms = 0;
 

@@ -38,8 +38,13 @@ struct TermParams {
     int flags;
     int n_table;           // entries of vtab (kernel layout)
     int max_row_off;       // longest off-diagonal row (sizes the staged index slices)
+    int packed;            // n_table <= 2: bit 31 of every ocol word is the value index (build.cu, k_pack_cols)
     // warp-specialised kernel: shared-memory stage geometry (bytes), filled by its launcher
     int n_stage, stage_bytes, cap_entries, off_col, off_idx, off_diag, off_vec;
+    int chunk;             // phased kernel: consecutive tiles per run of a block
+    int64_t pf_rows;       // phased kernel: L2 prefetch distance in rows (0: off)
+    int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first, 2: bulk L2 prefetch of the streams)
+    int64_t x_lead;        // experiment: rows between a tile and the leading edge of its gather window
 };
 
 __device__ __forceinline__ void cfma(double2 &h, double2 v, double2 x)   // h += v * x (complex)
@@ -60,5 +65,12 @@ inline int env_int(const char *name, int dflt)
 // (the caller then uses the direct kernel).  *grid_out = blocks launched (sizes the final reduction).
 bool term_ws_supported(int bt, const TermParams &p);
 int launch_term_ws(int bt, TermParams p, int num_sms, cudaStream_t st, int *grid_out);
+
+// Phased kernel (term_ph.cuh): matrix slices staged by bulk copies, vectors streamed directly; one file per tile width.
+bool term_ph_supported(int bt, const TermParams &p);
+int launch_term_ph_bt1(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
+int launch_term_ph_bt2(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
+int launch_term_ph_bt4(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
+int launch_term_ph_bt8(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
 }  // namespace tbpm_detail

@@ -1,0 +1,526 @@
+// term_ph.cuh -- the hot kernel: fused Chebyshev term, TMA-staged MATRIX slices, directly streamed VECTORS, and an
+// explicitly phased instruction stream (all index loads -> all global loads -> all complex FMAs).
+//
+//   T_k = a*H*T_{k-1} - T_{k-2}  (amxsy)  fused with  psi' += sum c_j T_j  (axpy, up to
+//   three terms at once) and, on the last term of a time step, <psi0|psi'> and <psi'|psi'> (calc_corr_dos).
+//
+// Why this shape (profiles/r1_ncu_full_cfg4_cfg5.md): with 8 interleaved states per row the previous kernel (term_ws.cu)
+// was bound in the SM clock domain -- by L1 data-pipe wavefronts (16-25 per row where the gathers and the store need
+// 8-10) and by three to four serialised memory round trips per row (a warp pass took ~4800 cycles).  Here
+//   producer warp (one elected lane): for every tile of R rows, n_stage tiles ahead, bulk-copies (cp.async.bulk +
+//       mbarrier complete_tx; SASS UBLKCP) ONLY the matrix slices of the tile -- row offsets, packed column words,
+//       value indices (large tables only), real diagonal -- into a 2-7 KB shared-memory stage;
+//   consumer warps: issue the streamed operands of their row (y, psi', psi0, x[row]; coalesced 128/256-bit LDG) before
+//       they even wait for the stage; then read ALL their indices from shared memory, release the stage at once
+//       (the producer refills it while the gathers are in flight), issue ALL gathers of x[col] back to back (one
+//       memory round trip per row of <= CH entries), and only then run the complex FMAs.  Results go straight to
+//       global memory.  No block-wide barrier in the main loop.
+//
+// Thread -> (row, SPT consecutive states).  What varies per term (accumulate 0..3 terms, reduce or not) is a template
+// parameter; what varies rarely (first term, first flush, diagonal present) is a warp-uniform runtime predicate.
+#pragma once
+
+#include <algorithm>
+
+#include "term.h"
+
+namespace tbpm_detail {
+namespace ph {
+
+constexpr int kMaxStages = 8;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes),
+                 "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_prefetch_l2(const void *src, uint32_t bytes)    // async engine, no LSU work (SASS UBLKPF)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u32_if(uint32_t a, bool on)      // 0 when off
+{
+    uint32_t v;
+    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\nmov.u32 %0, 0;\n@q ld.shared.u32 %0, [%1];\n}" : "=r"(v) : "r"(a), "r"((int)on));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u16_if(uint32_t a, bool on)
+{
+    uint32_t v;
+    asm volatile("{\n.reg .pred q;\n.reg .u16 h;\nsetp.ne.b32 q, %2, 0;\nmov.u16 h, 0;\n@q ld.shared.u16 h, [%1];\ncvt.u32.u16 %0, h;\n}"
+                 : "=r"(v)
+                 : "r"(a), "r"((int)on));
+    return v;
+}
+__device__ __forceinline__ double lds_f64(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+
+// SPT consecutive complex128 values of one row
+template <int SPT> struct CVec;
+template <> struct CVec<1> {
+    double2 v[1];
+    __device__ __forceinline__ void zero() { v[0] = make_double2(0.0, 0.0); }
+    __device__ __forceinline__ void gather_if(const double2 *p, bool on)      // read-only path, cacheable; zeros when off
+    {
+        asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %3, 0;\nmov.f64 %0, 0d0000000000000000;\nmov.f64 %1, 0d0000000000000000;\n"
+                     "@q ld.global.nc.v2.f64 {%0, %1}, [%2];\n}"
+                     : "=d"(v[0].x), "=d"(v[0].y)
+                     : "l"(p), "r"((int)on));
+    }
+    __device__ __forceinline__ void stream_if(const double2 *p, bool on)      // read once: evict first
+    {
+        asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %3, 0;\nmov.f64 %0, 0d0000000000000000;\nmov.f64 %1, 0d0000000000000000;\n"
+                     "@q ld.global.cs.v2.f64 {%0, %1}, [%2];\n}"
+                     : "=d"(v[0].x), "=d"(v[0].y)
+                     : "l"(p), "r"((int)on)
+                     : "memory");
+    }
+    __device__ __forceinline__ void st(double2 *p) const
+    {
+        asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v[0].x), "d"(v[0].y) : "memory");
+    }
+    __device__ __forceinline__ void st_stream(double2 *p) const
+    {
+        asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v[0].x), "d"(v[0].y) : "memory");
+    }
+};
+template <> struct CVec<2> {
+    double2 v[2];
+    __device__ __forceinline__ void zero() { v[0] = v[1] = make_double2(0.0, 0.0); }
+    __device__ __forceinline__ void gather_if(const double2 *p, bool on)      // one 256-bit load (LDG.E.256)
+    {
+        asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %5, 0;\nmov.f64 %0, 0d0000000000000000;\nmov.f64 %1, 0d0000000000000000;\n"
+                     "mov.f64 %2, 0d0000000000000000;\nmov.f64 %3, 0d0000000000000000;\n"
+                     "@q ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];\n}"
+                     : "=d"(v[0].x), "=d"(v[0].y), "=d"(v[1].x), "=d"(v[1].y)
+                     : "l"(p), "r"((int)on));
+    }
+    __device__ __forceinline__ void stream_if(const double2 *p, bool on)
+    {
+        asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %5, 0;\nmov.f64 %0, 0d0000000000000000;\nmov.f64 %1, 0d0000000000000000;\n"
+                     "mov.f64 %2, 0d0000000000000000;\nmov.f64 %3, 0d0000000000000000;\n"
+                     "@q ld.global.L1::no_allocate.L2::evict_first.v4.f64 {%0, %1, %2, %3}, [%4];\n}"
+                     : "=d"(v[0].x), "=d"(v[0].y), "=d"(v[1].x), "=d"(v[1].y)
+                     : "l"(p), "r"((int)on)
+                     : "memory");
+    }
+    __device__ __forceinline__ void st(double2 *p) const
+    {
+        asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v[0].x), "d"(v[0].y), "d"(v[1].x), "d"(v[1].y) : "memory");
+    }
+    __device__ __forceinline__ void st_stream(double2 *p) const
+    {
+        asm volatile("st.global.L1::no_allocate.L2::evict_first.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v[0].x), "d"(v[0].y), "d"(v[1].x),
+                     "d"(v[1].y)
+                     : "memory");
+    }
+};
+
+__device__ __forceinline__ void prefetch_l2_if(const void *p, bool on)
+{
+    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %1, 0;\n@q prefetch.global.L2 [%0];\n}" ::"l"(p), "r"((int)on));
+}
+
+__device__ __forceinline__ double2 ldg_value_if(const double2 *p, bool on)
+{
+    double2 v;
+    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %3, 0;\nmov.f64 %0, 0d0000000000000000;\nmov.f64 %1, 0d0000000000000000;\n"
+                 "@q ld.global.nc.v2.f64 {%0, %1}, [%2];\n}"
+                 : "=d"(v.x), "=d"(v.y)
+                 : "l"(p), "r"((int)on));
+    return v;
+}
+
+// BT states per tile row, SPT states per thread, CH gathers in flight per thread, NACC terms added to psi' by this launch
+// (0..3), REDUCE: last term of the time step (dot products, T_k not stored), T2: at most two distinct hopping values --
+// they live in registers and bit 31 of the packed column word selects one (build.cu, k_pack_cols).
+// NW consumer warps + 1 producer warp form the only block of an SM: (NW + 1) * 32 threads share the 64 K registers.
+template <int BT, int SPT, int CH, int NACC, bool REDUCE, bool T2, int NW>
+__global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p)
+{
+    constexpr int kConsumers = NW * 32;
+    constexpr int LPR = BT / SPT;                           // lanes per row
+    constexpr int R = kConsumers / LPR;                     // rows per tile
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ __align__(8) uint64_t bars[2 * kMaxStages];  // [0, S): full, [kMaxStages, kMaxStages + S): empty
+    __shared__ uint32_t lo_s[kMaxStages][2];                // first column / value-index element held by each stage
+    __shared__ double red_s[REDUCE ? kConsumers / 32 : 1][REDUCE ? BT : 1][3];
+
+    const int tid = threadIdx.x;
+    const bool sub_y = p.flags & F_SUB_Y;
+    const bool need_y = sub_y || NACC == 3;
+    const bool need_acc = NACC > 0 && !(p.flags & F_ACC_INIT);
+    const bool has_diag = p.diag != nullptr;
+    const bool need_xrow = NACC >= 2 || has_diag;
+    const int S = p.n_stage;
+    const int64_t n_tiles = (p.n_orb + R - 1) / R;
+    const uint32_t bar0 = smem_u32(bars), smem0 = smem_u32(smem);
+
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) { mbar_init(bar0 + 8 * s, 1); mbar_init(bar0 + 8 * (kMaxStages + s), kConsumers / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // Tile order of a block: runs of `chunk` consecutive tiles, runs dealt round-robin to the blocks.  All blocks together
+    // still sweep one moving window of the vectors (L2 locality), and inside a run the rows a block gathered for one tile
+    // (its lattice neighbours one line up) are the rows of its next tiles: they hit in its L1 instead of crossing the
+    // L2-to-SM fabric, which caps out near 6300 B/clk chip-wide (ncu: 79 % of it at chunk = 1, profiles/).
+    const int chunk = p.chunk;
+    const int64_t first_tile = (int64_t)blockIdx.x * chunk;
+    const int64_t run_skip = (int64_t)(gridDim.x - 1) * chunk + 1;
+    auto next_tile = [&](int64_t t, int &i) -> int64_t {
+        if (++i == chunk) { i = 0; return t + run_skip; }
+        return t + 1;
+    };
+
+    if (tid >= kConsumers) {
+        // ------------------------------------------------ producer warp ------------------------------------------------
+        if (tid != kConsumers) return;
+        uint32_t q_lo = 0, q_hi = 0;                        // offsets bounding the next tile to issue (prefetched)
+        int64_t tile = first_tile;
+        if (tile < n_tiles) {
+            const int64_t r0 = tile * R;
+            q_lo = __ldg(p.orp + r0);
+            q_hi = __ldg(p.orp + min(r0 + R, p.n_orb));
+        }
+        int s = 0, ci = 0;
+        uint32_t ph = 1;                                    // parity of the "empty" phase to wait for; first pass: free
+        for (; tile < n_tiles; tile = next_tile(tile, ci)) {
+            const uint32_t c_lo = q_lo, c_hi = q_hi;
+            int cj = ci;
+            const int64_t nt = next_tile(tile, cj);
+            if (nt < n_tiles) {                             // bounds of the following tile: latency hidden behind this issue
+                const int64_t nr0 = nt * R;
+                q_lo = __ldg(p.orp + nr0);
+                q_hi = __ldg(p.orp + min(nr0 + R, p.n_orb));
+            }
+            const uint32_t full = bar0 + 8 * s;
+            mbar_wait(bar0 + 8 * (kMaxStages + s), ph);     // a fresh barrier reports the "previous" phase complete
+            const uint32_t st = smem0 + (uint32_t)s * (uint32_t)p.stage_bytes;
+            const int64_t r0 = tile * R;
+            const int rows = (int)min((int64_t)R, p.n_orb - r0);
+            const uint32_t col_lo = c_lo & ~3u, idx_lo = c_lo & ~7u;
+            const uint32_t nc = ((c_hi - col_lo) + 3u) & ~3u, ni = ((c_hi - idx_lo) + 7u) & ~7u;
+            lo_s[s][0] = col_lo;
+            lo_s[s][1] = idx_lo;
+            const uint32_t orp_bytes = (uint32_t)(((rows + 1) * 4 + 15) & ~15);
+            uint32_t tx = orp_bytes;
+            bulk_g2s(st, p.orp + r0, orp_bytes, full);
+            if (nc > 0) {
+                bulk_g2s(st + p.off_col, p.ocol + col_lo, nc * 4, full);
+                tx += nc * 4;
+                if (!T2) { bulk_g2s(st + p.off_idx, p.oidx + idx_lo, ni * 2, full); tx += ni * 2; }
+            }
+            if (has_diag) {
+                const uint32_t db = (uint32_t)((rows * 8 + 15) & ~15);
+                bulk_g2s(st + p.off_diag, p.diag + r0, db, full);
+                tx += db;
+            }
+            mbar_expect_tx(full, tx);                       // release: also publishes lo_s[s]
+            if (p.pol & 2) {                                // HBM -> L2 for the vector rows this tile will stream, n_stage tiles ahead
+                const uint32_t vb = (uint32_t)rows * BT * sizeof(double2);
+                const int64_t e0 = r0 * BT;
+                if (need_y) bulk_prefetch_l2(p.y + e0, vb);
+                if (need_acc) bulk_prefetch_l2(p.acc + e0, vb);
+                if (REDUCE) bulk_prefetch_l2(p.psi0 + e0, vb);
+                if (p.x_lead > 0 && r0 + p.x_lead + rows <= p.n_orb) bulk_prefetch_l2(p.x + (r0 + p.x_lead) * BT, vb);
+            }
+            if (++s == S) { s = 0; ph ^= 1u; }
+        }
+        return;
+    }
+
+    // ---------------------------------------------------- consumer warps ----------------------------------------------------
+    const int rl = tid / LPR;                               // row within the tile
+    const int b0 = (tid % LPR) * SPT;                       // first state of this thread
+    const double2 *xb = p.x + b0;
+    const int64_t pf_rows = p.pf_rows, pf_el = pf_rows * BT;
+    const bool st_ef = p.pol & 1;                           // T_k leaves L2 first (its readers come a whole sweep later)
+    const uint32_t stage_bytes = (uint32_t)p.stage_bytes;
+    const uint32_t a_orp = smem0 + (uint32_t)rl * 4u, a_col = smem0 + (uint32_t)p.off_col, a_idx = smem0 + (uint32_t)p.off_idx,
+                   a_diag = smem0 + (uint32_t)p.off_diag + (uint32_t)rl * 8u;
+    double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // T2: the (at most two) hopping values, in registers
+    if (T2) {
+        t0 = __ldg(p.vtab);
+        t1 = p.n_table > 1 ? __ldg(p.vtab + 1) : t0;
+    }
+    double s_re[SPT], s_im[SPT], s_nn[SPT];
+#pragma unroll
+    for (int k = 0; k < SPT; ++k) s_re[k] = s_im[k] = s_nn[k] = 0.0;
+
+    // The loop is ROTATED: an iteration first consumes the chunk that the previous iteration (or the prologue) loaded,
+    // then loads the next chunk.  The loads and their uses are thereby separated by the loop back edge, which the
+    // assembler's scheduler does not move code across -- left in one basic block it sinks six of eight gathers below the
+    // first complex FMA and serialises the memory round trips.
+    int s = 0;
+    uint32_t ph = 0, so = 0;                                // so: byte offset of stage s
+    int64_t tile = first_tile;
+    int ci = 0;
+    bool valid = false;
+    int64_t e = 0;
+    uint32_t n = 0, nmax = 0, c0 = 0, ca = 0, ia = 0;
+    double d = 0.0;
+    CVec<SPT> yold, xrow, aold, z, h;
+    CVec<SPT> x[CH];
+    double2 v[CH];
+    uint32_t w[CH];
+
+    auto load_row = [&]() {                                 // streamed operands + row header of `tile`
+        const int64_t row = tile * R + rl;
+        valid = row < p.n_orb;
+        e = row * BT + b0;
+        // streamed operands of the row (HBM latency; they need no index, so they leave before the wait)
+        yold.stream_if(p.y + e, valid && need_y);
+        if (NACC > 0) aold.stream_if(p.acc + e, valid && need_acc);
+        if (REDUCE) z.stream_if(p.psi0 + e, valid);
+        xrow.gather_if(p.x + e, valid && need_xrow);        // the tile's own x rows are gathered by its neighbours: L1/L2 hit
+        if (pf_rows > 0) {                                  // the same operands of this block's next tile: HBM -> L2 now
+            const bool on = row + pf_rows < p.n_orb;
+            prefetch_l2_if(p.y + e + pf_el, on && need_y);
+            if (NACC > 0) prefetch_l2_if(p.acc + e + pf_el, on && need_acc);
+            if (REDUCE) prefetch_l2_if(p.psi0 + e + pf_el, on);
+        }
+        mbar_wait(bar0 + 8 * s, ph);
+        const uint32_t q0 = lds_u32(a_orp + so), q1 = lds_u32(a_orp + so + 4u);
+        n = valid ? q1 - q0 : 0u;
+        ca = a_col + so + (q0 - lo_s[s][0]) * 4u;
+        ia = a_idx + so + (q0 - lo_s[s][1]) * 2u;
+        d = has_diag ? lds_f64(a_diag + so) : 0.0;
+        nmax = __reduce_max_sync(0xffffffffu, n);
+        c0 = 0;
+        h.zero();
+    };
+    auto load_chunk = [&]() {                               // indices of entries [c0, c0 + CH) of the row, then their gathers
+        uint32_t id[CH];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) {
+            w[j] = lds_u32_if(ca + 4u * (c0 + j), c0 + j < n);
+            id[j] = T2 ? 0u : lds_u16_if(ia + 2u * (c0 + j), c0 + j < n);
+        }
+        if (c0 + CH >= nmax) {                              // last chunk of every row of this warp: the stage is free again
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(bar0 + 8 * (kMaxStages + s));
+            if (++s == S) { s = 0; ph ^= 1u; so = 0; } else so += stage_bytes;
+        }
+#pragma unroll
+        for (int j = 0; j < CH; ++j) x[j].gather_if(xb + (int64_t)(w[j] & 0x7fffffffu) * BT, c0 + j < n);
+        if (pf_rows > 0) {                                  // leading edge of the gather window (largest column), one tile ahead
+            uint32_t cmax = 0;
+#pragma unroll
+            for (int j = 0; j < CH; ++j) cmax = max(cmax, w[j] & 0x7fffffffu);
+            prefetch_l2_if(xb + ((int64_t)cmax + pf_rows) * BT, c0 < n && (int64_t)cmax + pf_rows < p.n_orb);
+        }
+        if (!T2) {
+#pragma unroll
+            for (int j = 0; j < CH; ++j) v[j] = ldg_value_if(p.vtab + id[j], c0 + j < n);
+        }
+    };
+
+    if (tile < n_tiles) {
+        load_row();
+        load_chunk();
+    }
+#pragma unroll 1
+    while (tile < n_tiles) {
+        // ---- consume: complex FMAs of the chunk in flight, in issue order
+#pragma unroll
+        for (int j = 0; j < CH; ++j) {
+            if (T2) v[j] = (w[j] >> 31) ? t1 : t0;
+#pragma unroll
+            for (int k = 0; k < SPT; ++k) cfma(h.v[k], v[j], x[j].v[k]);   // x[j] is zero past the row end
+        }
+        c0 += CH;
+        if (c0 >= nmax) {
+            // ---- epilogue of the row: diagonal, scale, subtract, store, accumulate, reduce
+            if (has_diag) {
+#pragma unroll
+                for (int k = 0; k < SPT; ++k) { h.v[k].x = fma(d, xrow.v[k].x, h.v[k].x); h.v[k].y = fma(d, xrow.v[k].y, h.v[k].y); }
+            }
+#pragma unroll
+            for (int k = 0; k < SPT; ++k) { h.v[k].x *= p.a; h.v[k].y *= p.a; }
+            if (sub_y) {
+#pragma unroll
+                for (int k = 0; k < SPT; ++k) { h.v[k].x -= yold.v[k].x; h.v[k].y -= yold.v[k].y; }
+            }
+            if (valid) {
+                if (!REDUCE) { if (st_ef) h.st_stream(p.y + e); else h.st(p.y + e); }   // T_k
+                if (NACC > 0) {
+#pragma unroll
+                    for (int k = 0; k < SPT; ++k) {
+                        cfma(aold.v[k], p.ca, h.v[k]);
+                        if (NACC >= 2) cfma(aold.v[k], p.cb, xrow.v[k]);
+                        if (NACC == 3) cfma(aold.v[k], p.cc, yold.v[k]);
+                    }
+                    if (REDUCE) {
+#pragma unroll
+                        for (int k = 0; k < SPT; ++k) {
+                            s_re[k] = fma(z.v[k].x, aold.v[k].x, s_re[k]);      // conj(z) * psi'
+                            s_re[k] = fma(z.v[k].y, aold.v[k].y, s_re[k]);
+                            s_im[k] = fma(z.v[k].x, aold.v[k].y, s_im[k]);
+                            s_im[k] = fma(-z.v[k].y, aold.v[k].x, s_im[k]);
+                            s_nn[k] = fma(aold.v[k].x, aold.v[k].x, s_nn[k]);
+                            s_nn[k] = fma(aold.v[k].y, aold.v[k].y, s_nn[k]);
+                        }
+                        aold.st(p.acc + e);                 // psi': T_0 of the next step, gathered right away
+                    } else {
+                        aold.st_stream(p.acc + e);
+                    }
+                }
+            }
+            tile = next_tile(tile, ci);
+            if (tile >= n_tiles) break;
+            load_row();
+        }
+        // ---- load: the next chunk (of this row, or the first of the next tile's row)
+        load_chunk();
+    }
+
+    if (REDUCE) {
+#pragma unroll
+        for (int k = 0; k < SPT; ++k) {                     // lanes with equal (lane % LPR) hold the same states
+#pragma unroll
+            for (int o = 16; o >= LPR; o >>= 1) {
+                s_re[k] += __shfl_xor_sync(0xffffffffu, s_re[k], o);
+                s_im[k] += __shfl_xor_sync(0xffffffffu, s_im[k], o);
+                s_nn[k] += __shfl_xor_sync(0xffffffffu, s_nn[k], o);
+            }
+        }
+        const int lane = tid & 31, warp = tid >> 5;
+        if (lane < LPR) {
+#pragma unroll
+            for (int k = 0; k < SPT; ++k) {
+                red_s[warp][lane * SPT + k][0] = s_re[k];
+                red_s[warp][lane * SPT + k][1] = s_im[k];
+                red_s[warp][lane * SPT + k][2] = s_nn[k];
+            }
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");   // consumers only (the producer warp has left)
+        if (tid < BT * 3) {
+            const int bb = tid / 3, c = tid % 3;
+            double t = 0.0;
+#pragma unroll
+            for (int w = 0; w < kConsumers / 32; ++w) t += red_s[w][bb][c];
+            p.partial[((int64_t)blockIdx.x * BT + bb) * 3 + c] = t;
+        }
+    }
+}
+
+template <int BT, int SPT, int CH, int NACC, bool REDUCE, bool T2, int NW>
+int launch_one(TermParams p, int num_sms, cudaStream_t st, int *grid_out)
+{
+    constexpr int kConsumers = NW * 32, kThreads = kConsumers + 32;
+    constexpr int R = kConsumers / (BT / SPT);
+    p.n_stage = std::min(kMaxStages, std::max(2, env_int("TBPM_STAGES", 4)));
+    p.chunk = std::max(1, env_int("TBPM_CHUNK", 1));
+    p.cap_entries = ((R * std::max(p.max_row_off, 1) + 8 + 7) / 8) * 8;          // + alignment slack of the slice start
+    size_t o = (size_t)(((R + 1) * 4 + 15) & ~15);
+    p.off_col = (int)o;  o += (size_t)p.cap_entries * 4;
+    p.off_idx = (int)o;  o += T2 ? 0 : (size_t)p.cap_entries * 2;
+    o = (o + 15) & ~size_t(15);
+    p.off_diag = (int)o; o += (size_t)((R * 8 + 15) & ~15);
+    p.off_vec = 0;
+    p.stage_bytes = (int)((o + 127) & ~size_t(127));
+    p.n_stage = (int)std::max<size_t>(2, std::min<size_t>(p.n_stage, (size_t)160 * 1024 / p.stage_bytes));
+    const size_t dyn = (size_t)p.stage_bytes * p.n_stage;
+    auto kern = k_term_ph<BT, SPT, CH, NACC, REDUCE, T2, NW>;
+    static size_t configured = 0;
+    static int cached_nb = 0;
+    static size_t cached_dyn = 0;
+    if (dyn > configured) {
+        const size_t want = std::max(dyn, (size_t)64 * 1024);
+        TBPM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)want));
+        configured = want;
+    }
+    if (cached_dyn != dyn || cached_nb == 0) {
+        int nb = 0;
+        TBPM_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, kThreads, dyn));
+        if (nb < 1) return TBPM_ENOMEM;
+        cached_nb = nb;
+        cached_dyn = dyn;
+    }
+    const int nb = std::min(cached_nb, std::max(1, env_int("TBPM_MAXB", 8)));
+    const int64_t need = (p.n_orb + R - 1) / R;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>({need, (int64_t)num_sms * nb, (int64_t)kMaxGrid}));
+    p.pol = env_int("TBPM_POL", 1);
+    p.x_lead = env_int("TBPM_XLEAD", 0);
+    p.pf_rows = p.chunk == 1 ? (int64_t)env_int("TBPM_PF", 0) * grid * R : 0;      // prefetch distance: whole tiles of this block
+    kern<<<grid, kThreads, dyn, st>>>(p);
+    count_launches(1);
+    *grid_out = grid;
+    return TBPM_OK;
+}
+
+template <int BT, int SPT, int CH, bool T2, int NW>
+int launch_variant(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
+{
+    const bool red = p.flags & F_REDUCE;
+    if (!red && p.n_acc == 0) return launch_one<BT, SPT, CH, 0, false, T2, NW>(p, num_sms, st, grid_out);
+    if (!red && p.n_acc == 3) return launch_one<BT, SPT, CH, 3, false, T2, NW>(p, num_sms, st, grid_out);
+    if (red && p.n_acc == 1) return launch_one<BT, SPT, CH, 1, true, T2, NW>(p, num_sms, st, grid_out);
+    if (red && p.n_acc == 2) return launch_one<BT, SPT, CH, 2, true, T2, NW>(p, num_sms, st, grid_out);
+    if (red && p.n_acc == 3) return launch_one<BT, SPT, CH, 3, true, T2, NW>(p, num_sms, st, grid_out);
+    return TBPM_EINVAL;
+}
+
+// Shape of the instruction stream per (tile width, table kind, row length).  One block per SM; its (NW + 1) warps share
+// the register file: NW = 23 -> 80 registers per thread, NW = 15 -> 128.
+//   T2 (<= 2 hopping values in registers): CH = 8 gathers in flight on 15 warps, except single-state tiles with rows of
+//   <= 4 entries (CH = 4 on 23 warps); large tables (values fetched per entry, 4 more registers each): CH = 4 on 15 warps.
+template <int BT>
+int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
+{
+    constexpr int SPT = BT >= 2 ? 2 : 1;
+    const bool t2 = p.packed != 0;
+    const int ch = env_int("TBPM_CH", (t2 && (BT >= 2 || p.max_row_off > 4)) ? 8 : 4);
+    if constexpr (BT == 8) if (env_int("TBPM_SPT", 2) == 1) {   // experiment: 128-bit gathers, one state per thread
+        if (t2) return launch_variant<BT, 1, 8, true, 23>(p, num_sms, st, grid_out);
+        return launch_variant<BT, 1, 8, false, 15>(p, num_sms, st, grid_out);
+    }
+    if (t2) {
+        if (ch == 8) return launch_variant<BT, SPT, 8, true, 15>(p, num_sms, st, grid_out);
+        return launch_variant<BT, SPT, 4, true, 23>(p, num_sms, st, grid_out);
+    }
+    return launch_variant<BT, SPT, 4, false, 15>(p, num_sms, st, grid_out);
+}
+
+}  // namespace ph
+}  // namespace tbpm_detail

@@ -1,0 +1,9 @@
+// term_ph_bt2.cu -- instantiations of the fused Chebyshev-term kernel (term_ph.cuh) for tiles of 2 interleaved state(s).
+#include "term_ph.cuh"
+
+namespace tbpm_detail {
+int launch_term_ph_bt2(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
+{
+    return ph::launch_bt<2>(p, num_sms, st, grid_out);
+}
+}  // namespace tbpm_detail

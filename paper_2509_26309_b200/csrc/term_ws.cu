@@ -213,10 +213,10 @@ __global__ void __launch_bounds__(kWsThreads, 3) k_term_ws(const TermParams p)
                 CVec<SPT> x0, x1, x2, x3;
 #pragma unroll
                 for (int k = 0; k < SPT; ++k) x1.v[k] = x2.v[k] = x3.v[k] = make_double2(0.0, 0.0);
-                x0.ldg(xb + (int64_t)cs[j] * BT);
-                if (p1) x1.ldg(xb + (int64_t)cs[j + 1] * BT);
-                if (p2) x2.ldg(xb + (int64_t)cs[j + 2] * BT);
-                if (p3) x3.ldg(xb + (int64_t)cs[j + 3] * BT);
+                x0.ldg(xb + (int64_t)(cs[j] & 0x7fffffff) * BT);
+                if (p1) x1.ldg(xb + (int64_t)(cs[j + 1] & 0x7fffffff) * BT);
+                if (p2) x2.ldg(xb + (int64_t)(cs[j + 2] & 0x7fffffff) * BT);
+                if (p3) x3.ldg(xb + (int64_t)(cs[j + 3] & 0x7fffffff) * BT);
                 const double2 v0 = value(is[j]);
                 const double2 v1 = value(p1 ? is[j + 1] : 0), v2 = value(p2 ? is[j + 2] : 0), v3 = value(p3 ? is[j + 3] : 0);
 #pragma unroll
@@ -388,6 +388,12 @@ int launch_term_ws(int bt, TermParams p, int num_sms, cudaStream_t st, int *grid
     case 8: return t2 ? launch_variant<8, true>(p, num_sms, st, grid_out) : launch_variant<8, false>(p, num_sms, st, grid_out);
     }
     return TBPM_EINVAL;
+}
+
+bool term_ph_supported(int bt, const TermParams &p)
+{
+    if (!term_ws_supported(bt, p)) return false;
+    return p.max_row_off <= 8;                                                   // two stages of the widest tile fit 160 KB
 }
 
 }  // namespace tbpm_detail
