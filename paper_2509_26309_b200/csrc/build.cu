@@ -19,6 +19,7 @@
 //      k_tab_insert / scan / k_tab_key / k_tab_compact / k_tab_rank / k_tab_number / k_tab_lookup
 //      ("hopping-table index for uniform lattices", north_star)
 #include <algorithm>
+#include <climits>
 #include <cstring>
 #include <new>
 
@@ -203,12 +204,13 @@ __global__ void k_fill(int64_t n_hop, const int32_t *__restrict__ hop_i, const i
 __global__ void k_sort_rows(int64_t n_orb, const int64_t *__restrict__ rowptr, int32_t *col, double2 *val, int32_t *status)
 {
     int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    int len = 0;
+    int len = 0, nlen = 0;                                  // nlen = -len of real rows: warp max of it is -(shortest row)
     double rowsum = 0.0;
     bool dup = false;
     if (r < n_orb) {
         int64_t b = rowptr[r], e = rowptr[r + 1];
         len = (int)(e - b);
+        nlen = -len;
         for (int64_t p = b + 1; p < e; ++p) {
             int32_t c = col[p];
             double2 v = val[p];
@@ -228,13 +230,16 @@ __global__ void k_sort_rows(int64_t n_orb, const int64_t *__restrict__ rowptr, i
         }
     }
     // block-level max to keep the number of global atomics small
+    if (r >= n_orb) nlen = INT_MIN;
     for (int o = 16; o > 0; o >>= 1) {
         len = max(len, __shfl_xor_sync(0xffffffffu, len, o));
+        nlen = max(nlen, __shfl_xor_sync(0xffffffffu, nlen, o));
         rowsum = fmax(rowsum, __shfl_xor_sync(0xffffffffu, rowsum, o));
     }
     if (__any_sync(0xffffffffu, dup) && (threadIdx.x & 31) == 0) atomicOr(&status[ST_ERR], 4);
     if ((threadIdx.x & 31) == 0) {
         atomicMax(&status[ST_MAX_ROW], len);
+        if (nlen != INT_MIN) atomicMax(&status[ST_NEG_MIN_ROW], nlen + (1 << 30));   // biased so that the zero-initialised word loses
         atomicMax(reinterpret_cast<unsigned long long *>(&status[ST_GERSH_LO]), (unsigned long long)__double_as_longlong(rowsum));
     }
 }
@@ -524,6 +529,7 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
     if (hst[ST_ERR] & 2) return fail(TBPM_EDIAG);
     if (hst[ST_ERR] & 4) return fail(TBPM_EDUP);
     H->max_row_nnz = hst[ST_MAX_ROW];
+    H->min_row_nnz = n_orb > 0 ? (1 << 30) - hst[ST_NEG_MIN_ROW] : 0;
     uint64_t gb = (uint64_t)(uint32_t)hst[ST_GERSH_LO] | ((uint64_t)(uint32_t)hst[ST_GERSH_HI] << 32);
     std::memcpy(&H->gershgorin, &gb, sizeof(double));
     H->n_table = 0;
@@ -542,6 +548,13 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
         TRY_OR_FAIL(cudaGetLastError());
         TRY_OR_FAIL(cudaStreamSynchronize(st));
         H->packed = pack;
+        H->single_real = 0;
+        if (n_table == 1) {                                  // one real hopping value: kernels sum the neighbours, then scale
+            double2 v0;
+            TRY_OR_FAIL(cudaMemcpyAsync(&v0, H->vtab, sizeof(double2), cudaMemcpyDeviceToHost, st));
+            TRY_OR_FAIL(cudaStreamSynchronize(st));
+            H->single_real = (v0.y == 0.0);
+        }
         H->n_table = hst[ST_NTAB];
     }
 #undef TRY_OR_FAIL

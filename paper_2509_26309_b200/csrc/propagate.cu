@@ -392,6 +392,8 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     tp.partial = partial;
     tp.n_table = H->n_table;
     tp.packed = H->packed;
+    tp.single_real = H->single_real;
+    tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
 
     for (int t = 0; t < P.n_tile; ++t) {

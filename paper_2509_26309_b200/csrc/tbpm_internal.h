@@ -35,7 +35,8 @@ enum StatusWord {
     ST_GERSH_LO = 2,     // bits of the double max_i (|onsite_i| + sum_j |H_ij|)   (non-negative doubles order as u64)
     ST_GERSH_HI = 3,
     ST_NTAB = 4,         // number of distinct off-diagonal values inserted into the hash table
-    ST_TAB_OVERFLOW = 5  // more than kTableMax distinct values (or a probe sequence gave up)
+    ST_TAB_OVERFLOW = 5, // more than kTableMax distinct values (or a probe sequence gave up)
+    ST_NEG_MIN_ROW = 6   // 2^30 - (fewest entries in a row of the canonical CSR)
 };
 
 }  // namespace tbpm_detail
@@ -49,6 +50,8 @@ struct tbpm_ham {
     int has_onsite = 0;
     uint32_t flags = 0;
     int32_t max_row_nnz = 0;
+    int32_t min_row_nnz = 0;
+    int32_t single_real = 0;   // the table holds one value and it is real
     double gershgorin = 0.0;
     int32_t n_table = 0;   // 0: kernels read complex128 values from the canonical CSR
     int32_t packed = 0;    // n_table <= 2: bit 31 of every ocol word holds the value index (oidx is not read by the kernels)

@@ -42,9 +42,9 @@ struct TermParams {
     // warp-specialised kernel: shared-memory stage geometry (bytes), filled by its launcher
     int n_stage, stage_bytes, cap_entries, off_col, off_idx, off_diag, off_vec;
     int chunk;             // phased kernel: consecutive tiles per run of a block
-    int64_t pf_rows;       // phased kernel: L2 prefetch distance in rows (0: off)
-    int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first, 2: bulk L2 prefetch of the streams)
-    int64_t x_lead;        // experiment: rows between a tile and the leading edge of its gather window
+    int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
+    int uniform;           // every row holds exactly max_row_off off-diagonal entries
+    int single_real;       // the table holds one value and it is real
 };
 
 __device__ __forceinline__ void cfma(double2 &h, double2 v, double2 x)   // h += v * x (complex)

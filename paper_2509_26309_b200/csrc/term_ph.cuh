@@ -28,6 +28,7 @@ namespace tbpm_detail {
 namespace ph {
 
 constexpr int kMaxStages = 8;
+constexpr int kNwA = 23, kNwB = 19;       // consumer warps of the short-row / six-entry shapes (see launch_bt)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
@@ -62,10 +63,6 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
                  "r"(bar)
                  : "memory");
 }
-__device__ __forceinline__ void bulk_prefetch_l2(const void *src, uint32_t bytes)    // async engine, no LSU work (SASS UBLKPF)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
-}
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a)
 {
     uint32_t v;
@@ -86,6 +83,12 @@ __device__ __forceinline__ uint32_t lds_u16_if(uint32_t a, bool on)
                  : "r"(a), "r"((int)on));
     return v;
 }
+__device__ __forceinline__ uint32_t lds_u16(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("{\n.reg .u16 h;\nld.shared.u16 h, [%1];\ncvt.u32.u16 %0, h;\n}" : "=r"(v) : "r"(a));
+    return v;
+}
 __device__ __forceinline__ double lds_f64(uint32_t a)
 {
     double v;
@@ -104,6 +107,10 @@ template <> struct CVec<1> {
                      "@q ld.global.nc.v2.f64 {%0, %1}, [%2];\n}"
                      : "=d"(v[0].x), "=d"(v[0].y)
                      : "l"(p), "r"((int)on));
+    }
+    __device__ __forceinline__ void gather(const double2 *p)
+    {
+        asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(v[0].x), "=d"(v[0].y) : "l"(p));
     }
     __device__ __forceinline__ void stream_if(const double2 *p, bool on)      // read once: evict first
     {
@@ -133,6 +140,10 @@ template <> struct CVec<2> {
                      : "=d"(v[0].x), "=d"(v[0].y), "=d"(v[1].x), "=d"(v[1].y)
                      : "l"(p), "r"((int)on));
     }
+    __device__ __forceinline__ void gather(const double2 *p)
+    {
+        asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v[0].x), "=d"(v[0].y), "=d"(v[1].x), "=d"(v[1].y) : "l"(p));
+    }
     __device__ __forceinline__ void stream_if(const double2 *p, bool on)
     {
         asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %5, 0;\nmov.f64 %0, 0d0000000000000000;\nmov.f64 %1, 0d0000000000000000;\n"
@@ -154,11 +165,6 @@ template <> struct CVec<2> {
     }
 };
 
-__device__ __forceinline__ void prefetch_l2_if(const void *p, bool on)
-{
-    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %1, 0;\n@q prefetch.global.L2 [%0];\n}" ::"l"(p), "r"((int)on));
-}
-
 __device__ __forceinline__ double2 ldg_value_if(const double2 *p, bool on)
 {
     double2 v;
@@ -170,10 +176,14 @@ __device__ __forceinline__ double2 ldg_value_if(const double2 *p, bool on)
 }
 
 // BT states per tile row, SPT states per thread, CH gathers in flight per thread, NACC terms added to psi' by this launch
-// (0..3), REDUCE: last term of the time step (dot products, T_k not stored), T2: at most two distinct hopping values --
-// they live in registers and bit 31 of the packed column word selects one (build.cu, k_pack_cols).
+// (0..3), REDUCE: last term of the time step (dot products, T_k not stored).
+// VK, where the hopping values come from:  0 = 16-bit index per entry into the table in global memory;  1 = at most two
+//   values, in registers, selected by bit 31 of the packed column word (build.cu);  2 = ONE REAL value (clean lattices,
+//   Anderson disorder, vacancies): the neighbours are summed and the sum scaled once -- 2 DADD per entry and state
+//   where the complex FMA takes 4 DFMA.
+// UNI: every row holds exactly max_row_off entries, a multiple of CH (periodic lattices): no row offsets, no predicates.
 // NW consumer warps + 1 producer warp form the only block of an SM: (NW + 1) * 32 threads share the 64 K registers.
-template <int BT, int SPT, int CH, int NACC, bool REDUCE, bool T2, int NW>
+template <int BT, int SPT, int CH, int NACC, bool REDUCE, int VK, bool UNI, int NW>
 __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p)
 {
     constexpr int kConsumers = NW * 32;
@@ -248,7 +258,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
             if (nc > 0) {
                 bulk_g2s(st + p.off_col, p.ocol + col_lo, nc * 4, full);
                 tx += nc * 4;
-                if (!T2) { bulk_g2s(st + p.off_idx, p.oidx + idx_lo, ni * 2, full); tx += ni * 2; }
+                if (VK == 0) { bulk_g2s(st + p.off_idx, p.oidx + idx_lo, ni * 2, full); tx += ni * 2; }
             }
             if (has_diag) {
                 const uint32_t db = (uint32_t)((rows * 8 + 15) & ~15);
@@ -256,14 +266,6 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
                 tx += db;
             }
             mbar_expect_tx(full, tx);                       // release: also publishes lo_s[s]
-            if (p.pol & 2) {                                // HBM -> L2 for the vector rows this tile will stream, n_stage tiles ahead
-                const uint32_t vb = (uint32_t)rows * BT * sizeof(double2);
-                const int64_t e0 = r0 * BT;
-                if (need_y) bulk_prefetch_l2(p.y + e0, vb);
-                if (need_acc) bulk_prefetch_l2(p.acc + e0, vb);
-                if (REDUCE) bulk_prefetch_l2(p.psi0 + e0, vb);
-                if (p.x_lead > 0 && r0 + p.x_lead + rows <= p.n_orb) bulk_prefetch_l2(p.x + (r0 + p.x_lead) * BT, vb);
-            }
             if (++s == S) { s = 0; ph ^= 1u; }
         }
         return;
@@ -273,13 +275,13 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     const int rl = tid / LPR;                               // row within the tile
     const int b0 = (tid % LPR) * SPT;                       // first state of this thread
     const double2 *xb = p.x + b0;
-    const int64_t pf_rows = p.pf_rows, pf_el = pf_rows * BT;
     const bool st_ef = p.pol & 1;                           // T_k leaves L2 first (its readers come a whole sweep later)
     const uint32_t stage_bytes = (uint32_t)p.stage_bytes;
+    const uint32_t n_uni = (uint32_t)p.max_row_off;         // UNI: every row holds exactly this many entries (a multiple of CH)
     const uint32_t a_orp = smem0 + (uint32_t)rl * 4u, a_col = smem0 + (uint32_t)p.off_col, a_idx = smem0 + (uint32_t)p.off_idx,
-                   a_diag = smem0 + (uint32_t)p.off_diag + (uint32_t)rl * 8u;
-    double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // T2: the (at most two) hopping values, in registers
-    if (T2) {
+                   a_diag = smem0 + (uint32_t)p.off_diag;
+    double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // VK >= 1: the (at most two) hopping values, in registers
+    if (VK >= 1) {
         t0 = __ldg(p.vtab);
         t1 = p.n_table > 1 ? __ldg(p.vtab + 1) : t0;
     }
@@ -313,19 +315,22 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
         if (NACC > 0) aold.stream_if(p.acc + e, valid && need_acc);
         if (REDUCE) z.stream_if(p.psi0 + e, valid);
         xrow.gather_if(p.x + e, valid && need_xrow);        // the tile's own x rows are gathered by its neighbours: L1/L2 hit
-        if (pf_rows > 0) {                                  // the same operands of this block's next tile: HBM -> L2 now
-            const bool on = row + pf_rows < p.n_orb;
-            prefetch_l2_if(p.y + e + pf_el, on && need_y);
-            if (NACC > 0) prefetch_l2_if(p.acc + e + pf_el, on && need_acc);
-            if (REDUCE) prefetch_l2_if(p.psi0 + e + pf_el, on);
-        }
         mbar_wait(bar0 + 8 * s, ph);
-        const uint32_t q0 = lds_u32(a_orp + so), q1 = lds_u32(a_orp + so + 4u);
-        n = valid ? q1 - q0 : 0u;
-        ca = a_col + so + (q0 - lo_s[s][0]) * 4u;
-        ia = a_idx + so + (q0 - lo_s[s][1]) * 2u;
-        d = has_diag ? lds_f64(a_diag + so) : 0.0;
-        nmax = __reduce_max_sync(0xffffffffu, n);
+        if (UNI) {                                          // rows past the end of the last tile redo its first row, unstored
+            const uint32_t rle = valid ? (uint32_t)rl : 0u;
+            const uint32_t q0 = (uint32_t)(tile * R) * n_uni;          // low 32 bits suffice for the offsets below
+            n = nmax = n_uni;
+            ca = a_col + so + (rle * n_uni + (q0 & 3u)) * 4u;
+            ia = a_idx + so + (rle * n_uni + (q0 & 7u)) * 2u;
+            d = has_diag ? lds_f64(a_diag + so + rle * 8u) : 0.0;
+        } else {
+            const uint32_t q0 = lds_u32(a_orp + so), q1 = lds_u32(a_orp + so + 4u);
+            n = valid ? q1 - q0 : 0u;
+            ca = a_col + so + (q0 - lo_s[s][0]) * 4u;
+            ia = a_idx + so + (q0 - lo_s[s][1]) * 2u;
+            d = has_diag ? lds_f64(a_diag + so + (uint32_t)rl * 8u) : 0.0;
+            nmax = __reduce_max_sync(0xffffffffu, n);
+        }
         c0 = 0;
         h.zero();
     };
@@ -333,8 +338,13 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
         uint32_t id[CH];
 #pragma unroll
         for (int j = 0; j < CH; ++j) {
-            w[j] = lds_u32_if(ca + 4u * (c0 + j), c0 + j < n);
-            id[j] = T2 ? 0u : lds_u16_if(ia + 2u * (c0 + j), c0 + j < n);
+            if (UNI) {
+                w[j] = lds_u32(ca + 4u * (c0 + j));
+                id[j] = VK == 0 ? lds_u16(ia + 2u * (c0 + j)) : 0u;
+            } else {
+                w[j] = lds_u32_if(ca + 4u * (c0 + j), c0 + j < n);
+                id[j] = VK == 0 ? lds_u16_if(ia + 2u * (c0 + j), c0 + j < n) : 0u;
+            }
         }
         if (c0 + CH >= nmax) {                              // last chunk of every row of this warp: the stage is free again
             __syncwarp();
@@ -342,16 +352,13 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
             if (++s == S) { s = 0; ph ^= 1u; so = 0; } else so += stage_bytes;
         }
 #pragma unroll
-        for (int j = 0; j < CH; ++j) x[j].gather_if(xb + (int64_t)(w[j] & 0x7fffffffu) * BT, c0 + j < n);
-        if (pf_rows > 0) {                                  // leading edge of the gather window (largest column), one tile ahead
-            uint32_t cmax = 0;
-#pragma unroll
-            for (int j = 0; j < CH; ++j) cmax = max(cmax, w[j] & 0x7fffffffu);
-            prefetch_l2_if(xb + ((int64_t)cmax + pf_rows) * BT, c0 < n && (int64_t)cmax + pf_rows < p.n_orb);
+        for (int j = 0; j < CH; ++j) {
+            const double2 *src = xb + (int64_t)(w[j] & 0x7fffffffu) * BT;
+            if (UNI) x[j].gather(src); else x[j].gather_if(src, c0 + j < n);
         }
-        if (!T2) {
+        if (VK == 0) {
 #pragma unroll
-            for (int j = 0; j < CH; ++j) v[j] = ldg_value_if(p.vtab + id[j], c0 + j < n);
+            for (int j = 0; j < CH; ++j) v[j] = ldg_value_if(p.vtab + id[j], UNI || c0 + j < n);
         }
     };
 
@@ -361,16 +368,28 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     }
 #pragma unroll 1
     while (tile < n_tiles) {
-        // ---- consume: complex FMAs of the chunk in flight, in issue order
+        // ---- consume the chunk in flight, in issue order
+        if (VK == 2) {                                      // one real hopping value: sum the neighbours, scale once per row
 #pragma unroll
-        for (int j = 0; j < CH; ++j) {
-            if (T2) v[j] = (w[j] >> 31) ? t1 : t0;
+            for (int j = 0; j < CH; ++j) {
 #pragma unroll
-            for (int k = 0; k < SPT; ++k) cfma(h.v[k], v[j], x[j].v[k]);   // x[j] is zero past the row end
+                for (int k = 0; k < SPT; ++k) { h.v[k].x += x[j].v[k].x; h.v[k].y += x[j].v[k].y; }   // x[j] is zero past the row end
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < CH; ++j) {
+                if (VK == 1) v[j] = (w[j] >> 31) ? t1 : t0;
+#pragma unroll
+                for (int k = 0; k < SPT; ++k) cfma(h.v[k], v[j], x[j].v[k]);
+            }
         }
         c0 += CH;
         if (c0 >= nmax) {
             // ---- epilogue of the row: diagonal, scale, subtract, store, accumulate, reduce
+            if (VK == 2) {
+#pragma unroll
+                for (int k = 0; k < SPT; ++k) { h.v[k].x *= t0.x; h.v[k].y *= t0.x; }
+            }
             if (has_diag) {
 #pragma unroll
                 for (int k = 0; k < SPT; ++k) { h.v[k].x = fma(d, xrow.v[k].x, h.v[k].x); h.v[k].y = fma(d, xrow.v[k].y, h.v[k].y); }
@@ -444,82 +463,72 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     }
 }
 
-template <int BT, int SPT, int CH, int NACC, bool REDUCE, bool T2, int NW>
+template <int BT, int SPT, int CH, int NACC, bool REDUCE, int VK, bool UNI, int NW>
 int launch_one(TermParams p, int num_sms, cudaStream_t st, int *grid_out)
 {
     constexpr int kConsumers = NW * 32, kThreads = kConsumers + 32;
     constexpr int R = kConsumers / (BT / SPT);
     p.n_stage = std::min(kMaxStages, std::max(2, env_int("TBPM_STAGES", 4)));
     p.chunk = std::max(1, env_int("TBPM_CHUNK", 1));
+    p.pol = env_int("TBPM_POL", 1);
     p.cap_entries = ((R * std::max(p.max_row_off, 1) + 8 + 7) / 8) * 8;          // + alignment slack of the slice start
     size_t o = (size_t)(((R + 1) * 4 + 15) & ~15);
     p.off_col = (int)o;  o += (size_t)p.cap_entries * 4;
-    p.off_idx = (int)o;  o += T2 ? 0 : (size_t)p.cap_entries * 2;
+    p.off_idx = (int)o;  o += VK == 0 ? (size_t)p.cap_entries * 2 : 0;
     o = (o + 15) & ~size_t(15);
     p.off_diag = (int)o; o += (size_t)((R * 8 + 15) & ~15);
     p.off_vec = 0;
     p.stage_bytes = (int)((o + 127) & ~size_t(127));
     p.n_stage = (int)std::max<size_t>(2, std::min<size_t>(p.n_stage, (size_t)160 * 1024 / p.stage_bytes));
     const size_t dyn = (size_t)p.stage_bytes * p.n_stage;
-    auto kern = k_term_ph<BT, SPT, CH, NACC, REDUCE, T2, NW>;
+    auto kern = k_term_ph<BT, SPT, CH, NACC, REDUCE, VK, UNI, NW>;
     static size_t configured = 0;
-    static int cached_nb = 0;
-    static size_t cached_dyn = 0;
     if (dyn > configured) {
         const size_t want = std::max(dyn, (size_t)64 * 1024);
         TBPM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)want));
         configured = want;
     }
-    if (cached_dyn != dyn || cached_nb == 0) {
-        int nb = 0;
-        TBPM_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, kThreads, dyn));
-        if (nb < 1) return TBPM_ENOMEM;
-        cached_nb = nb;
-        cached_dyn = dyn;
-    }
-    const int nb = std::min(cached_nb, std::max(1, env_int("TBPM_MAXB", 8)));
     const int64_t need = (p.n_orb + R - 1) / R;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>({need, (int64_t)num_sms * nb, (int64_t)kMaxGrid}));
-    p.pol = env_int("TBPM_POL", 1);
-    p.x_lead = env_int("TBPM_XLEAD", 0);
-    p.pf_rows = p.chunk == 1 ? (int64_t)env_int("TBPM_PF", 0) * grid * R : 0;      // prefetch distance: whole tiles of this block
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>({need, (int64_t)num_sms, (int64_t)kMaxGrid}));   // one block per SM
     kern<<<grid, kThreads, dyn, st>>>(p);
     count_launches(1);
     *grid_out = grid;
     return TBPM_OK;
 }
 
-template <int BT, int SPT, int CH, bool T2, int NW>
+template <int BT, int SPT, int CH, int VK, bool UNI, int NW>
 int launch_variant(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
     const bool red = p.flags & F_REDUCE;
-    if (!red && p.n_acc == 0) return launch_one<BT, SPT, CH, 0, false, T2, NW>(p, num_sms, st, grid_out);
-    if (!red && p.n_acc == 3) return launch_one<BT, SPT, CH, 3, false, T2, NW>(p, num_sms, st, grid_out);
-    if (red && p.n_acc == 1) return launch_one<BT, SPT, CH, 1, true, T2, NW>(p, num_sms, st, grid_out);
-    if (red && p.n_acc == 2) return launch_one<BT, SPT, CH, 2, true, T2, NW>(p, num_sms, st, grid_out);
-    if (red && p.n_acc == 3) return launch_one<BT, SPT, CH, 3, true, T2, NW>(p, num_sms, st, grid_out);
+    if (!red && p.n_acc == 0) return launch_one<BT, SPT, CH, 0, false, VK, UNI, NW>(p, num_sms, st, grid_out);
+    if (!red && p.n_acc == 3) return launch_one<BT, SPT, CH, 3, false, VK, UNI, NW>(p, num_sms, st, grid_out);
+    if (red && p.n_acc == 1) return launch_one<BT, SPT, CH, 1, true, VK, UNI, NW>(p, num_sms, st, grid_out);
+    if (red && p.n_acc == 2) return launch_one<BT, SPT, CH, 2, true, VK, UNI, NW>(p, num_sms, st, grid_out);
+    if (red && p.n_acc == 3) return launch_one<BT, SPT, CH, 3, true, VK, UNI, NW>(p, num_sms, st, grid_out);
     return TBPM_EINVAL;
 }
 
-// Shape of the instruction stream per (tile width, table kind, row length).  One block per SM; its (NW + 1) warps share
-// the register file: NW = 23 -> 80 registers per thread, NW = 15 -> 128.
-//   T2 (<= 2 hopping values in registers): CH = 8 gathers in flight on 15 warps, except single-state tiles with rows of
-//   <= 4 entries (CH = 4 on 23 warps); large tables (values fetched per entry, 4 more registers each): CH = 4 on 15 warps.
+// Shape of the instruction stream, chosen from what the builder found (table size, one real value, uniform rows) and
+// the tile width.  NW = 23 leaves 80 registers per thread, NW = 19 -> 96, NW = 15 -> 128.
 template <int BT>
 int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
     constexpr int SPT = BT >= 2 ? 2 : 1;
-    const bool t2 = p.packed != 0;
-    const int ch = env_int("TBPM_CH", (t2 && (BT >= 2 || p.max_row_off > 4)) ? 8 : 4);
-    if constexpr (BT == 8) if (env_int("TBPM_SPT", 2) == 1) {   // experiment: 128-bit gathers, one state per thread
-        if (t2) return launch_variant<BT, 1, 8, true, 23>(p, num_sms, st, grid_out);
-        return launch_variant<BT, 1, 8, false, 15>(p, num_sms, st, grid_out);
+    const int n = p.max_row_off;
+    const bool uni = p.uniform && env_int("TBPM_UNI", 1);
+    const int vk = (p.single_real && env_int("TBPM_VK2", 1)) ? 2 : (p.packed ? 1 : 0);
+    if (vk == 2) {
+        if (uni && n == 3) return launch_variant<BT, SPT, 3, 2, true, kNwA>(p, num_sms, st, grid_out);   // honeycomb
+        if (uni && n == 6) return launch_variant<BT, SPT, 6, 2, true, kNwB>(p, num_sms, st, grid_out);   // cubic
+        if (n <= 4) return launch_variant<BT, SPT, 4, 2, false, kNwA>(p, num_sms, st, grid_out);         // e.g. vacancies
+        return launch_variant<BT, SPT, 8, 2, false, 15>(p, num_sms, st, grid_out);
     }
-    if (t2) {
-        if (ch == 8) return launch_variant<BT, SPT, 8, true, 15>(p, num_sms, st, grid_out);
-        return launch_variant<BT, SPT, 4, true, 23>(p, num_sms, st, grid_out);
+    if (vk == 1) {
+        if (BT == 1 && n <= 4) return launch_variant<BT, SPT, 4, 1, false, 23>(p, num_sms, st, grid_out);
+        return launch_variant<BT, SPT, 8, 1, false, 15>(p, num_sms, st, grid_out);
     }
-    return launch_variant<BT, SPT, 4, false, 15>(p, num_sms, st, grid_out);
+    if (uni && n % 4 == 0) return launch_variant<BT, SPT, 4, 0, true, 15>(p, num_sms, st, grid_out);     // square + flux
+    return launch_variant<BT, SPT, 4, 0, false, 15>(p, num_sms, st, grid_out);
 }
 
 }  // namespace ph
