@@ -549,11 +549,12 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
         TRY_OR_FAIL(cudaStreamSynchronize(st));
         H->packed = pack;
         H->single_real = 0;
-        if (n_table == 1) {                                  // one real hopping value: kernels sum the neighbours, then scale
-            double2 v0;
-            TRY_OR_FAIL(cudaMemcpyAsync(&v0, H->vtab, sizeof(double2), cudaMemcpyDeviceToHost, st));
+        if (n_table <= 2) {   // one real hopping value t (its conjugate differs only in the sign of the zero): sum, then scale
+            double2 v01[2];
+            TRY_OR_FAIL(cudaMemcpyAsync(v01, H->vtab, sizeof(double2) * n_table, cudaMemcpyDeviceToHost, st));
             TRY_OR_FAIL(cudaStreamSynchronize(st));
-            H->single_real = (v0.y == 0.0);
+            if (n_table == 1) v01[1] = v01[0];
+            H->single_real = v01[0].y == 0.0 && v01[1].y == 0.0 && v01[0].x == v01[1].x;
         }
         H->n_table = hst[ST_NTAB];
     }

@@ -20,6 +20,7 @@
 //     second tiny kernel adds the block partials in a fixed order.  No floating-point atomics anywhere.
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <vector>
 
@@ -393,6 +394,11 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     tp.n_table = H->n_table;
     tp.packed = H->packed;
     tp.single_real = H->single_real;
+    tp.walk_stride = 0; tp.walk_run = 1;
+    if (const char *w = std::getenv("TBPM_WALK")) {          // "rows per lattice line,lines per run"
+        long long a = 0; int b = 1;
+        if (std::sscanf(w, "%lld,%d", &a, &b) >= 1) { tp.walk_stride = a; tp.walk_run = b; }
+    }
     tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
 

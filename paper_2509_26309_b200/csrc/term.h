@@ -41,7 +41,10 @@ struct TermParams {
     int packed;            // n_table <= 2: bit 31 of every ocol word is the value index (build.cu, k_pack_cols)
     // warp-specialised kernel: shared-memory stage geometry (bytes), filled by its launcher
     int n_stage, stage_bytes, cap_entries, off_col, off_idx, off_diag, off_vec;
-    int chunk;             // phased kernel: consecutive tiles per run of a block
+    int64_t walk_d0;       // phased kernel: tiles per lattice line (1: linear order)
+    int walk_len;          // phased kernel: tiles per run of a block
+    int64_t walk_stride;   // rows per lattice line (0: unknown)
+    int walk_run;          // lines per run when walk_stride is used
     int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
     int uniform;           // every row holds exactly max_row_off off-diagonal entries
     int single_real;       // the table holds one value and it is real

@@ -210,17 +210,25 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     }
     __syncthreads();
 
-    // Tile order of a block: runs of `chunk` consecutive tiles, runs dealt round-robin to the blocks.  All blocks together
-    // still sweep one moving window of the vectors (L2 locality), and inside a run the rows a block gathered for one tile
-    // (its lattice neighbours one line up) are the rows of its next tiles: they hit in its L1 instead of crossing the
-    // L2-to-SM fabric, which caps out near 6300 B/clk chip-wide (ncu: 79 % of it at chunk = 1, profiles/).
-    const int chunk = p.chunk;
-    const int64_t first_tile = (int64_t)blockIdx.x * chunk;
-    const int64_t run_skip = (int64_t)(gridDim.x - 1) * chunk + 1;
-    auto next_tile = [&](int64_t t, int &i) -> int64_t {
-        if (++i == chunk) { i = 0; return t + run_skip; }
-        return t + 1;
+    // Tile order of a block.  The tiles are viewed as a [line][d0] grid (d0 tiles per lattice line; d0 = 1: no lattice
+    // known) and dealt to the blocks in RUNS of `len` tiles that step one line at a time: run u covers the tiles
+    // ((u / d0) * len + i) * d0 + u % d0, i < len.  Inside a run the rows gathered for one tile (the neighbours one line
+    // up and down) are the rows of the run's previous and next tiles, so they are found in the SM's L1 instead of crossing
+    // the L2 fabric again; all blocks together still sweep one moving window of the vectors (L2 locality).
+    const int64_t d0 = p.walk_d0;
+    const int wlen = p.walk_len;
+    auto run_base = [&](int64_t u) -> int64_t {
+        const int64_t lb = u / d0;
+        const int64_t t = lb * wlen * d0 + (u - lb * d0);
+        return t < n_tiles ? t : n_tiles;                   // the base grows with u: the first one past the end ends the walk
     };
+    auto next_tile = [&](int64_t t, int &i, int64_t &u) -> int64_t {
+        if (++i < wlen) { t += d0; if (t < n_tiles) return t; }
+        i = 0;
+        u += gridDim.x;
+        return run_base(u);
+    };
+    const int64_t first_tile = run_base(blockIdx.x);
 
     if (tid >= kConsumers) {
         // ------------------------------------------------ producer warp ------------------------------------------------
@@ -233,11 +241,13 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
             q_hi = __ldg(p.orp + min(r0 + R, p.n_orb));
         }
         int s = 0, ci = 0;
+        int64_t cu = blockIdx.x;
         uint32_t ph = 1;                                    // parity of the "empty" phase to wait for; first pass: free
-        for (; tile < n_tiles; tile = next_tile(tile, ci)) {
+        for (; tile < n_tiles; tile = next_tile(tile, ci, cu)) {
             const uint32_t c_lo = q_lo, c_hi = q_hi;
             int cj = ci;
-            const int64_t nt = next_tile(tile, cj);
+            int64_t cv = cu;
+            const int64_t nt = next_tile(tile, cj, cv);
             if (nt < n_tiles) {                             // bounds of the following tile: latency hidden behind this issue
                 const int64_t nr0 = nt * R;
                 q_lo = __ldg(p.orp + nr0);
@@ -295,7 +305,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     // first complex FMA and serialises the memory round trips.
     int s = 0;
     uint32_t ph = 0, so = 0;                                // so: byte offset of stage s
-    int64_t tile = first_tile;
+    int64_t tile = first_tile, cu = blockIdx.x;
     int ci = 0;
     bool valid = false;
     int64_t e = 0;
@@ -425,7 +435,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
                     }
                 }
             }
-            tile = next_tile(tile, ci);
+            tile = next_tile(tile, ci, cu);
             if (tile >= n_tiles) break;
             load_row();
         }
@@ -469,7 +479,12 @@ int launch_one(TermParams p, int num_sms, cudaStream_t st, int *grid_out)
     constexpr int kConsumers = NW * 32, kThreads = kConsumers + 32;
     constexpr int R = kConsumers / (BT / SPT);
     p.n_stage = std::min(kMaxStages, std::max(2, env_int("TBPM_STAGES", 4)));
-    p.chunk = std::max(1, env_int("TBPM_CHUNK", 1));
+    p.walk_d0 = 1;
+    p.walk_len = std::max(1, env_int("TBPM_CHUNK", 1));
+    if (p.walk_stride > 0 && p.walk_stride % R == 0) {      // a lattice line is a whole number of tiles: walk across lines
+        p.walk_d0 = p.walk_stride / R;
+        p.walk_len = std::max(1, p.walk_run);
+    }
     p.pol = env_int("TBPM_POL", 1);
     p.cap_entries = ((R * std::max(p.max_row_off, 1) + 8 + 7) / 8) * 8;          // + alignment slack of the slice start
     size_t o = (size_t)(((R + 1) * 4 + 15) & ~15);
@@ -517,6 +532,10 @@ int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
     const int n = p.max_row_off;
     const bool uni = p.uniform && env_int("TBPM_UNI", 1);
     const int vk = (p.single_real && env_int("TBPM_VK2", 1)) ? 2 : (p.packed ? 1 : 0);
+    if (uni && p.walk_stride > 0 && p.walk_stride % (512 / (BT / SPT)) == 0) {   // 16 consumer warps: 2^k rows per tile
+        if (vk == 2 && n == 6) return launch_variant<BT, SPT, 6, 2, true, 16>(p, num_sms, st, grid_out);
+        if (vk == 0 && n % 4 == 0) return launch_variant<BT, SPT, 4, 0, true, 16>(p, num_sms, st, grid_out);
+    }
     if (vk == 2) {
         if (uni && n == 3) return launch_variant<BT, SPT, 3, 2, true, kNwA>(p, num_sms, st, grid_out);   // honeycomb
         if (uni && n == 6) return launch_variant<BT, SPT, 6, 2, true, kNwB>(p, num_sms, st, grid_out);   // cubic
