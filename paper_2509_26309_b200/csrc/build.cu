@@ -558,6 +558,22 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
         }
         H->n_table = hst[ST_NTAB];
     }
+    // Lattice strides: on a matrix whose rows all have the same length, the column offsets of one row in the middle are
+    // the strides of the lattice (1, a line, a plane); propagate walks its tiles along the largest usable one.
+    {
+        const int n_off = H->max_row_nnz - (has_onsite ? 1 : 0);
+        if (n_orb > 0 && H->min_row_nnz == H->max_row_nnz && n_off > 0 && n_off <= 16) {
+            const int64_t mid = n_orb / 2;
+            int32_t cw[16];
+            TRY_OR_FAIL(cudaMemcpyAsync(cw, H->ocol + mid * n_off, sizeof(int32_t) * n_off, cudaMemcpyDeviceToHost, st));
+            TRY_OR_FAIL(cudaStreamSynchronize(st));
+            for (int j = 0; j < n_off; ++j) {
+                const int64_t c = cw[j] & 0x7fffffff;
+                H->lat_off[H->n_lat_off++] = c > mid ? c - mid : mid - c;
+            }
+            std::sort(H->lat_off, H->lat_off + H->n_lat_off);
+        }
+    }
 #undef TRY_OR_FAIL
     *out = H;
     return TBPM_OK;

@@ -395,6 +395,8 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     tp.packed = H->packed;
     tp.single_real = H->single_real;
     tp.walk_stride = 0; tp.walk_run = 1;
+    tp.n_lat_off = H->n_lat_off;
+    for (int j = 0; j < H->n_lat_off; ++j) tp.lat_off[j] = H->lat_off[j];
     if (const char *w = std::getenv("TBPM_WALK")) {          // "rows per lattice line,lines per run"
         long long a = 0; int b = 1;
         if (std::sscanf(w, "%lld,%d", &a, &b) >= 1) { tp.walk_stride = a; tp.walk_run = b; }

@@ -52,6 +52,8 @@ struct tbpm_ham {
     int32_t max_row_nnz = 0;
     int32_t min_row_nnz = 0;
     int32_t single_real = 0;   // the table holds one value and it is real
+    int32_t n_lat_off = 0;     // uniform rows: |col - row| of the entries of one sample row (lattice strides), ascending
+    int64_t lat_off[16] = {0};
     double gershgorin = 0.0;
     int32_t n_table = 0;   // 0: kernels read complex128 values from the canonical CSR
     int32_t packed = 0;    // n_table <= 2: bit 31 of every ocol word holds the value index (oidx is not read by the kernels)

@@ -45,6 +45,8 @@ struct TermParams {
     int walk_len;          // phased kernel: tiles per run of a block
     int64_t walk_stride;   // rows per lattice line (0: unknown)
     int walk_run;          // lines per run when walk_stride is used
+    int n_lat_off;         // lattice strides found by the builder (uniform rows only), ascending
+    int64_t lat_off[16];
     int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
     int uniform;           // every row holds exactly max_row_off off-diagonal entries
     int single_real;       // the table holds one value and it is real
