@@ -58,6 +58,24 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused term, MB, from the one `ncu --set full` capture per
+# workload summarised in profiles/r1b_ncu_full_cfg2-5.md: (first term k=1, first flush k=2, plain term, flush, last term).
+NCU_TRAFFIC_SRC = "profiles/r1b_ncu_full_cfg2-5.md (ncu --set full, one capture per workload; average over the launches of a time step)"
+NCU_TRAFFIC_MB = {"cfg2": (279.2, 531.7, 414.6, 668.7, 694.5), "cfg3": (1384.0, 2330.0, 1868.0, 2815.0, 2839.0),
+                  "cfg4": (5137.0, 9412.0, 7284.0, 11560.0, 11584.0), "cfg5": (5002.0, 9322.0, 7152.0, 11646.0, 12547.0)}
+
+
+def ncu_traffic(workload_name: str, K: int):
+    """Average DRAM bytes per term launch over one time step (K-1 launches: flush every third term), or None."""
+    t = NCU_TRAFFIC_MB.get(workload_name.split(":")[0])
+    if t is None or K < 4:
+        return None
+    first, first_flush, plain, flush, last = t
+    n_flush = len([k for k in range(3, K - 1) if k % 3 == 2])
+    n_plain = (K - 1) - 3 - n_flush
+    return 1e6 * (first + first_flush + last + n_flush * flush + n_plain * plain) / (K - 1)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -254,8 +272,9 @@ def main_ours(args):
     bytes_per_launch = H.matrix_bytes_per_term + 3 * 16 * w.n_orb * min(tile, n_state)
     peak, peak_src = load_peaks()
     achieved = bytes_per_launch / avg_term_s / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_cheb_term", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
+    roofline = {"bound": "hbm", "kernel": "k_term_ph (fused Chebyshev term, term_ph.cuh)", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(w.name, K), "traffic_source": NCU_TRAFFIC_SRC,
+                "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
                 "avg_launch_us": avg_term_s * 1e6, "launches_per_step": term_launches,
                 "counted_csr_gbs": (8 * (w.n_orb + 1) + 20 * nnz + 48 * w.n_orb * min(tile, n_state)) / avg_term_s / 1e9,
                 "frac_of_nominal_8000": achieved / 8000.0,

@@ -4,7 +4,7 @@
 //   T_k = a*H*T_{k-1} - T_{k-2}  (amxsy)  fused with  psi' += sum c_j T_j  (axpy, up to
 //   three terms at once) and, on the last term of a time step, <psi0|psi'> and <psi'|psi'> (calc_corr_dos).
 //
-// Why this shape (profiles/r1_ncu_full_cfg4_cfg5.md): with 8 interleaved states per row the previous kernel (term_ws.cu)
+// Why this shape (profiles/r1b_ncu_full_cfg2-5.md): with 8 interleaved states per row the previous kernel (term_ws.cu)
 // was bound in the SM clock domain -- by L1 data-pipe wavefronts (16-25 per row where the gathers and the store need
 // 8-10) and by three to four serialised memory round trips per row (a warp pass took ~4800 cycles).  Here
 //   producer warp (one elected lane): for every tile of R rows, n_stage tiles ahead, bulk-copies (cp.async.bulk +

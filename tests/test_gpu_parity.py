@@ -164,6 +164,7 @@ def test_config1_full_length(dev, oracle_mod):
     (4, dict(Lx=32, Ly=24, phi_den=8), 5, 6),                        # 5 states -> padded tile of 8
     (5, dict(L=17), 32, 12),                                         # 4 tiles of 8
     (5, dict(L=12), 11, 5),                                          # tile of 8 + padded tile of 4
+    (5, dict(L=32), 8, 6),                                           # plane stride 1024 = 8 tiles: the builder's lattice walk
 ])
 @pytest.mark.parametrize("flags", [0, tbpm.TBPM_NO_TABLE])
 def test_small_configs_every_element(dev, oracle_mod, cfg, over, n_state, n_step, flags):
