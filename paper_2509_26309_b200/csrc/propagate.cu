@@ -404,6 +404,7 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
 
+    const int rev_mode = env_int("TBPM_REV", 1);   // odd terms sweep backwards (term_ph.cuh)
     for (int t = 0; t < P.n_tile; ++t) {
         const int state0 = t * P.tile;
         const int n_valid = std::min(P.tile, n_state - state0);
@@ -455,6 +456,7 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
                 }
                 if (last) { flags |= F_REDUCE; flags &= ~F_WRITE_Y; }   // T_{K-1} is never read again
                 tp.flags = flags;
+                tp.reverse = rev_mode ? (k & 1) : 0;
                 if ((rc = launch_term(bt, table, tp, H->num_sms, st, &grid))) return rc;
             }
             k_reduce_final<<<bt, 96, 0, st>>>(partial, grid, bt, n_valid, state0, n_step, n, corr, norm2);

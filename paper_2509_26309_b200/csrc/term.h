@@ -48,6 +48,7 @@ struct TermParams {
     int n_lat_off;         // lattice strides found by the builder (uniform rows only), ascending
     int64_t lat_off[16];
     int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
+    int reverse;           // phased kernel: sweep the tiles from the last row block to the first
     int uniform;           // every row holds exactly max_row_off off-diagonal entries
     int single_real;       // the table holds one value and it is real
 };

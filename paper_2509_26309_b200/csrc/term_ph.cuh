@@ -229,6 +229,10 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
         return run_base(u);
     };
     const int64_t first_tile = run_base(blockIdx.x);
+    // Every other term sweeps the rows from the end: what the previous term wrote and gathered last is still in L2 when this
+    // term starts there (worth 20-25 % of the DRAM reads when the vectors are a few times the L2, nothing when far larger).
+    const bool rev = p.reverse != 0;
+    auto tile_rows = [&](int64_t t) -> int64_t { return (rev ? n_tiles - 1 - t : t) * R; };
 
     if (tid >= kConsumers) {
         // ------------------------------------------------ producer warp ------------------------------------------------
@@ -236,7 +240,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
         uint32_t q_lo = 0, q_hi = 0;                        // offsets bounding the next tile to issue (prefetched)
         int64_t tile = first_tile;
         if (tile < n_tiles) {
-            const int64_t r0 = tile * R;
+            const int64_t r0 = tile_rows(tile);
             q_lo = __ldg(p.orp + r0);
             q_hi = __ldg(p.orp + min(r0 + R, p.n_orb));
         }
@@ -249,14 +253,14 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
             int64_t cv = cu;
             const int64_t nt = next_tile(tile, cj, cv);
             if (nt < n_tiles) {                             // bounds of the following tile: latency hidden behind this issue
-                const int64_t nr0 = nt * R;
+                const int64_t nr0 = tile_rows(nt);
                 q_lo = __ldg(p.orp + nr0);
                 q_hi = __ldg(p.orp + min(nr0 + R, p.n_orb));
             }
             const uint32_t full = bar0 + 8 * s;
             mbar_wait(bar0 + 8 * (kMaxStages + s), ph);     // a fresh barrier reports the "previous" phase complete
             const uint32_t st = smem0 + (uint32_t)s * (uint32_t)p.stage_bytes;
-            const int64_t r0 = tile * R;
+            const int64_t r0 = tile_rows(tile);
             const int rows = (int)min((int64_t)R, p.n_orb - r0);
             const uint32_t col_lo = c_lo & ~3u, idx_lo = c_lo & ~7u;
             const uint32_t nc = ((c_hi - col_lo) + 3u) & ~3u, ni = ((c_hi - idx_lo) + 7u) & ~7u;
@@ -317,7 +321,8 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     uint32_t w[CH];
 
     auto load_row = [&]() {                                 // streamed operands + row header of `tile`
-        const int64_t row = tile * R + rl;
+        const int64_t trow = tile_rows(tile);
+        const int64_t row = trow + rl;
         valid = row < p.n_orb;
         e = row * BT + b0;
         // streamed operands of the row (HBM latency; they need no index, so they leave before the wait)
@@ -328,7 +333,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
         mbar_wait(bar0 + 8 * s, ph);
         if (UNI) {                                          // rows past the end of the last tile redo its first row, unstored
             const uint32_t rle = valid ? (uint32_t)rl : 0u;
-            const uint32_t q0 = (uint32_t)(tile * R) * n_uni;          // low 32 bits suffice for the offsets below
+            const uint32_t q0 = (uint32_t)trow * n_uni;                // low 32 bits suffice for the offsets below
             n = nmax = n_uni;
             ca = a_col + so + (rle * n_uni + (q0 & 3u)) * 4u;
             ia = a_idx + so + (rle * n_uni + (q0 & 7u)) * 2u;
