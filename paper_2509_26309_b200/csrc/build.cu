@@ -247,7 +247,7 @@ __global__ void k_sort_rows(int64_t n_orb, const int64_t *__restrict__ rowptr, i
 // 5. kernel layout: off-diagonal columns in a separate array (they are packed with the value index later, so they never
 //    alias the canonical CSR).  has_onsite: every row holds exactly one diagonal entry -> off-diagonal offset = rowptr[r] - r.
 __global__ void k_strip(int64_t n_orb, int has_onsite, const int64_t *__restrict__ rowptr, const int32_t *__restrict__ col,
-                        const double2 *__restrict__ val, uint32_t *orp, int32_t *ocol, double *diag)
+                        const double2 *__restrict__ val, uint32_t *orp, int32_t *ocol, double *diag, int32_t *status)
 {
     int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r > n_orb) return;
@@ -256,11 +256,16 @@ __global__ void k_strip(int64_t n_orb, int has_onsite, const int64_t *__restrict
     orp[r] = (uint32_t)ob;
     if (r == n_orb) return;
     int64_t e = rowptr[r + 1];
+    int32_t halo = 0;                                       // widest |col - row|, taken round the periodic boundary
     for (int64_t p = b; p < e; ++p) {
         int32_t c = col[p];
         if (has_onsite && c == (int32_t)r) diag[r] = val[p].x;
         else ocol[ob++] = c;
+        int64_t dd = c > r ? c - r : r - c;
+        dd = min(dd, n_orb - dd);
+        halo = max(halo, (int32_t)dd);
     }
+    if (halo > *(volatile int32_t *)&status[ST_HALO]) atomicMax(&status[ST_HALO], halo);   // read first: few distinct values
 }
 
 // 6. distinct-value table
@@ -513,7 +518,7 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
         k_fill<<<gh, kThreads, 0, st>>>(n_hop, hop_i, hop_j, reinterpret_cast<const double2 *>(hop_val), n_orb, full, H->rowptr,
                                         cur, H->col, H->val, H->status);
     if (n_orb > 0) k_sort_rows<<<gr, kThreads, 0, st>>>(n_orb, H->rowptr, H->col, H->val, H->status);
-    k_strip<<<gr, kThreads, 0, st>>>(n_orb, has_onsite, H->rowptr, H->col, H->val, H->orp, H->ocol, H->diag);
+    k_strip<<<gr, kThreads, 0, st>>>(n_orb, has_onsite, H->rowptr, H->col, H->val, H->orp, H->ocol, H->diag, H->status);
     const bool want_table = !(flags & TBPM_NO_TABLE) && H->nnz_off > 0;
     if (want_table) {
         TRY_OR_FAIL(cudaMemsetAsync(slots, 0xFF, sizeof(uint32_t) * kHashSlots, st));
@@ -529,6 +534,7 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
     if (hst[ST_ERR] & 2) return fail(TBPM_EDIAG);
     if (hst[ST_ERR] & 4) return fail(TBPM_EDUP);
     H->max_row_nnz = hst[ST_MAX_ROW];
+    H->halo_rows = hst[ST_HALO];
     H->min_row_nnz = n_orb > 0 ? (1 << 30) - hst[ST_NEG_MIN_ROW] : 0;
     uint64_t gb = (uint64_t)(uint32_t)hst[ST_GERSH_LO] | ((uint64_t)(uint32_t)hst[ST_GERSH_HI] << 32);
     std::memcpy(&H->gershgorin, &gb, sizeof(double));

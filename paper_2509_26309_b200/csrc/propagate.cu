@@ -404,6 +404,9 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
 
+    bool fused_any = false;
+    int *pair_progress = reinterpret_cast<int *>(reinterpret_cast<char *>(partial) + kPartialBytes - 4 * sizeof(int) * kMaxGrid);   // [0,G): counters; [kMaxGrid]: error; [2 kMaxGrid, ..): per-warp scratch
+    TBPM_CUDA_TRY(cudaMemsetAsync(pair_progress + kMaxGrid, 0, sizeof(int), st));
     const int rev_mode = env_int("TBPM_REV", 1);   // odd terms sweep backwards (term_ph.cuh)
     for (int t = 0; t < P.n_tile; ++t) {
         const int state0 = t * P.tile;
@@ -427,6 +430,19 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
             ++g_launches; count_launches(1);
         }
         tp.psi0 = bra;
+        // Two terms per sweep when the gather halo and the lag between the two phases fit the L2 (see term_pair.cuh)
+        bool fuse = false;
+        {
+            const int fm = env_int("TBPM_FUSE", 0);       // 0: off, 1: when it pays, 2: always (tests)
+            TermParams probe = tp;
+            probe.flags = F_WRITE_Y; probe.n_acc = 0;
+            if (fm > 0 && table && (bt == 2 || bt == 4 || bt == 8) && term_ph_supported(bt, probe)) {
+                const int64_t tile_rows = 15 * 32 / (bt / 2);
+                const int64_t window = 3 * (int64_t)H->halo_rows + 2 * (int64_t)H->num_sms * tile_rows;      // rows alive in L2
+                const double mb = (double)window * bt * 16.0 * 2.0 / 1e6;
+                fuse = fm == 2 || (mb <= env_int("TBPM_FUSE_MB", 80) && H->n_orb >= 8 * window);
+            }
+        }
         int slot = start_slot;
         for (int n = 0; n < n_step; ++n) {
             double2 *psi = buf[slot], *t1 = buf[(slot + 1) % 3], *acc = buf[(slot + 2) % 3];
@@ -437,6 +453,7 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
                 if ((rc = launch_term(bt, table, tp, H->num_sms, st, &grid))) return rc;
             }
             int flushed = -1;                             // highest term already added to psi'
+            std::vector<TermParams> term((size_t)K);      // term[k]: launch parameters of Chebyshev term k of this step
             for (int k = 1; k < K; ++k) {
                 // buffers: T_k overwrites T_{k-2}; T_0 = psi, T_1 = t1, T_2 -> psi's buffer, ...
                 tp.x = (k % 2 == 1) ? psi : t1;           // T_{k-1}
@@ -456,8 +473,35 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
                 }
                 if (last) { flags |= F_REDUCE; flags &= ~F_WRITE_Y; }   // T_{K-1} is never read again
                 tp.flags = flags;
-                tp.reverse = rev_mode ? (k & 1) : 0;
-                if ((rc = launch_term(bt, table, tp, H->num_sms, st, &grid))) return rc;
+                tp.reverse = 0;
+                term[k] = tp;
+            }
+            for (int k = 1; k < K;) {
+                if (fuse && k + 1 < K) {                  // two terms in one sweep (term_pair.cuh)
+                    PairParams pp{};
+                    pp.t = term[k];
+                    for (int f = 0; f < 2; ++f) {
+                        const TermParams &s = term[k + f];
+                        pp.ph[f] = PhaseParams{s.x, s.y, s.a, s.ca, s.cb, s.cc, (s.flags & F_SUB_Y) ? 1 : 0, s.n_acc,
+                                               (s.flags & F_ACC_INIT) ? 1 : 0, (s.flags & F_REDUCE) ? 1 : 0};
+                    }
+                    pp.halo = H->halo_rows;
+                    pp.progress = pair_progress;
+                    pp.error = pair_progress + kMaxGrid;
+                    ++g_launches;
+                    switch (bt) {
+                    case 2: rc = launch_term_pair_bt2(pp, H->num_sms, st, &grid); break;
+                    case 4: rc = launch_term_pair_bt4(pp, H->num_sms, st, &grid); break;
+                    default: rc = launch_term_pair_bt8(pp, H->num_sms, st, &grid); break;
+                    }
+                    if (rc) return rc;
+                    fused_any = true;
+                    k += 2;
+                } else {
+                    term[k].reverse = (rev_mode && !fuse) ? (k & 1) : 0;
+                    if ((rc = launch_term(bt, table, term[k], H->num_sms, st, &grid))) return rc;
+                    k += 1;
+                }
             }
             k_reduce_final<<<bt, 96, 0, st>>>(partial, grid, bt, n_valid, state0, n_step, n, corr, norm2);
             ++g_launches; count_launches(1);
@@ -465,6 +509,12 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
         }
     }
     TBPM_CUDA_TRY(cudaGetLastError());
+    if (fused_any) {                                      // a dependency wait that gave up means the blocks were not co-resident
+        int err = 0;
+        TBPM_CUDA_TRY(cudaMemcpyAsync(&err, pair_progress + kMaxGrid, sizeof(int), cudaMemcpyDeviceToHost, st));
+        TBPM_CUDA_TRY(cudaStreamSynchronize(st));
+        if (err) return TBPM_ECUDA;
+    }
     return TBPM_OK;
 }
 

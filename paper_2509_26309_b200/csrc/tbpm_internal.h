@@ -36,7 +36,8 @@ enum StatusWord {
     ST_GERSH_HI = 3,
     ST_NTAB = 4,         // number of distinct off-diagonal values inserted into the hash table
     ST_TAB_OVERFLOW = 5, // more than kTableMax distinct values (or a probe sequence gave up)
-    ST_NEG_MIN_ROW = 6   // 2^30 - (fewest entries in a row of the canonical CSR)
+    ST_NEG_MIN_ROW = 6,  // 2^30 - (fewest entries in a row of the canonical CSR)
+    ST_HALO = 7          // widest |col - row| (circular): how far a row reaches into the vector
 };
 
 }  // namespace tbpm_detail
@@ -52,6 +53,7 @@ struct tbpm_ham {
     int32_t max_row_nnz = 0;
     int32_t min_row_nnz = 0;
     int32_t single_real = 0;   // the table holds one value and it is real
+    int32_t halo_rows = 0;     // widest circular |col - row|
     int32_t n_lat_off = 0;     // uniform rows: |col - row| of the entries of one sample row (lattice strides), ascending
     int64_t lat_off[16] = {0};
     double gershgorin = 0.0;

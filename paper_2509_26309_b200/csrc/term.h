@@ -53,6 +53,26 @@ struct TermParams {
     int single_real;       // the table holds one value and it is real
 };
 
+// Two consecutive Chebyshev terms in ONE sweep (term_pair.cuh).  Phase 0 is term k (x = T_{k-1}, y = T_{k-2} -> T_k), phase 1 is
+// term k+1 (x = T_k, y = T_{k-1} -> T_{k+1}); phase 1 of a tile runs a few hundred tiles behind phase 0, while T_k, T_{k-1} and the
+// matrix slices are still in L2, so the pair moves matrix + 4 vectors through DRAM where two launches move 2 x (matrix + 3).
+struct PhaseParams {
+    const double2 *x;
+    double2 *y;
+    double a;
+    double2 ca, cb, cc;
+    int sub_y, n_acc, acc_init, reduce;
+};
+
+struct PairParams {
+    TermParams t;          // matrix, n_orb, acc, psi0, partial, table / row-shape facts, stage geometry
+    PhaseParams ph[2];
+    int64_t halo;          // tiles: phase 1 of tile t needs phase 0 of every tile within +-halo (circular)
+    int lag;               // steps of a block's sequence between phase 0 and phase 1 of its tiles
+    int *progress;         // [grid] phase-0 tiles finished by each block (zeroed before the launch)
+    int *error;            // set when a dependency wait gave up (never, unless the blocks are not co-resident)
+};
+
 __device__ __forceinline__ void cfma(double2 &h, double2 v, double2 x)   // h += v * x (complex)
 {
     h.x = fma(v.x, x.x, h.x);
@@ -78,5 +98,10 @@ int launch_term_ph_bt1(const TermParams &p, int num_sms, cudaStream_t st, int *g
 int launch_term_ph_bt2(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 int launch_term_ph_bt4(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 int launch_term_ph_bt8(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
+
+// Pair kernel, one file per tile width (2, 4, 8 states).
+int launch_term_pair_bt2(const PairParams &p, int num_sms, cudaStream_t st, int *grid_out);
+int launch_term_pair_bt4(const PairParams &p, int num_sms, cudaStream_t st, int *grid_out);
+int launch_term_pair_bt8(const PairParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
 }  // namespace tbpm_detail

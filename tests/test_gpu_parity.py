@@ -172,6 +172,19 @@ def test_small_configs_every_element(dev, oracle_mod, cfg, over, n_state, n_step
     run_parity(dev, oracle_mod, w, n_state, n_step, flags)
 
 
+@pytest.mark.parametrize("cfg,over,n_state,n_step", [
+    (2, dict(Na=96, Nb=70), 4, 12),                                  # honeycomb shape, tile of 4
+    (4, dict(Lx=64, Ly=48, phi_den=32), 8, 10),                      # table shape, two chunks per row
+    (5, dict(L=17), 16, 9),                                          # cubic shape, odd number of terms' worth of flushes
+    (3, dict(Na=100, Nb=60), 2, 7),                                  # irregular rows, tile of 2
+])
+def test_two_terms_per_sweep(dev, oracle_mod, cfg, over, n_state, n_step, monkeypatch):
+    """term_pair.cuh (experimental, TBPM_FUSE): phase 1 of a tile waits for phase 0 of its halo; same 1e-10 bar."""
+    monkeypatch.setenv("TBPM_FUSE", "2")
+    w = W.make_workload(cfg, device=dev, **over)
+    run_parity(dev, oracle_mod, w, n_state, n_step)
+
+
 @pytest.mark.parametrize("tile", ["1", "2", "4", "16", "32"])
 def test_other_tile_widths(dev, oracle_mod, tile, monkeypatch):
     monkeypatch.setenv("TBPM_TILE", tile)
