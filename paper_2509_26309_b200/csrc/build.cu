@@ -15,7 +15,8 @@
 //   4. one thread per row: insertion sort by column, duplicate check, Gershgorin row sum, max row length   k_sort_rows
 //   5. kernel layout: off-diagonal CSR with 32-bit row offsets + real diagonal                     k_strip
 //   6. table of distinct off-diagonal values (open-addressing hash on the 128-bit pattern), numbered by first use in
-//      (entry-within-row, row) order; 16-bit index per entry, or -- tables of <= 2 values -- bit 31 of the column word
+//      (entry-within-row, row) order, v and conj(v) sharing an entry; 15-bit index + conjugate bit per entry, or -- a
+//      table of one value -- only the conjugate bit, in bit 31 of the column word
 //      k_tab_insert / scan / k_tab_key / k_tab_compact / k_tab_rank / k_tab_number / k_tab_lookup
 //      ("hopping-table index for uniform lattices", north_star)
 #include <algorithm>
@@ -275,13 +276,18 @@ __device__ __forceinline__ uint64_t mix64(uint64_t z)
     z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
     return z ^ (z >> 31);
 }
+// The table holds every value ONCE for v and conj(v): the key is (re, |im|) as bit patterns, and the sign bit of im travels
+// with the entry (bit 15 of the 16-bit index, or bit 31 of a packed column word).  H is Hermitian, so this halves the table
+// (cfg4: 15,728 -> 7,865 values, 126 KB: it stays in L1) and makes a real hopping value a table of one.
+constexpr unsigned long long kSignBit = 0x8000000000000000ull;
 __device__ __forceinline__ bool same_bits(double2 a, double2 b)
 {
-    return __double_as_longlong(a.x) == __double_as_longlong(b.x) && __double_as_longlong(a.y) == __double_as_longlong(b.y);
+    return __double_as_longlong(a.x) == __double_as_longlong(b.x) &&
+           ((unsigned long long)__double_as_longlong(a.y) & ~kSignBit) == ((unsigned long long)__double_as_longlong(b.y) & ~kSignBit);
 }
 __device__ __forceinline__ uint32_t slot_of(double2 v)
 {
-    return (uint32_t)(mix64((uint64_t)__double_as_longlong(v.x) ^ mix64((uint64_t)__double_as_longlong(v.y) + 0x9E3779B97F4A7C15ull))) &
+    return (uint32_t)(mix64((uint64_t)__double_as_longlong(v.x) ^ mix64(((uint64_t)__double_as_longlong(v.y) & ~kSignBit) + 0x9E3779B97F4A7C15ull))) &
            (kHashSlots - 1);
 }
 
@@ -363,10 +369,14 @@ __global__ void k_tab_number(const uint32_t *__restrict__ slots, const int64_t *
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= kHashSlots) return;
     uint32_t s = slots[i];
-    if (s != kEmpty && slot_id[i] < kTableMax) vtab[rank[slot_id[i]]] = val[s];
+    if (s != kEmpty && slot_id[i] < kTableMax) {
+        double2 v = val[s];
+        v.y = __longlong_as_double((long long)((unsigned long long)__double_as_longlong(v.y) & ~kSignBit));   // canonical: im >= +0
+        vtab[rank[slot_id[i]]] = v;
+    }
 }
 
-// oidx[q] = table index of off-diagonal entry q; pack: additionally bit 31 of ocol[q] (tables of <= 2 values)
+// oidx[q] = table index of off-diagonal entry q, bit 15 = conjugate; pack (table of ONE value): the same flag in bit 31 of ocol[q]
 __global__ void k_tab_lookup(int64_t n_orb, int has_onsite, const int64_t *__restrict__ rowptr, const int32_t *__restrict__ col,
                              const double2 *__restrict__ val, const uint32_t *__restrict__ slots, const int64_t *__restrict__ slot_id,
                              const int32_t *__restrict__ rank, int pack, uint16_t *oidx, int32_t *ocol)
@@ -379,9 +389,9 @@ __global__ void k_tab_lookup(int64_t n_orb, int has_onsite, const int64_t *__res
         double2 v = val[p];
         uint32_t h = slot_of(v);
         while (!same_bits(val[slots[h]], v)) h = (h + 1) & (kHashSlots - 1);
-        const int32_t id = rank[slot_id[h]];
-        oidx[q] = (uint16_t)id;
-        if (pack) ocol[q] = (int32_t)((uint32_t)ocol[q] | ((uint32_t)id << 31));
+        const uint32_t cj = (uint32_t)((unsigned long long)__double_as_longlong(v.y) >> 63);   // 1: this entry is conj(table value)
+        oidx[q] = (uint16_t)((uint32_t)rank[slot_id[h]] | (cj << 15));
+        if (pack) ocol[q] = (int32_t)((uint32_t)ocol[q] | (cj << 31));
         ++q;
     }
 }
@@ -543,7 +553,7 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
         k_tab_flags<<<blocks_for(kHashSlots + 1, kThreads), kThreads, 0, st>>>(slots, flag);
         if ((rc = scan_exclusive(flag, kHashSlots + 1, slot_id, bsum, st)) != TBPM_OK) return fail(rc);
         const int n_table = hst[ST_NTAB];
-        const int pack = n_table <= 2;
+        const int pack = n_table == 1;
         TRY_OR_FAIL(cudaMemsetAsync(keys, 0xFF, sizeof(unsigned long long) * kHashSlots, st));
         k_tab_key<<<gr, kThreads, 0, st>>>(n_orb, has_onsite, H->rowptr, H->col, H->val, slots, keys);
         k_tab_compact<<<blocks_for(kHashSlots, kThreads), kThreads, 0, st>>>(slots, slot_id, keys, ckeys);
@@ -555,12 +565,11 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
         TRY_OR_FAIL(cudaStreamSynchronize(st));
         H->packed = pack;
         H->single_real = 0;
-        if (n_table <= 2) {   // one real hopping value t (its conjugate differs only in the sign of the zero): sum, then scale
-            double2 v01[2];
-            TRY_OR_FAIL(cudaMemcpyAsync(v01, H->vtab, sizeof(double2) * n_table, cudaMemcpyDeviceToHost, st));
+        if (n_table == 1) {   // one hopping value; if it is real the kernels sum the neighbours and scale once
+            double2 v0;
+            TRY_OR_FAIL(cudaMemcpyAsync(&v0, H->vtab, sizeof(double2), cudaMemcpyDeviceToHost, st));
             TRY_OR_FAIL(cudaStreamSynchronize(st));
-            if (n_table == 1) v01[1] = v01[0];
-            H->single_real = v01[0].y == 0.0 && v01[1].y == 0.0 && v01[0].x == v01[1].x;
+            H->single_real = v0.y == 0.0;
         }
         H->n_table = hst[ST_NTAB];
     }

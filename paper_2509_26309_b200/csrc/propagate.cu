@@ -103,10 +103,10 @@ __global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p
                     if (p1) { c1 = __ldg(p.ocol + q + 1) & 0x7fffffff; i1 = __ldg(p.oidx + q + 1); }
                     if (p2) { c2 = __ldg(p.ocol + q + 2) & 0x7fffffff; i2 = __ldg(p.oidx + q + 2); }
                     if (p3) { c3 = __ldg(p.ocol + q + 3) & 0x7fffffff; i3 = __ldg(p.oidx + q + 3); }
-                    v0 = __ldg(p.vtab + i0);
-                    if (p1) v1 = __ldg(p.vtab + i1);
-                    if (p2) v2 = __ldg(p.vtab + i2);
-                    if (p3) v3 = __ldg(p.vtab + i3);
+                    v0 = table_value(__ldg(p.vtab + (i0 & 0x7fffu)), i0);
+                    if (p1) v1 = table_value(__ldg(p.vtab + (i1 & 0x7fffu)), i1);
+                    if (p2) v2 = table_value(__ldg(p.vtab + (i2 & 0x7fffu)), i2);
+                    if (p3) v3 = table_value(__ldg(p.vtab + (i3 & 0x7fffu)), i3);
                 } else {
                     c0 = __ldg(p.col + q); v0 = __ldg(p.val + q);
                     if (p1) { c1 = __ldg(p.col + q + 1); v1 = __ldg(p.val + q + 1); }

@@ -24,7 +24,7 @@ void count_launches(int n);   // process-wide kernel-launch counter (tbpm_total_
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a; }
 
-constexpr int kTableMax = 65536;        // distinct hopping values addressable by a 16-bit index
+constexpr int kTableMax = 32768;        // distinct hopping values (v and conj v count once): 15-bit index + conjugate bit
 constexpr int kHashSlots = 1 << 18;     // open-addressing table used while collecting distinct values
 constexpr int kStatusWords = 64;
 
@@ -58,7 +58,7 @@ struct tbpm_ham {
     int64_t lat_off[16] = {0};
     double gershgorin = 0.0;
     int32_t n_table = 0;   // 0: kernels read complex128 values from the canonical CSR
-    int32_t packed = 0;    // n_table <= 2: bit 31 of every ocol word holds the value index (oidx is not read by the kernels)
+    int32_t packed = 0;    // n_table == 1: bit 31 of every ocol word = "conjugate of the table value" (oidx is not read by the kernels)
     int device = 0;
     int num_sms = 0;
 

@@ -38,7 +38,7 @@ struct TermParams {
     int flags;
     int n_table;           // entries of vtab (kernel layout)
     int max_row_off;       // longest off-diagonal row (sizes the staged index slices)
-    int packed;            // n_table <= 2: bit 31 of every ocol word is the value index (build.cu, k_pack_cols)
+    int packed;            // n_table == 1: bit 31 of every ocol word = conjugate of the table value (build.cu)
     // warp-specialised kernel: shared-memory stage geometry (bytes), filled by its launcher
     int n_stage, stage_bytes, cap_entries, off_col, off_idx, off_diag, off_vec;
     int64_t walk_d0;       // phased kernel: tiles per lattice line (1: linear order)
@@ -72,6 +72,13 @@ struct PairParams {
     int *progress;         // [grid] phase-0 tiles finished by each block (zeroed before the launch)
     int *error;            // set when a dependency wait gave up (never, unless the blocks are not co-resident)
 };
+
+// Table value of an entry: index in bits 0-14, bit 15 = take the conjugate (exact: only the sign bit of im changes).
+__device__ __forceinline__ double2 table_value(double2 v, uint32_t idx)
+{
+    v.y = __longlong_as_double(__double_as_longlong(v.y) ^ ((long long)(idx >> 15) << 63));
+    return v;
+}
 
 __device__ __forceinline__ void cfma(double2 &h, double2 v, double2 x)   // h += v * x (complex)
 {

@@ -223,10 +223,10 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_pair(const PairParams
     const uint32_t stage_bytes = (uint32_t)p.stage_bytes;
     const uint32_t a_orp = smem0 + (uint32_t)rl * 4u, a_col = smem0 + (uint32_t)p.off_col, a_idx = smem0 + (uint32_t)p.off_idx,
                    a_diag = smem0 + (uint32_t)p.off_diag;
-    double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // VK >= 1: the (at most two) hopping values, in registers
+    double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // VK >= 1: the one hopping value and its conjugate, in registers
     if (VK >= 1) {
         t0 = __ldg(p.vtab);
-        t1 = p.n_table > 1 ? __ldg(p.vtab + 1) : t0;
+        t1 = make_double2(t0.x, -t0.y);                     // the one table value and its conjugate (bit 31 of the column word)
     }
     double s_re[SPT], s_im[SPT], s_nn[SPT];
 #pragma unroll
@@ -296,7 +296,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_pair(const PairParams
         for (int j = 0; j < CH; ++j) CLoad<SPT>::ld(x[j], xb + (int64_t)(w[j] & 0x7fffffffu) * BT, UNI || c0 + j < n);
         if (VK == 0) {
 #pragma unroll
-            for (int j = 0; j < CH; ++j) v[j] = ldg_value_if(p.vtab + id[j], UNI || c0 + j < n);
+            for (int j = 0; j < CH; ++j) v[j] = table_value(ldg_value_if(p.vtab + (id[j] & 0x7fffu), UNI || c0 + j < n), id[j]);
         }
     };
 

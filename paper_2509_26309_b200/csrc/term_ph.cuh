@@ -177,8 +177,8 @@ __device__ __forceinline__ double2 ldg_value_if(const double2 *p, bool on)
 
 // BT states per tile row, SPT states per thread, CH gathers in flight per thread, NACC terms added to psi' by this launch
 // (0..3), REDUCE: last term of the time step (dot products, T_k not stored).
-// VK, where the hopping values come from:  0 = 16-bit index per entry into the table in global memory;  1 = at most two
-//   values, in registers, selected by bit 31 of the packed column word (build.cu);  2 = ONE REAL value (clean lattices,
+// VK, where the hopping values come from:  0 = 15-bit index + conjugate bit per entry into the table in global memory;
+//   1 = ONE value, in registers, v or conj(v) by bit 31 of the packed column word (build.cu);  2 = ONE REAL value (clean lattices,
 //   Anderson disorder, vacancies): the neighbours are summed and the sum scaled once -- 2 DADD per entry and state
 //   where the complex FMA takes 4 DFMA.
 // UNI: every row holds exactly max_row_off entries, a multiple of CH (periodic lattices): no row offsets, no predicates.
@@ -294,10 +294,10 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     const uint32_t n_uni = (uint32_t)p.max_row_off;         // UNI: every row holds exactly this many entries (a multiple of CH)
     const uint32_t a_orp = smem0 + (uint32_t)rl * 4u, a_col = smem0 + (uint32_t)p.off_col, a_idx = smem0 + (uint32_t)p.off_idx,
                    a_diag = smem0 + (uint32_t)p.off_diag;
-    double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // VK >= 1: the (at most two) hopping values, in registers
+    double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // VK >= 1: the one hopping value and its conjugate, in registers
     if (VK >= 1) {
         t0 = __ldg(p.vtab);
-        t1 = p.n_table > 1 ? __ldg(p.vtab + 1) : t0;
+        t1 = make_double2(t0.x, -t0.y);                     // the one table value and its conjugate (bit 31 of the column word)
     }
     double s_re[SPT], s_im[SPT], s_nn[SPT];
 #pragma unroll
@@ -373,7 +373,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
         }
         if (VK == 0) {
 #pragma unroll
-            for (int j = 0; j < CH; ++j) v[j] = ldg_value_if(p.vtab + id[j], UNI || c0 + j < n);
+            for (int j = 0; j < CH; ++j) v[j] = table_value(ldg_value_if(p.vtab + (id[j] & 0x7fffu), UNI || c0 + j < n), id[j]);
         }
     };
 

@@ -178,10 +178,10 @@ __global__ void __launch_bounds__(kWsThreads, 3) k_term_ws(const TermParams p)
     const int b0 = (tid % LPR) * SPT;                       // first state of this thread
     const double2 *xb = p.x + b0;
     const int le = rl * BT + b0;                            // element within a vector slice of the stage
-    double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // T2: the (at most two) hopping values, in registers
+    double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // T2: the one hopping value and its conjugate, in registers
     if (T2) {
         t0 = __ldg(p.vtab);
-        t1 = p.n_table > 1 ? __ldg(p.vtab + 1) : t0;
+        t1 = make_double2(t0.x, -t0.y);                     // the one table value and its conjugate
     }
     double s_re[SPT], s_im[SPT], s_nn[SPT];
 #pragma unroll
@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(kWsThreads, 3) k_term_ws(const TermParams p)
             const uint16_t *is = reinterpret_cast<const uint16_t *>(st + p.off_idx) + (q0 - lo_s[s][1]);
             auto value = [&](uint32_t i) -> double2 {
                 if (T2) return i ? t1 : t0;
-                return tab_in_smem ? tab_s[i] : __ldg(p.vtab + i);
+                return table_value(tab_in_smem ? tab_s[i & 0x7fffu] : __ldg(p.vtab + (i & 0x7fffu)), i);
             };
             for (uint32_t j = 0; j < n; j += 4) {           // up to 4 independent gathers in flight, predicated tail
                 const bool p1 = j + 1 < n, p2 = j + 2 < n, p3 = j + 3 < n;
@@ -380,7 +380,7 @@ bool term_ws_supported(int bt, const TermParams &p)
 
 int launch_term_ws(int bt, TermParams p, int num_sms, cudaStream_t st, int *grid_out)
 {
-    const bool t2 = p.n_table <= 2;
+    const bool t2 = p.n_table == 1;
     switch (bt) {
     case 1: return t2 ? launch_variant<1, true>(p, num_sms, st, grid_out) : launch_variant<1, false>(p, num_sms, st, grid_out);
     case 2: return t2 ? launch_variant<2, true>(p, num_sms, st, grid_out) : launch_variant<2, false>(p, num_sms, st, grid_out);
