@@ -53,7 +53,8 @@ typedef struct tbpm_ham tbpm_ham; /* opaque host handle pointing into caller-own
 #define TBPM_HOPS_FULL 2u   /* the list already holds both orientations of every pair (default: each pair once and
                                the conjugate partner H_ji = conj(H_ij) is generated)                    */
 #define TBPM_NO_TABLE 4u    /* keep complex128 values in the kernel layout instead of 16-bit indices into a table of
-                               distinct hopping values (the table is the default whenever <= 65536 values occur)      */
+                               distinct hopping values (the table is the default whenever <= 32768 values occur,
+                               v and conj(v) counting once)                                                            */
 
 const char *tbpm_strerror(int code);
 const char *tbpm_version(void);
