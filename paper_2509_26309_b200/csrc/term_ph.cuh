@@ -89,6 +89,14 @@ __device__ __forceinline__ uint32_t lds_u16(uint32_t a)
     asm volatile("{\n.reg .u16 h;\nld.shared.u16 h, [%1];\ncvt.u32.u16 %0, h;\n}" : "=r"(v) : "r"(a));
     return v;
 }
+__device__ __forceinline__ void lds_v2_u32(uint32_t a, uint32_t &x, uint32_t &y)
+{
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(x), "=r"(y) : "r"(a));
+}
+__device__ __forceinline__ void lds_v4_u32(uint32_t a, uint32_t &x, uint32_t &y, uint32_t &z, uint32_t &w)
+{
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(w) : "r"(a));
+}
 __device__ __forceinline__ double lds_f64(uint32_t a)
 {
     double v;
@@ -351,14 +359,34 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     };
     auto load_chunk = [&]() {                               // indices of entries [c0, c0 + CH) of the row, then their gathers
         uint32_t id[CH];
+        if constexpr (UNI && CH % 4 == 0) {                 // uniform rows of 4k entries: the slices are 16-byte aligned
 #pragma unroll
-        for (int j = 0; j < CH; ++j) {
-            if (UNI) {
-                w[j] = lds_u32(ca + 4u * (c0 + j));
-                id[j] = VK == 0 ? lds_u16(ia + 2u * (c0 + j)) : 0u;
-            } else {
-                w[j] = lds_u32_if(ca + 4u * (c0 + j), c0 + j < n);
-                id[j] = VK == 0 ? lds_u16_if(ia + 2u * (c0 + j), c0 + j < n) : 0u;
+            for (int j = 0; j < CH; j += 4) {
+                lds_v4_u32(ca + 4u * (c0 + j), w[j], w[j + 1], w[j + 2], w[j + 3]);
+                if (VK == 0) {
+                    uint32_t lo, hi;
+                    lds_v2_u32(ia + 2u * (c0 + j), lo, hi);
+                    id[j] = lo & 0xffffu; id[j + 1] = lo >> 16; id[j + 2] = hi & 0xffffu; id[j + 3] = hi >> 16;
+                } else {
+                    id[j] = id[j + 1] = id[j + 2] = id[j + 3] = 0u;
+                }
+            }
+        } else if constexpr (UNI && CH % 2 == 0 && VK != 0) { // uniform rows of 2k entries (cubic: 6): 8-byte aligned
+#pragma unroll
+            for (int j = 0; j < CH; j += 2) {
+                lds_v2_u32(ca + 4u * (c0 + j), w[j], w[j + 1]);
+                id[j] = id[j + 1] = 0u;
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < CH; ++j) {
+                if (UNI) {
+                    w[j] = lds_u32(ca + 4u * (c0 + j));
+                    id[j] = VK == 0 ? lds_u16(ia + 2u * (c0 + j)) : 0u;
+                } else {
+                    w[j] = lds_u32_if(ca + 4u * (c0 + j), c0 + j < n);
+                    id[j] = VK == 0 ? lds_u16_if(ia + 2u * (c0 + j), c0 + j < n) : 0u;
+                }
             }
         }
         if (c0 + CH >= nmax) {                              // last chunk of every row of this warp: the stage is free again
