@@ -119,6 +119,15 @@ int64_t tbpm_last_launch_count(void);
 /* Kernels launched by this library in this process since it was loaded (build + propagate + get_state). */
 int64_t tbpm_total_launch_count(void);
 
+/* ---- NEXT-1: DOS from the correlation function (`Analyzer.calc_dos(corr)`) ----------------
+ * The paper prints no formula; reading #27: average corr over the states, C_0 = 1, C_{-n} = conj(C_n), Hann window
+ * w_n = (1 + cos(pi n / n_step)) / 2, and
+ *     dos[j] = (dt / 2 pi) * [ 1 + 2 Re sum_{n=1}^{n_step} w_n C_n exp(+i n E_j dt) ],   E_j = -rescale + j * rescale / n_step,
+ * j = 0 .. 2 n_step (at dt = pi / rescale the sampling interval matches the window [-rescale, rescale] and the sum of dos[j]
+ * times the grid step is 1).  corr: device [n_state][n_step][2] as written by tbpm_propagate / tbpm_ldos; energy, dos: device
+ * out [2 n_step + 1].  Plain direct transform (n_step <= a few thousand), one thread per energy.  Asynchronous on `stream`. */
+int tbpm_dos(const double *corr, int n_state, int n_step, double dt, double rescale, double *energy, double *dos, void *stream);
+
 /* ---- end to end with HOST buffers ------------------------------------------------------------------------------------
  * Whole path for host-resident inputs: H2D of the list and psi0, tbpm_build, tbpm_propagate, D2H of corr/norm2, then a
  * stream synchronise.  `arena` is caller-owned device memory of at least tbpm_corr_host_bytes(); host buffers should be

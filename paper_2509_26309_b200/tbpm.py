@@ -51,6 +51,7 @@ def lib() -> C.CDLL:
         L.tbpm_propagate.argtypes = [vp, vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp, sz, vp]
         L.tbpm_ldos.argtypes = [vp, vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp, sz, vp]
         L.tbpm_get_state.argtypes = [vp, vp, C.c_int, vp, vp]
+        L.tbpm_dos.argtypes = [vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp]
         L.tbpm_last_launch_count.restype = i64
         L.tbpm_total_launch_count.restype = i64
         L.tbpm_corr_host_bytes.argtypes = [i64, i64, C.c_int, C.c_int, C.c_int, u32, P(sz)]
@@ -205,6 +206,18 @@ def tbpm_ldos(H: Hamiltonian, sites, n_step: int, dt: float, rescale: float, wor
                              _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "tbpm_ldos")
     return corr, norm2, workspace
+
+
+def tbpm_dos(corr: torch.Tensor, dt: float, rescale: float):
+    """corr complex128 [n_state][n_step] on the device -> (energy, dos), float64 [2 n_step + 1] each (tbpm.h: NEXT-1)."""
+    _need_cuda(corr)
+    corr = corr.contiguous()
+    n_state, n_step = (1, corr.shape[0]) if corr.dim() == 1 else corr.shape
+    energy = torch.zeros(2 * n_step + 1, dtype=torch.float64, device=corr.device)
+    dos = torch.zeros_like(energy)
+    with torch.cuda.device(corr.device):
+        _check(lib().tbpm_dos(_ptr(corr), n_state, n_step, dt, rescale, _ptr(energy), _ptr(dos), _stream(corr.device)), "tbpm_dos")
+    return energy, dos
 
 
 def tbpm_get_state(H: Hamiltonian, workspace: torch.Tensor, state: int) -> torch.Tensor:

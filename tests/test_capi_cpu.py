@@ -69,6 +69,9 @@ def test_sizes_and_argument_checks():
     assert L.tbpm_get_state(None, None, 0, None, None) == tbpm.TBPM_EINVAL
     assert L.tbpm_export_csr(None, None, None, None, None) == tbpm.TBPM_EINVAL
     assert L.tbpm_check_bound(None, 1.0) == tbpm.TBPM_EINVAL
+    assert L.tbpm_dos(None, 1, 4, 0.1, 1.0, None, None, None) == tbpm.TBPM_EINVAL
+    assert L.tbpm_dos(None, 0, 4, 0.1, 1.0, None, None, None) == tbpm.TBPM_OK        # nothing to do
+    assert L.tbpm_dos(None, 1, 4, 0.1, -1.0, None, None, None) == tbpm.TBPM_EINVAL
     b = tbpm.tbpm_corr_host_bytes(8192, 12288, False, 1, 256)
     assert b > p
     for code in range(0, -8, -1):

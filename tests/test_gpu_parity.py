@@ -288,6 +288,27 @@ def test_corr_host_matches_device_path(dev, oracle_mod):
 # ---------------------------------------------------------------------------------------------------------------------
 # full-size configs, in the launch configuration bench.py times
 # ---------------------------------------------------------------------------------------------------------------------
+def test_dos_from_corr(dev, oracle_mod):
+    """NEXT-1 (tbpm_dos): Hann-windowed direct transform of the state-averaged correlation against the oracle's
+    dos_from_corr (itself pinned by the honeycomb and chain closed forms, tests/test_oracle_pins.py)."""
+    w = W.make_workload(2, device=dev, Na=48, Nb=40, n_state=3)
+    psi0 = w.psi0(n_state=3)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    n_step = 200
+    corr, _, _ = tbpm.tbpm_propagate(H, psi0, n_step, w.dt, w.rescale)
+    E, D = tbpm.tbpm_dos(corr, w.dt, w.rescale)
+    torch.cuda.synchronize()
+    Eo, Do = oracle_mod.dos_from_corr(corr.cpu().numpy().mean(axis=0), w.rescale)
+    assert E.shape == (2 * n_step + 1,)
+    assert np.abs(E.cpu().numpy() - Eo).max() <= 1e-12 * w.rescale
+    assert np.abs(D.cpu().numpy() - Do).max() <= 1e-10 * np.abs(Do).max()
+    assert abs(float(D.sum()) * w.rescale / n_step - 1.0) < 2e-2           # integrates to one state per orbital
+    E1, D1 = tbpm.tbpm_dos(corr[1], w.dt, w.rescale)                      # one state, 1-D input
+    _, D1o = oracle_mod.dos_from_corr(corr[1].cpu().numpy(), w.rescale)
+    assert np.abs(D1.cpu().numpy() - D1o).max() <= 1e-10 * np.abs(D1o).max()
+    assert tbpm.lib().tbpm_dos(None, 1, 4, 0.1, 1.0, None, None, None) == tbpm.TBPM_EINVAL
+
+
 FULL = os.environ.get("TBPM_TEST_FULL", "1") != "0"
 
 
