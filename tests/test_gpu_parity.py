@@ -288,6 +288,26 @@ def test_corr_host_matches_device_path(dev, oracle_mod):
 # ---------------------------------------------------------------------------------------------------------------------
 # full-size configs, in the launch configuration bench.py times
 # ---------------------------------------------------------------------------------------------------------------------
+LONG = os.environ.get("TBPM_TEST_LONG", "0") == "1"
+
+
+@pytest.mark.skipif(not LONG, reason="TBPM_TEST_LONG=1 runs the full-length oracle of config 2 (minutes of CPU time)")
+def test_config2_full_length(dev, oracle_mod):
+    """BASELINE.json:configs[1] exactly: 4 states x 1024 steps at 2,097,152 orbitals, every entry of corr against the
+    oracle (parity protocol (1) of SURVEY 8(d)).  Opt-in: about three minutes of oracle time on 16 host cores."""
+    w = W.make_workload(2, device=dev)
+    psi0 = w.psi0(device=dev)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    corr, norm2, _ = tbpm.tbpm_propagate(H, psi0, w.n_step, w.dt, w.rescale)
+    torch.cuda.synchronize()
+    hi, hj, hv, on = to_np(w)
+    ref, refn = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0.cpu().numpy(), w.n_step, w.dt, w.rescale, form="csr")
+    err = np.abs(corr.cpu().numpy() - ref).max()
+    print(f"config 2 full length: max|dcorr| = {err:.3e}, max|norm2 - 1| = {np.abs(norm2.cpu().numpy() - 1).max():.3e}")
+    assert err <= CORR_TOL
+    assert np.abs(norm2.cpu().numpy() - 1).max() <= NORM_TOL
+
+
 def test_dos_from_corr(dev, oracle_mod):
     """NEXT-1 (tbpm_dos): Hann-windowed direct transform of the state-averaged correlation against the oracle's
     dos_from_corr (itself pinned by the honeycomb and chain closed forms, tests/test_oracle_pins.py)."""
