@@ -357,6 +357,7 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     if (!H || n_state < 0 || n_step < 0 || !(rescale > 0.0) || !(dt >= 0.0) || !std::isfinite(dt) || !std::isfinite(rescale))
         return TBPM_EINVAL;
     g_launches = 0;
+    ++env_epoch();                                        // re-read the TBPM_* switches for this call
     if (n_state == 0 || n_step == 0) return TBPM_OK;
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || !corr || (!psi0 && !sites)) return TBPM_EINVAL;
     if (psi0 && (reinterpret_cast<uintptr_t>(psi0) & 15u)) return TBPM_EINVAL;
@@ -405,6 +406,7 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
 
     bool fused_any = false;
+    std::vector<TermParams> term;
     int *pair_progress = reinterpret_cast<int *>(reinterpret_cast<char *>(partial) + kPartialBytes - 4 * sizeof(int) * kMaxGrid);   // [0,G): counters; [kMaxGrid]: error; [2 kMaxGrid, ..): per-warp scratch
     TBPM_CUDA_TRY(cudaMemsetAsync(pair_progress + kMaxGrid, 0, sizeof(int), st));
     const int rev_mode = env_int("TBPM_REV", 1);   // odd terms sweep backwards (term_ph.cuh)
@@ -453,7 +455,7 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
                 if ((rc = launch_term(bt, table, tp, H->num_sms, st, &grid))) return rc;
             }
             int flushed = -1;                             // highest term already added to psi'
-            std::vector<TermParams> term((size_t)K);      // term[k]: launch parameters of Chebyshev term k of this step
+            term.assign((size_t)K, TermParams{});        // term[k]: launch parameters of Chebyshev term k of this step
             for (int k = 1; k < K; ++k) {
                 // buffers: T_k overwrites T_{k-2}; T_0 = psi, T_1 = t1, T_2 -> psi's buffer, ...
                 tp.x = (k % 2 == 1) ? psi : t1;           // T_{k-1}

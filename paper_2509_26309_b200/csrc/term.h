@@ -2,6 +2,7 @@
 #pragma once
 
 #include <cstdlib>
+#include <unordered_map>
 
 #include "tbpm_internal.h"
 
@@ -88,10 +89,24 @@ __device__ __forceinline__ void cfma(double2 &h, double2 v, double2 x)   // h +=
     h.y = fma(v.y, x.x, h.y);
 }
 
+// Experiment switches (TBPM_*): read from the environment once per tbpm_propagate / tbpm_ldos call -- env_epoch() is bumped
+// at the start of every call -- not once per kernel launch.
+inline unsigned long long &env_epoch()
+{
+    static thread_local unsigned long long e = 1;
+    return e;
+}
 inline int env_int(const char *name, int dflt)
 {
-    const char *e = std::getenv(name);
-    return e ? std::atoi(e) : dflt;
+    struct Entry { unsigned long long epoch; int value; };
+    static thread_local std::unordered_map<const char *, Entry> cache;   // keyed by the literal's address: one entry per call site
+    Entry &c = cache[name];
+    if (c.epoch != env_epoch()) {
+        const char *e = std::getenv(name);
+        c.value = e ? std::atoi(e) : dflt;
+        c.epoch = env_epoch();
+    }
+    return c.value;
 }
 
 // Warp-specialised bulk-copy (TMA) kernel, term_ws.cu.  Returns TBPM_EINVAL if (bt, flags) has no instantiation
