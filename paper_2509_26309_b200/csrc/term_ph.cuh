@@ -557,7 +557,7 @@ int launch_variant(const TermParams &p, int num_sms, cudaStream_t st, int *grid_
 }
 
 // Shape of the instruction stream, chosen from what the builder found (table size, one real value, uniform rows) and
-// the tile width.  NW = 23 leaves 80 registers per thread, NW = 19 -> 96, NW = 15 -> 128.
+// the tile width.  NW = 31 leaves 64 registers per thread, NW = 23 -> 80, NW = 19 -> 96, NW = 15 -> 128.
 template <int BT>
 int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
@@ -576,6 +576,10 @@ int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
             for (int j = 0; j < q.n_lat_off; ++j)
                 if (q.lat_off[j] % R16 == 0 && q.lat_off[j] * 4 <= q.n_orb) { q.walk_stride = q.lat_off[j]; q.walk_run = 64; }
         if (q.walk_stride > 0 && q.walk_stride % R16 == 0) return launch_variant<BT, SPT, 6, 2, true, 16>(q, num_sms, st, grid_out);
+    }
+    if constexpr (BT == 1) if (p.n_orb >= (int64_t)31 * 32 * num_sms) {   // one state per tile: 64 registers suffice -> 31 consumer warps
+        if (vk == 2 && uni && n == 3) return launch_variant<BT, SPT, 3, 2, true, 31>(p, num_sms, st, grid_out);
+        if (vk == 2 && n <= 4) return launch_variant<BT, SPT, 4, 2, false, 31>(p, num_sms, st, grid_out);   // cfg3: 0.72 -> 0.79
     }
     if (vk == 2) {
         if (uni && n == 3) return launch_variant<BT, SPT, 3, 2, true, kNwA>(p, num_sms, st, grid_out);   // honeycomb
