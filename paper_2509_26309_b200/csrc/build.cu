@@ -23,6 +23,7 @@
 #include <climits>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "tbpm_internal.h"
 
@@ -573,18 +574,35 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
         }
         H->n_table = hst[ST_NTAB];
     }
-    // Lattice strides: on a matrix whose rows all have the same length, the column offsets of one row in the middle are
-    // the strides of the lattice (1, a line, a plane); propagate walks its tiles along the largest usable one.
+    // Lattice strides: on a matrix whose rows all have the same length, the column offsets (col - row) of a typical row are
+    // the strides of the lattice (1, a line, a plane).  64 rows spread over the matrix are sampled and the most frequent tuple
+    // of offsets wins (a single sample could sit on the periodic boundary).  propagate walks its tiles along the largest
+    // usable stride, and the staged-gather kernel takes its segments from the tuple.
     {
         const int n_off = H->max_row_nnz - (has_onsite ? 1 : 0);
         if (n_orb > 0 && H->min_row_nnz == H->max_row_nnz && n_off > 0 && n_off <= 16) {
-            const int64_t mid = n_orb / 2;
-            int32_t cw[16];
-            TRY_OR_FAIL(cudaMemcpyAsync(cw, H->ocol + mid * n_off, sizeof(int32_t) * n_off, cudaMemcpyDeviceToHost, st));
+            constexpr int kSamples = 64;
+            std::vector<int32_t> cw((size_t)kSamples * n_off);
+            std::vector<int64_t> rows(kSamples);
+            for (int i = 0; i < kSamples; ++i) {
+                rows[i] = (int64_t)(((unsigned long long)(i + 1) * 0x9E3779B97F4A7C15ull >> 11) % (unsigned long long)n_orb);   // scattered
+                TRY_OR_FAIL(cudaMemcpyAsync(cw.data() + (size_t)i * n_off, H->ocol + rows[i] * n_off, sizeof(int32_t) * n_off,
+                                            cudaMemcpyDeviceToHost, st));
+            }
             TRY_OR_FAIL(cudaStreamSynchronize(st));
+            std::vector<std::vector<int64_t>> tup(kSamples, std::vector<int64_t>(n_off));
+            for (int i = 0; i < kSamples; ++i)
+                for (int j = 0; j < n_off; ++j) tup[i][j] = (int64_t)(cw[(size_t)i * n_off + j] & 0x7fffffff) - rows[i];
+            int best = 0, best_count = 0;
+            for (int i = 0; i < kSamples; ++i) {
+                int c = 0;
+                for (int k = 0; k < kSamples; ++k) c += tup[k] == tup[i];
+                if (c > best_count) { best_count = c; best = i; }
+            }
             for (int j = 0; j < n_off; ++j) {
-                const int64_t c = cw[j] & 0x7fffffff;
-                H->lat_off[H->n_lat_off++] = c > mid ? c - mid : mid - c;
+                const int64_t dlt = tup[best][j];
+                H->lat_delta[H->n_lat_off] = dlt;           // signed, in the order of the row's entries
+                H->lat_off[H->n_lat_off++] = dlt > 0 ? dlt : -dlt;
             }
             std::sort(H->lat_off, H->lat_off + H->n_lat_off);
         }

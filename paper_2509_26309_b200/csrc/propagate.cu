@@ -322,6 +322,10 @@ int launch_term(int bt, bool table, const TermParams &p, int num_sms, cudaStream
 {
     // phased kernel (term_ph.cuh) whenever it has an instantiation for this term; TBPM_KERNEL=0: the earlier
     // warp-specialised kernel with staged vectors (term_ws.cu); else the direct kernel below
+    if (table && term_sg_supported(bt, p)) {               // vector rows staged in shared memory (uniform lattices, 8 states)
+        ++g_launches;
+        return launch_term_sg(p, num_sms, st, grid_out);
+    }
     if (table && env_int("TBPM_KERNEL", 1) != 0 && term_ph_supported(bt, p)) {
         ++g_launches;
         switch (bt) {
@@ -397,7 +401,7 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     tp.single_real = H->single_real;
     tp.walk_stride = 0; tp.walk_run = 1;
     tp.n_lat_off = H->n_lat_off;
-    for (int j = 0; j < H->n_lat_off; ++j) tp.lat_off[j] = H->lat_off[j];
+    for (int j = 0; j < H->n_lat_off; ++j) { tp.lat_off[j] = H->lat_off[j]; tp.lat_delta[j] = H->lat_delta[j]; }
     if (const char *w = std::getenv("TBPM_WALK")) {          // "rows per lattice line,lines per run"
         long long a = 0; int b = 1;
         if (std::sscanf(w, "%lld,%d", &a, &b) >= 1) { tp.walk_stride = a; tp.walk_run = b; }

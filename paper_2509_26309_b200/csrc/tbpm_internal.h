@@ -56,6 +56,7 @@ struct tbpm_ham {
     int32_t halo_rows = 0;     // widest circular |col - row|
     int32_t n_lat_off = 0;     // uniform rows: |col - row| of the entries of one sample row (lattice strides), ascending
     int64_t lat_off[16] = {0};
+    int64_t lat_delta[16] = {0};   // the same offsets signed, in the order of the sample row's entries (slot j -> col - row)
     double gershgorin = 0.0;
     int32_t n_table = 0;   // 0: kernels read complex128 values from the canonical CSR
     int32_t packed = 0;    // n_table == 1: bit 31 of every ocol word = "conjugate of the table value" (oidx is not read by the kernels)

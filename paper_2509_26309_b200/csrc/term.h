@@ -48,6 +48,7 @@ struct TermParams {
     int walk_run;          // lines per run when walk_stride is used
     int n_lat_off;         // lattice strides found by the builder (uniform rows only), ascending
     int64_t lat_off[16];
+    int64_t lat_delta[16]; // signed offsets of the sample row's entries, in slot order
     int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
     int reverse;           // phased kernel: sweep the tiles from the last row block to the first
     int uniform;           // every row holds exactly max_row_off off-diagonal entries
@@ -120,6 +121,10 @@ int launch_term_ph_bt1(const TermParams &p, int num_sms, cudaStream_t st, int *g
 int launch_term_ph_bt2(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 int launch_term_ph_bt4(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 int launch_term_ph_bt8(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
+
+// Staged-gather kernel (term_sg.cu): tiles of 8 states on uniform lattices; false / TBPM_EINVAL when it does not apply.
+bool term_sg_supported(int bt, const TermParams &p);
+int launch_term_sg(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
 // Pair kernel, one file per tile width (2, 4, 8 states).
 int launch_term_pair_bt2(const PairParams &p, int num_sms, cudaStream_t st, int *grid_out);

@@ -186,6 +186,18 @@ def test_two_terms_per_sweep(dev, oracle_mod, cfg, over, n_state, n_step, monkey
     run_parity(dev, oracle_mod, w, n_state, n_step)
 
 
+@pytest.mark.parametrize("cfg,over,n_state,n_step", [
+    (4, dict(Lx=64, Ly=48, phi_den=32), 8, 10),                      # table shape: three segments, rows at the boundary fall back
+    (5, dict(L=17), 16, 9),                                          # cubic shape: five segments, two tiles of states
+    (5, dict(L=32), 8, 6),                                           # tiles wholly inside a lattice line: the LDS-only path
+])
+def test_staged_gathers(dev, oracle_mod, cfg, over, n_state, n_step, monkeypatch):
+    """term_sg.cu (experimental, TBPM_SG): vector rows of a tile staged in shared memory by bulk copies of lattice runs."""
+    monkeypatch.setenv("TBPM_SG", "1")
+    w = W.make_workload(cfg, device=dev, **over)
+    run_parity(dev, oracle_mod, w, n_state, n_step)
+
+
 @pytest.mark.parametrize("tile", ["1", "2", "4", "16", "32"])
 def test_other_tile_widths(dev, oracle_mod, tile, monkeypatch):
     monkeypatch.setenv("TBPM_TILE", tile)
