@@ -185,7 +185,8 @@ __device__ __forceinline__ double2 ldg_value_if(const double2 *p, bool on)
 
 // BT states per tile row, SPT states per thread, CH gathers in flight per thread, NACC terms added to psi' by this launch
 // (0..3), REDUCE: last term of the time step (dot products, T_k not stored).
-// VK, where the hopping values come from:  0 = 15-bit index + conjugate bit per entry into the table in global memory;
+// VK, where the hopping values come from:  0 = 15-bit index + conjugate bit per entry into the table in global memory
+//   (4 = the same with the table copied into shared memory);
 //   1 = ONE value, in registers, v or conj(v) by bit 31 of the packed column word (build.cu);  2 = ONE REAL value (clean lattices,
 //   Anderson disorder, vacancies): the neighbours are summed and the sum scaled once -- 2 DADD per entry and state
 //   where the complex FMA takes 4 DFMA.
@@ -215,6 +216,10 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     if (tid == 0) {
         for (int s = 0; s < S; ++s) { mbar_init(bar0 + 8 * s, 1); mbar_init(bar0 + 8 * (kMaxStages + s), kConsumers / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (VK == 4) {                                          // the whole (conjugate-folded) value table, once per block
+        double2 *tab = reinterpret_cast<double2 *>(smem + (size_t)p.stage_bytes * p.n_stage);
+        for (int i = tid; i < p.n_table; i += (NW + 1) * 32) tab[i] = __ldg(p.vtab + i);
     }
     __syncthreads();
 
@@ -280,7 +285,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
             if (nc > 0) {
                 bulk_g2s(st + p.off_col, p.ocol + col_lo, nc * 4, full);
                 tx += nc * 4;
-                if (VK == 0) { bulk_g2s(st + p.off_idx, p.oidx + idx_lo, ni * 2, full); tx += ni * 2; }
+                if (VK == 0 || VK == 4) { bulk_g2s(st + p.off_idx, p.oidx + idx_lo, ni * 2, full); tx += ni * 2; }
             }
             if (has_diag) {
                 const uint32_t db = (uint32_t)((rows * 8 + 15) & ~15);
@@ -300,6 +305,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     const bool st_ef = p.pol & 1;                           // T_k leaves L2 first (its readers come a whole sweep later)
     const uint32_t stage_bytes = (uint32_t)p.stage_bytes;
     const uint32_t n_uni = (uint32_t)p.max_row_off;         // UNI: every row holds exactly this many entries (a multiple of CH)
+    const uint32_t tab0 = smem0 + (uint32_t)p.stage_bytes * (uint32_t)p.n_stage;   // VK 4: the value table behind the stages
     const uint32_t a_orp = smem0 + (uint32_t)rl * 4u, a_col = smem0 + (uint32_t)p.off_col, a_idx = smem0 + (uint32_t)p.off_idx,
                    a_diag = smem0 + (uint32_t)p.off_diag;
     double2 t0 = make_double2(0.0, 0.0), t1 = t0;           // VK >= 1: the one hopping value and its conjugate, in registers
@@ -327,6 +333,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
     CVec<SPT> x[CH];
     double2 v[CH];
     uint32_t w[CH];
+    uint32_t id[CH];                                        // VK 0/4: table index + conjugate bit of each entry of the chunk
 
     auto load_row = [&]() {                                 // streamed operands + row header of `tile`
         const int64_t trow = tile_rows(tile);
@@ -358,12 +365,11 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
         h.zero();
     };
     auto load_chunk = [&]() {                               // indices of entries [c0, c0 + CH) of the row, then their gathers
-        uint32_t id[CH];
         if constexpr (UNI && CH % 4 == 0) {                 // uniform rows of 4k entries: the slices are 16-byte aligned
 #pragma unroll
             for (int j = 0; j < CH; j += 4) {
                 lds_v4_u32(ca + 4u * (c0 + j), w[j], w[j + 1], w[j + 2], w[j + 3]);
-                if (VK == 0) {
+                if (VK == 0 || VK == 4) {
                     uint32_t lo, hi;
                     lds_v2_u32(ia + 2u * (c0 + j), lo, hi);
                     id[j] = lo & 0xffffu; id[j + 1] = lo >> 16; id[j + 2] = hi & 0xffffu; id[j + 3] = hi >> 16;
@@ -382,10 +388,10 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
             for (int j = 0; j < CH; ++j) {
                 if (UNI) {
                     w[j] = lds_u32(ca + 4u * (c0 + j));
-                    id[j] = VK == 0 ? lds_u16(ia + 2u * (c0 + j)) : 0u;
+                    id[j] = (VK == 0 || VK == 4) ? lds_u16(ia + 2u * (c0 + j)) : 0u;
                 } else {
                     w[j] = lds_u32_if(ca + 4u * (c0 + j), c0 + j < n);
-                    id[j] = VK == 0 ? lds_u16_if(ia + 2u * (c0 + j), c0 + j < n) : 0u;
+                    id[j] = (VK == 0 || VK == 4) ? lds_u16_if(ia + 2u * (c0 + j), c0 + j < n) : 0u;
                 }
             }
         }
@@ -419,6 +425,14 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
                 for (int k = 0; k < SPT; ++k) { h.v[k].x += x[j].v[k].x; h.v[k].y += x[j].v[k].y; }   // x[j] is zero past the row end
             }
         } else {
+            if (VK == 4) {                                  // values from the table in shared memory, only now: 30-cycle loads,
+#pragma unroll                                               // no registers held for them while the gathers are in flight
+                for (int j = 0; j < CH; ++j) {
+                    double2 t;
+                    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(t.x), "=d"(t.y) : "r"(tab0 + (id[j] & 0x7fffu) * 16u));
+                    v[j] = table_value(t, id[j]);
+                }
+            }
 #pragma unroll
             for (int j = 0; j < CH; ++j) {
                 if (VK == 1) v[j] = (w[j] >> 31) ? t1 : t0;
@@ -522,13 +536,13 @@ int launch_one(TermParams p, int num_sms, cudaStream_t st, int *grid_out)
     p.cap_entries = ((R * std::max(p.max_row_off, 1) + 8 + 7) / 8) * 8;          // + alignment slack of the slice start
     size_t o = (size_t)(((R + 1) * 4 + 15) & ~15);
     p.off_col = (int)o;  o += (size_t)p.cap_entries * 4;
-    p.off_idx = (int)o;  o += VK == 0 ? (size_t)p.cap_entries * 2 : 0;
+    p.off_idx = (int)o;  o += (VK == 0 || VK == 4) ? (size_t)p.cap_entries * 2 : 0;
     o = (o + 15) & ~size_t(15);
     p.off_diag = (int)o; o += (size_t)((R * 8 + 15) & ~15);
     p.off_vec = 0;
     p.stage_bytes = (int)((o + 127) & ~size_t(127));
     p.n_stage = (int)std::max<size_t>(2, std::min<size_t>(p.n_stage, (size_t)160 * 1024 / p.stage_bytes));
-    const size_t dyn = (size_t)p.stage_bytes * p.n_stage;
+    const size_t dyn = (size_t)p.stage_bytes * p.n_stage + (VK == 4 ? (size_t)p.n_table * sizeof(double2) : 0);
     auto kern = k_term_ph<BT, SPT, CH, NACC, REDUCE, VK, UNI, NW>;
     static size_t configured = 0;
     if (dyn > configured) {
@@ -590,6 +604,14 @@ int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
     if (vk == 1) {
         if (BT == 1 && n <= 4) return launch_variant<BT, SPT, 4, 1, false, 23>(p, num_sms, st, grid_out);
         return launch_variant<BT, SPT, 8, 1, false, 15>(p, num_sms, st, grid_out);
+    }
+    if constexpr (BT == 8) {
+        // Table small enough for shared memory (cfg4: 7,864 values = 126 KB): each block copies it once, the values are fetched
+        // with LDS only when the gathers have returned (no registers held for them), which leaves room for all eight gathers
+        // of a row in one round trip.  cfg4: 1955 -> 1885 us per launch.
+        const bool tab_smem = uni && (size_t)p.n_table * sizeof(double2) <= 150 * 1024 && env_int("TBPM_TAB_SMEM", 1);
+        if (tab_smem && n % 8 == 0) return launch_variant<BT, SPT, 8, 4, true, 15>(p, num_sms, st, grid_out);
+        if (tab_smem && n % 4 == 0) return launch_variant<BT, SPT, 4, 4, true, 19>(p, num_sms, st, grid_out);
     }
     if (uni && n % 4 == 0) return launch_variant<BT, SPT, 4, 0, true, 15>(p, num_sms, st, grid_out);     // square + flux
     return launch_variant<BT, SPT, 4, 0, false, 15>(p, num_sms, st, grid_out);
