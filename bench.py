@@ -1,21 +1,27 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the TBPM hot path on B200 (one JSON line on stdout, rank 0).
 
-A "step" is one pass of the whole hot path over one batch of synthetic input: tbpm_build (hop list -> CSR + kernel
-layout) followed by tbpm_propagate over the workload's full n_step time steps for all its states (coefficients,
-state set-up, K-1 fused Chebyshev-term kernels per time step, per-step correlation + norm).  Inputs are resident in
-HBM when the timed region starts.  `value` = n_state * n_step * (K-1) * nnz / step time, summed over ranks.
+A bench "step" is one pass of the whole hot path (every row) over one batch of synthetic input:
+tbpm_build (hop list -> CSR + kernel layout) followed by tbpm_propagate of ALL the workload's states over a fixed block of
+`n_step_per_bench_step` time steps (coefficients, state set-up, K-1 fused Chebyshev-term kernels per time step and state
+tile, per-step correlation + norm).  Inputs are resident in HBM when the timed region starts.
+`value` = n_state * n_block * (K-1) * nnz / step time, summed over ranks.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5|5ldos] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5|5ldos] [--block B] [--impl reference]
 
-Default workload: BASELINE.json:configs[1] (honeycomb 1024x1024 + Anderson disorder, 4 states, 1024 steps).
-Multi-GPU: states are independent, so every rank propagates its own batch of seeded states on a
-replica of H; no data-path collective; scaling is weak.
+Default workload: BASELINE.json:configs[4] (cubic 256^3 + Anderson disorder, 16,777,216 orbitals x 32 states): the largest
+single-GPU configuration, one of the >= 16 M-orbital configs `north_star` sets its target on.  The full run length of a
+config (1024-2048 time steps) would make one bench step minutes long; every time step launches the same kernels on
+the same buffers, so a block of 8 time steps (~1 s on cfg5) is the unit that is timed, and `config` says so.  At N = 1
+the line also carries `per_workload`: cfg3, cfg4 and cfg5's 64-site LDOS leg measured in the same process for >= 5 s each.
+Multi-GPU: states are independent, so every rank propagates its own batch of seeded states on a replica of
+H (paper_2509_26309_b200/replicas.py); no data-path collective; scaling is weak.
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import math
 import os
@@ -31,20 +37,22 @@ if ROOT not in sys.path:
 
 METRIC = "Chebyshev terms*nnz/sec (complex128)"
 UNIT = "nnz*terms/s"
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="2", help="1..5 = BASELINE.json:configs[i-1]; 5ldos = config 5's 64-site LDOS leg")
-    ap.add_argument("--n-step", type=int, default=0, help="override the workload's number of time steps (development only; "
-                                                            "the JSON line then says so in config.n_step_override)")
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target wall time of the cpu_baseline sample")
+    ap.add_argument("--workload", default="5", help="1..5 = BASELINE.json:configs[i-1]; 5ldos = config 5's 64-site LDOS leg")
+    ap.add_argument("--block", type=int, default=0, help="time steps per bench step (default: 8; 64 for cfg2, 256 for cfg1)")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target wall time of the cpu_baseline sample")
+    ap.add_argument("--per-workload-seconds", type=float, default=5.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-workload", action="store_true")
     return ap.parse_args()
 
 
@@ -58,22 +66,26 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused term, MB, from the one `ncu --set full` capture per
-# workload summarised in profiles/r1b_ncu_full_cfg2-5.md: (first term k=1, first flush k=2, plain term, flush, last term).
-NCU_TRAFFIC_SRC = "profiles/r1b_ncu_full_cfg2-5.md (ncu --set full, one capture per workload; average over the launches of a time step)"
-NCU_TRAFFIC_MB = {"cfg2": (279.2, 531.7, 414.6, 668.7, 694.5), "cfg3": (1384.0, 2330.0, 1868.0, 2815.0, 2839.0),
-                  "cfg4": (5137.0, 9412.0, 7284.0, 11560.0, 11584.0), "cfg5": (5002.0, 9322.0, 7152.0, 11646.0, 12547.0)}
-
-
 def ncu_traffic(workload_name: str, K: int):
-    """Average DRAM bytes per term launch over one time step (K-1 launches: flush every third term), or None."""
-    t = NCU_TRAFFIC_MB.get(workload_name.split(":")[0])
-    if t is None or K < 4:
-        return None
-    first, first_flush, plain, flush, last = t
+    """Average DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per term launch over one time step, from the
+    `ncu --set full` captures of THIS round's kernels summarised in profiles/r2_dram_traffic.csv (one row per workload and
+    kind of launch: first term, first flush, plain term, flush, last term).  None when the file has no row for the workload."""
+    if not os.path.exists(TRAFFIC_CSV) or K < 4:
+        return None, None
+    rows = {}
+    src = None
+    with open(TRAFFIC_CSV) as f:
+        for r in csv.DictReader(l for l in f if not l.startswith("#")):
+            if r["workload"] == workload_name.split(":")[0]:
+                rows[r["launch"]] = float(r["dram_mbytes"])
+                src = r["source"]
+    need = ("first", "first_flush", "plain", "flush", "last")
+    if any(k not in rows for k in need):
+        return None, None
     n_flush = len([k for k in range(3, K - 1) if k % 3 == 2])
     n_plain = (K - 1) - 3 - n_flush
-    return 1e6 * (first + first_flush + last + n_flush * flush + n_plain * plain) / (K - 1)
+    avg = 1e6 * (rows["first"] + rows["first_flush"] + rows["last"] + n_flush * rows["flush"] + n_plain * rows["plain"]) / (K - 1)
+    return avg, src
 
 
 class ClockSampler:
@@ -116,68 +128,74 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def workload_of(tag: str, device, rank: int, n_step_override: int):
-    from paper_2509_26309_b200 import workloads as W
-    ldos = tag.lower().endswith("ldos")
-    cfg = int(tag[0])
-    w = W.make_workload(cfg, device=device)
-    n_step = n_step_override or w.n_step
-    n_state = w.ldos_n_site if ldos else w.n_state
-    return w, cfg, ldos, n_state, n_step
+def default_block(cfg: int) -> int:
+    return {1: 256, 2: 64}.get(cfg, 8)
+
+
+def parse_tag(tag: str):
+    return int(tag[0]), tag.lower().endswith("ldos")
 
 
 # ---------------------------------------------------------------------------------------------------------------------
 # reference arm: the CPU oracle, as it stands, on a bounded sample of the same workload
 # ---------------------------------------------------------------------------------------------------------------------
-def oracle_sample(w, cfg_tag, seconds, steps=1, warmup=0):
+def oracle_sample(w, ldos, seconds, steps=1, warmup=0, serial=False):
     """Times oracle.propagate (OpenMP row form, all host cores) on ONE state of the workload for m time steps chosen so
-    that one sample takes about `seconds`.  Returns (value nnz*terms/s, ms per sample, description, cores)."""
+    that one sample takes about `seconds`.  Returns a dict (value nnz*terms/s, ms per sample, description, cores); with
+    serial=True also the single-thread hop-list form (the authoritative statement of PAPER.md:437-443) over one time step."""
     import numpy as np
     import oracle
     hi, hj, hv = w.hop_i.cpu().numpy(), w.hop_j.cpu().numpy(), w.hop_val.cpu().numpy()
     on = None if w.onsite is None else w.onsite.cpu().numpy()
-    if cfg_tag.endswith("ldos"):
+    if ldos:
         psi0 = np.zeros((1, w.n_orb), dtype=np.complex128)
         psi0[0, int(w.sites()[0])] = 1.0
     else:
         psi0 = w.psi0(device="cpu", n_state=1).numpy()
     K = len(oracle.cheb_coeff(w.rescale * w.dt))
-    rowptr, col, val = oracle.build_csr(w.n_orb, on, hi, hj, hv)          # (re-built inside propagate; this one sizes nnz)
-    nnz = int(rowptr[-1])
+    nnz = w.nnz
 
-    def one(m):
+    def one(m, form="csr"):
         t0 = time.perf_counter()
-        corr, norm2 = oracle.propagate(w.n_orb, on, hi, hj, hv, psi0, m, w.dt, w.rescale, form="csr")
-        return time.perf_counter() - t0, corr
+        oracle.propagate(w.n_orb, on, hi, hj, hv, psi0, m, w.dt, w.rescale, form=form)
+        return time.perf_counter() - t0
 
-    t1, _ = one(1)
-    m = max(1, min(int(seconds / max(t1, 1e-6)), 4096))
+    t1 = one(1)
+    t2 = one(2)
+    per_step = max(t2 - t1, 1e-6)                           # the CSR build inside propagate is in both
+    m = max(1, min(int((seconds - (t1 - per_step)) / per_step), 4096))
     times = []
     for it in range(warmup + steps):
-        t, corr = one(m)
+        t = one(m)
         if it >= warmup:
             times.append(t)
     t = max(times)
-    value = m * (K - 1) * nnz / t
-    return value, 1e3 * statistics.mean(times), f"1 state x {m} time steps ({m * (K - 1)} H-applications) of the full-size lattice, " \
-        f"oracle row form incl. its CSR build", oracle.num_threads()
+    out = {"value": m * (K - 1) * nnz / t, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+           "sample": f"1 state x {m} time steps ({m * (K - 1)} H-applications) of the full-size lattice, oracle row form incl. its CSR build",
+           "ms_per_sample": 1e3 * statistics.mean(times)}
+    if serial:
+        ts = one(1, form="hops")
+        out["serial_hop_form"] = {"value": (K - 1) * nnz / ts, "unit": UNIT, "cores": 1,
+                                  "sample": "1 state x 1 time step, single-thread hop-list form (oracle_propagate)"}
+    return out
 
 
 def main_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    import torch
-    from paper_2509_26309_b200 import workloads as W  # noqa: F401
-    w, cfg, ldos, n_state, n_step = workload_of(args.workload, "cpu", 0, args.n_step)
-    value, ms, sample, cores = oracle_sample(w, args.workload, args.cpu_seconds, steps=max(1, args.steps), warmup=min(args.warmup, 1))
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+    from paper_2509_26309_b200 import workloads as W
+    cfg, ldos = parse_tag(args.workload)
+    w = W.make_workload(cfg, device="cpu")
+    n_state = w.ldos_n_site if ldos else w.n_state
+    r = oracle_sample(w, ldos, args.cpu_seconds, steps=max(1, args.steps), warmup=min(args.warmup, 1))
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": r["ms_per_sample"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "complex128", "data": "synthetic",
-            "config": {"workload": w.name, "n_orb": w.n_orb, "nnz": w.nnz, "n_state": n_state, "n_step": n_step, "rescale": w.rescale,
-                       "tau": math.pi},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
-            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "config": {"workload": w.name + ("-ldos" if ldos else ""), "n_orb": w.n_orb, "nnz": w.nnz, "n_state": n_state, "n_step": w.n_step,
+                       "n_step_per_bench_step": args.block or default_block(cfg), "rescale": w.rescale, "tau": math.pi},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
     return 0
@@ -186,142 +204,206 @@ def main_reference(args):
 # ---------------------------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------------------------
+class Runner:
+    """One workload on one device: builds, propagates a block of time steps, reports rates and the roofline figures."""
+
+    def __init__(self, tag, dev, shard, block):
+        import torch
+        from paper_2509_26309_b200 import tbpm, workloads as W
+        self.torch, self.tbpm = torch, tbpm
+        self.cfg, self.ldos = parse_tag(tag)
+        self.dev = dev
+        self.w = w = W.make_workload(self.cfg, device=dev)
+        self.n_state = w.ldos_n_site if self.ldos else w.n_state
+        self.block = block or default_block(self.cfg)
+        # each rank propagates its own batch of seeded states (sub-streams shard.first_state ...); H is replicated
+        self.psi0 = None if self.ldos else w.psi0(device=dev, n_state=self.n_state, first_state=shard.first_state)
+        self.sites = W.ldos_sites(w.n_orb, self.n_state * shard.world)[shard.first_state: shard.first_state + self.n_state] if self.ldos else None
+        self.K = len(tbpm.tbpm_cheb_coeff(w.rescale * w.dt))
+        self.corr = torch.zeros((self.n_state, self.block), dtype=torch.complex128, device=dev)
+        self.norm2 = torch.zeros((self.n_state, self.block), dtype=torch.float64, device=dev)
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)          # > L2 (126 MB)
+        self.ws = None
+        self.H = None
+        self.name = w.name + ("-ldos" if self.ldos else "")
+
+    def step(self, ev=None):
+        torch, tbpm, w = self.torch, self.tbpm, self.w
+        self.flush.fill_(1)                                                # evict L2 between iterations (untimed)
+        if ev is not None:
+            ev[0].record()
+        H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val, 0)
+        if self.ws is None:
+            self.ws = torch.empty(tbpm.tbpm_propagate_bytes(H, self.n_state), dtype=torch.uint8, device=self.dev)
+        if ev is not None:
+            ev[1].record()
+        if self.ldos:
+            lc, ln, _ = tbpm.tbpm_ldos(H, self.sites, self.block, w.dt, w.rescale, workspace=self.ws)
+            self.corr.copy_(lc); self.norm2.copy_(ln)
+        else:
+            tbpm.tbpm_propagate(H, self.psi0, self.block, w.dt, w.rescale, workspace=self.ws, corr=self.corr, norm2=self.norm2)
+        if ev is not None:
+            ev[2].record()
+        self.H = H
+
+    def units_per_step(self):
+        return self.n_state * self.block * (self.K - 1) * self.H.nnz
+
+    def roofline(self, prop_ms_per_step, peak, peak_src):
+        """Algorithmic bytes (matrix as stored + 3 vectors) against the measured launch time of the fused term."""
+        H, w = self.H, self.w
+        tile = min(8, 1 << max(self.n_state - 1, 0).bit_length())
+        n_tile = -(-self.n_state // tile)
+        term_launches = n_tile * self.block * (self.K - 1)
+        avg_launch_s = prop_ms_per_step * 1e-3 / term_launches
+        bytes_tile = H.matrix_bytes_per_term + 48 * w.n_orb * min(tile, self.n_state)     # what ONE launch (one tile of states) must move
+        bytes_term_strict = H.matrix_bytes_per_term + 48 * w.n_orb * self.n_state          # one term for ALL states, matrix counted once
+        achieved_strict = bytes_term_strict / (avg_launch_s * n_tile) / 1e9
+        achieved_tile = bytes_tile / avg_launch_s / 1e9
+        traffic, tsrc = ncu_traffic(w.name, self.K)
+        lattice = self.cfg in (4, 5)
+        return {"bound": "hbm", "kernel": "k_term_rw (fused Chebyshev term, rolling window, term_rw.cu)" if lattice else
+                "k_term_ph (fused Chebyshev term, term_ph.cuh)",
+                "achieved": achieved_strict, "peak": peak, "unit": "GB/s", "frac": achieved_strict / peak,
+                "traffic": traffic, "traffic_source": tsrc, "peak_source": peak_src,
+                "bytes_per_launch": bytes_tile, "avg_launch_us": avg_launch_s * 1e6, "launches_per_step": term_launches,
+                "count": "strict: matrix_bytes_as_stored + 3*16*N*n_state once per term for all states (SURVEY 8(d)), over the time of "
+                         "the n_tile launches that make one term; *_per_tile counts the matrix once per launch (one tile of <= 8 states)",
+                "achieved_per_tile": achieved_tile, "frac_per_tile": achieved_tile / peak, "n_tile": n_tile,
+                "frac_of_nominal_8000": achieved_strict / 8000.0,
+                "note": "avg launch = CUDA-event time of tbpm_propagate / term launches (includes the <1% of tiny kernels)"}
+
+
+def timed_steps(r, n, barrier):
+    torch = r.torch
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(n)]
+    for i in range(n):
+        r.step(evs[i])
+    barrier()
+    step_ms = [e[0].elapsed_time(e[2]) for e in evs]                      # device time, build + propagate
+    prop_ms = [e[1].elapsed_time(e[2]) for e in evs]
+    return sum(step_ms), sum(prop_ms)
+
+
 def main_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2509_26309_b200 import tbpm
+    from paper_2509_26309_b200 import tbpm, replicas
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = replicas.env_rank_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the TBPM path has no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-
-    w, cfg, ldos, n_state, n_step = workload_of(args.workload, dev, rank, args.n_step)
-    # each rank propagates its own batch of seeded states (sub-streams rank*n_state ...); H is replicated
-    psi0 = None if ldos else w.psi0(device=dev, n_state=n_state, first_state=rank * n_state)
-    sites = w.sites() if ldos else None
-    K = len(tbpm.tbpm_cheb_coeff(w.rescale * w.dt))
-    flags = 0
-
-    pb, sb = tbpm.tbpm_build_bytes(w.n_orb, w.n_hop, w.onsite is not None, flags)
-    corr = torch.zeros((n_state, n_step), dtype=torch.complex128, device=dev)
-    norm2 = torch.zeros((n_state, n_step), dtype=torch.float64, device=dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)          # > L2 (126 MB)
-    state = {}
-
-    def one_step(timers=None):
-        flush.fill_(1)                                                     # evict L2 between iterations (untimed)
-        if timers is not None:
-            timers[0].record()
-        H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val, flags)
-        if "ws" not in state:
-            state["ws"] = torch.empty(tbpm.tbpm_propagate_bytes(H, n_state), dtype=torch.uint8, device=dev)
-        if timers is not None:
-            timers[1].record()
-        if ldos:
-            lc, ln, _ = tbpm.tbpm_ldos(H, sites, n_step, w.dt, w.rescale, workspace=state["ws"])
-            corr.copy_(lc); norm2.copy_(ln)
-        else:
-            tbpm.tbpm_propagate(H, psi0, n_step, w.dt, w.rescale, workspace=state["ws"], corr=corr, norm2=norm2)
-        if timers is not None:
-            timers[2].record()
-        state["H"] = H
-        return H
+    peak, peak_src = load_peaks()
 
     def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(dev)
 
+    cfg, ldos = parse_tag(args.workload)
+    probe_n_state = None
+
+    def make(tag, block):
+        from paper_2509_26309_b200 import workloads as W
+        c, l = parse_tag(tag)
+        n_state = W._FULL[c].get("ldos", 0) if l else W._FULL[c]["n_state"]
+        return Runner(tag, dev, replicas.weak_shard(n_state, rank, world), block)
+
+    r = make(args.workload, args.block)
     for _ in range(max(args.warmup, 0)):
-        one_step()
+        r.step()
     barrier()
     launches0 = tbpm.tbpm_total_launch_count()
     sampler = ClockSampler(local) if rank == 0 else None
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
-    for i in range(args.steps):
-        one_step(evs[i])
-    barrier()
+    total_ms, prop_ms = timed_steps(r, args.steps, barrier)
     clocks = sampler.stop() if sampler else None
     launches = tbpm.tbpm_total_launch_count() - launches0
-    step_ms = [e[0].elapsed_time(e[2]) for e in evs]                      # device time, build + propagate
-    prop_ms = [e[1].elapsed_time(e[2]) for e in evs]
-    total_ms = sum(step_ms)
-    t = torch.tensor([total_ms, sum(prop_ms)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, prop_total_ms = float(t[0]), float(t[1])
-    H = state["H"]
-    nnz = H.nnz
-    happs = n_state * n_step * (K - 1)
-    value = world * args.steps * happs * nnz / (total_ms * 1e-3)
-    norm_dev = float((norm2 - 1).abs().max())
-
-    # roofline of the dominant kernel (the fused Chebyshev term): algorithmic bytes per launch = matrix as stored + 3 vectors
-    # of the tile the launch processes; average launch duration = propagate time / number of term launches
-    tile = min(8, 1 << (n_state - 1).bit_length()) if not os.environ.get("TBPM_TILE") else int(os.environ["TBPM_TILE"])
-    n_tile = -(-n_state // tile)
-    term_launches = n_tile * n_step * (K - 1)
-    avg_term_s = (prop_total_ms * 1e-3 / args.steps) / term_launches
-    bytes_per_launch = H.matrix_bytes_per_term + 3 * 16 * w.n_orb * min(tile, n_state)
-    peak, peak_src = load_peaks()
-    achieved = bytes_per_launch / avg_term_s / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_term_ph (fused Chebyshev term, term_ph.cuh)", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(w.name, K), "traffic_source": NCU_TRAFFIC_SRC,
-                "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
-                "avg_launch_us": avg_term_s * 1e6, "launches_per_step": term_launches,
-                "counted_csr_gbs": (8 * (w.n_orb + 1) + 20 * nnz + 48 * w.n_orb * min(tile, n_state)) / avg_term_s / 1e9,
-                "frac_of_nominal_8000": achieved / 8000.0,
-                "note": "avg launch = CUDA-event time of tbpm_propagate / term launches (includes the <1% of tiny kernels)"}
+    total_ms, prop_ms = replicas.max_over_ranks([total_ms, prop_ms], dev)
+    value = replicas.whole_job_rate(args.steps * r.units_per_step(), total_ms * 1e-3, dev)
+    norm_dev = replicas.max_over_ranks([float((r.norm2 - 1).abs().max())], dev)[0]
+    all_corr = replicas.gather_corr(r.corr, replicas.weak_shard(r.n_state, rank, world))
+    gathered_ok = None
+    if rank == 0:
+        gathered_ok = bool(all_corr is not None and tuple(all_corr.shape) == (world * r.n_state, r.block) and
+                           bool(torch.isfinite(torch.view_as_real(all_corr)).all()))
+    w, H = r.w, r.H
+    roofline = r.roofline(prop_ms / args.steps, peak, peak_src)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "complex128", "data": "synthetic",
-            "config": {"workload": w.name, "n_orb": w.n_orb, "nnz": nnz, "n_state": n_state, "n_step": n_step, "K": K, "rescale": w.rescale,
-                       "tau": math.pi, "tile": tile, "n_table": H.n_table, "matrix_bytes_per_term": H.matrix_bytes_per_term,
+            "config": {"workload": r.name, "n_orb": w.n_orb, "nnz": H.nnz, "n_state": r.n_state, "n_step": w.n_step,
+                       "n_step_per_bench_step": r.block, "K": r.K, "rescale": w.rescale, "tau": math.pi, "tile": 8, "n_table": H.n_table,
+                       "matrix_bytes_per_term": H.matrix_bytes_per_term,
                        "l2": "256 MB flush between iterations; working set > L2", "ldos": ldos,
-                       "parallelism": f"replicas x{world}: each rank its own {n_state} states"},
-            "ms_build": sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps, "ms_propagate": prop_total_ms / args.steps,
-            "h_apps_per_s": world * args.steps * happs / (total_ms * 1e-3), "ms_per_time_step": prop_total_ms / args.steps / n_step,
-            "max_norm_dev": norm_dev, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
-    if args.n_step:
-        line["config"]["n_step_override"] = args.n_step
+                       "parallelism": f"replicas x{world}: each rank its own {r.n_state} states (paper_2509_26309_b200/replicas.py)"},
+            "ms_build": (total_ms - prop_ms) / args.steps, "ms_propagate": prop_ms / args.steps,
+            "h_apps_per_s": value / H.nnz, "ms_per_time_step": prop_ms / args.steps / r.block,
+            "max_norm_dev": norm_dev, "norm_ok": bool(norm_dev <= 1e-12), "gathered_corr_ok": gathered_ok,
+            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
 
     # end to end through the C ABI with HOST buffers: H2D of the hop list and psi0, build, propagate, D2H of corr/norm2
     if not args.no_e2e and not ldos:
         hw = {k: getattr(w, k).cpu().pin_memory() for k in ("hop_i", "hop_j", "hop_val")}
         hon = None if w.onsite is None else w.onsite.cpu().pin_memory()
-        hpsi = psi0.cpu().pin_memory()
-        hcorr = torch.zeros((n_state, n_step), dtype=torch.complex128).pin_memory()
-        hnorm = torch.zeros((n_state, n_step), dtype=torch.float64).pin_memory()
-        state.clear()
-        arena = torch.empty(tbpm.tbpm_corr_host_bytes(w.n_orb, w.n_hop, hon is not None, n_state, n_step, flags), dtype=torch.uint8, device=dev)
+        hpsi = r.psi0.cpu().pin_memory()
+        hcorr = torch.zeros((r.n_state, r.block), dtype=torch.complex128).pin_memory()
+        hnorm = torch.zeros((r.n_state, r.block), dtype=torch.float64).pin_memory()
+        dev_corr = r.corr.clone()
+        r.ws = None                                                        # the arena below holds its own workspace
+        torch.cuda.empty_cache()
+        arena = torch.empty(tbpm.tbpm_corr_host_bytes(w.n_orb, w.n_hop, hon is not None, r.n_state, r.block, 0), dtype=torch.uint8, device=dev)
         up = down = 0
         e2e_t = []
-        for i in range(1 + max(1, min(args.steps, 2))):
+        for i in range(1 + max(1, min(args.steps, 3))):
             barrier()
             t0 = time.perf_counter()
-            up, down = tbpm.tbpm_corr_host(w.n_orb, hon, hw["hop_i"], hw["hop_j"], hw["hop_val"], hpsi, n_step, w.dt, w.rescale, arena,
-                                           hcorr, hnorm, flags)
+            up, down = tbpm.tbpm_corr_host(w.n_orb, hon, hw["hop_i"], hw["hop_j"], hw["hop_val"], hpsi, r.block, w.dt, w.rescale, arena,
+                                           hcorr, hnorm, 0)
             if i > 0:
                 e2e_t.append(time.perf_counter() - t0)
-        te = torch.tensor([sum(e2e_t)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        line["e2e"] = {"value": world * len(e2e_t) * happs * nnz / float(te[0]), "unit": UNIT, "h2d_bytes_per_step": int(up),
-                       "d2h_bytes_per_step": int(down), "ms_per_step": 1e3 * float(te[0]) / len(e2e_t),
-                       "max_abs_diff_vs_device_path": float((hcorr.to(dev) - corr).abs().max())}
-        del arena
+        te = replicas.max_over_ranks([sum(e2e_t)], dev)[0]
+        line["e2e"] = {"value": replicas.sum_over_ranks([len(e2e_t) * r.units_per_step()], dev)[0] / te, "unit": UNIT,
+                       "h2d_bytes_per_step": int(up), "d2h_bytes_per_step": int(down), "ms_per_step": 1e3 * te / len(e2e_t),
+                       "max_abs_diff_vs_device_path": float((hcorr.to(dev) - dev_corr).abs().max()),
+                       "api": "tbpm_corr_host: pinned host hop list + psi0 -> H2D, build, propagate, D2H of corr/norm2"}
+        del arena, hpsi, hw
+
+    # the other >= 16 M-orbital workloads, in the same process, for >= per_workload_seconds each (sustained clocks)
+    if world == 1 and not args.no_per_workload and args.workload == "5":
+        per = [{"workload": r.name, "value": value, "frac": roofline["frac"], "frac_per_tile": roofline["frac_per_tile"],
+                "avg_launch_us": roofline["avg_launch_us"], "clocks": clocks, "max_norm_dev": norm_dev,
+                "seconds": total_ms * 1e-3, "n_step_per_bench_step": r.block}]
+        del r
+        torch.cuda.empty_cache()
+        for tag in ("3", "4", "5ldos"):
+            q = make(tag, args.block)
+            for _ in range(3):
+                q.step()
+            barrier()
+            smp = ClockSampler(local)
+            tot = prp = 0.0
+            n = 0
+            while tot * 1e-3 < args.per_workload_seconds:
+                a, b = timed_steps(q, 2, barrier)
+                tot += a; prp += b; n += 2
+            ck = smp.stop()
+            rf = q.roofline(prp / n, peak, peak_src)
+            nd = float((q.norm2 - 1).abs().max())
+            per.append({"workload": q.name, "value": n * q.units_per_step() / (tot * 1e-3), "frac": rf["frac"], "frac_per_tile": rf["frac_per_tile"],
+                        "avg_launch_us": rf["avg_launch_us"], "bytes_per_launch": rf["bytes_per_launch"], "kernel": rf["kernel"],
+                        "traffic": rf["traffic"], "clocks": ck, "max_norm_dev": nd, "norm_ok": bool(nd <= 1e-12),
+                        "seconds": tot * 1e-3, "n_step_per_bench_step": q.block})
+            del q
+            torch.cuda.empty_cache()
+        line["per_workload"] = per
 
     if rank == 0 and not args.no_cpu_baseline:
-        v, ms, sample, cores = oracle_sample(w, args.workload, args.cpu_seconds)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        from paper_2509_26309_b200 import workloads as W
+        wc = W.make_workload(cfg, device="cpu")
+        line["cpu_baseline"] = oracle_sample(wc, ldos, args.cpu_seconds, serial=True)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

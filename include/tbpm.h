@@ -38,18 +38,20 @@ typedef struct tbpm_ham tbpm_ham; /* opaque host handle pointing into caller-own
 /* error codes */
 #define TBPM_OK 0
 #define TBPM_EINVAL (-1)  /* NULL / negative / misaligned argument, n_orb >= 2^31, rescale <= 0, ...                 */
-#define TBPM_EINDEX (-2)  /* hop index out of [0, n_orb)                                   (TBPM_VALIDATE only)      */
+#define TBPM_EINDEX (-2)  /* hop, site or state index out of range                                                    */
 #define TBPM_EDIAG (-3)   /* hop with i == j: illegal, on-site energy is an orbital attribute    */
 #define TBPM_EDUP (-4)    /* the same (row, col) produced twice (the paper's dict-update semantic, PAPER.md:190-191,
-                             has no meaning for a flat list; SURVEY reading #15)          (TBPM_VALIDATE only)      */
+                             has no meaning for a flat list; SURVEY reading #15)                                     */
 #define TBPM_ENOMEM (-5)  /* a caller-provided buffer is too small                                                   */
 #define TBPM_ECUDA (-6)   /* CUDA runtime error (no device, launch failure, sticky error)                            */
 #define TBPM_EBOUND (-7)  /* Gershgorin bound max_i(|onsite_i| + sum_j |H_ij|) > rescale (strictly): the Chebyshev
                              recursion would diverge.  Returned by tbpm_check_bound only; never fatal elsewhere.     */
 
 /* flags of tbpm_build */
-#define TBPM_VALIDATE 1u    /* run the precondition checks (index range, i != j, duplicates); following the paper's
-                               "bugs vs exceptions" split they are off by default         */
+#define TBPM_VALIDATE 1u    /* accepted and ignored: the precondition checks (index range, i != j, duplicates) ride on
+                               kernels that run anyway and are reported through the status word that tbpm_build has to
+                               read back for the table size, so they are ALWAYS on (the paper's "bugs vs exceptions"
+                               split, would make them optional)                             */
 #define TBPM_HOPS_FULL 2u   /* the list already holds both orientations of every pair (default: each pair once and
                                the conjugate partner H_ji = conj(H_ij) is generated)                    */
 #define TBPM_NO_TABLE 4u    /* keep complex128 values in the kernel layout instead of 16-bit indices into a table of
@@ -93,9 +95,21 @@ int tbpm_check_bound(const tbpm_ham *H, double rescale);
 /* Canonical CSR in caller order, copied device -> device: rowptr int64[n_orb+1], col int32[nnz], val [nnz][2]. */
 int tbpm_export_csr(const tbpm_ham *H, int64_t *rowptr, int32_t *col, double *val, void *stream);
 
-void tbpm_free(tbpm_ham *H); /* frees only the host struct */
+/* Frees only the host struct (PAPER.md has no counterpart: its solver holds `const model_t*`).  Work
+ * enqueued on the handle must have completed. */
+void tbpm_free(tbpm_ham *H);
 
-/* ---- a2-a7: propagate ------------------------------------------------------------------------------------------------ */
+/* Options of a handle; set before tbpm_propagate_bytes / tbpm_propagate / tbpm_ldos (the workspace size depends on
+ * TBPM_OPT_TILE).  The library reads nothing from the environment: its behaviour is a function of its arguments. */
+#define TBPM_OPT_TILE 1   /* states propagated together per tile (SpMM width, PAPER.md:554 runs one state at a time):
+                             1, 2, 4, 8 (default: 8 interleaved complex128 = one 128-byte line per row), 16, 32        */
+#define TBPM_OPT_KERNEL 2 /* 0 (default): the fastest kernel that applies (rolling-window on lattices, else phased, else
+                             general); 1: every term on the general kernel; 2: no rolling-window kernel                */
+int tbpm_set_option(tbpm_ham *H, int option, int64_t value);
+
+/* ---- a2-a7: propagate ------------------------------------------------------------------------------------------------
+ * Size of the caller-owned `workspace` for n_state states: four vectors [n_orb][tile] complex128 per tile of states (the
+ * rotating p0 / p1 / wf_out of PAPER.md:437-443 and the bra psi0 of calc_corr_dos) + block partials. */
 int tbpm_propagate_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes);
 
 /* psi0: device [n_state][n_orb][2], state-major (one random initial state per row; one independent propagation per
@@ -103,19 +117,24 @@ int tbpm_propagate_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes
  * not stored).  norm2: device out [n_state][n_step] or NULL.  rescale = s > 0 must bound the spectrum, ||H|| <= s
  * (config.rescale).  n_step == 0 or n_state == 0: success, outputs untouched.  Asynchronous on `stream`.
  * Deterministic: the same inputs give bit-identical outputs, and the first m entries do not depend on n_step. */
-int tbpm_propagate(const tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale,
+int tbpm_propagate(tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale,
                    double *corr, double *norm2, void *workspace, size_t workspace_bytes, void *stream);
 
-/* ---- a8: TBPM-style LDOS correlation: psi0_b = e_{sites[b]}, corr[b][n] = <site_b| psi_b(t_n) > -------------------- */
-int tbpm_ldos(const tbpm_ham *H, const int64_t *sites /* host [n_site] */, int n_site, int n_step, double dt,
+/* ---- a8: TBPM-style LDOS correlation: psi0_b = e_{sites[b]}, corr[b][n] = <site_b| psi_b(t_n) > ----------------------
+ * BASELINE.json:configs[4] ("LDOS correlation on 64 seeded site-localized initial states"); the paper's own LDOS is the
+ * Haydock recursion, see tbpm_haydock below.  Same kernels as tbpm_propagate with unit initial vectors. */
+int tbpm_ldos(tbpm_ham *H, const int64_t *sites /* host [n_site] */, int n_site, int n_step, double dt,
               double rescale, double *corr, double *norm2, void *workspace, size_t workspace_bytes, void *stream);
 
-/* State `state` as left in `workspace` by the last tbpm_propagate / tbpm_ldos call on it (psi after its n_step steps),
- * caller order, device out [n_orb][2].  A snapshot at step j is a call with n_step = j. */
+/* State `state` as left in `workspace` by the last tbpm_propagate / tbpm_ldos call of THIS handle on it (psi after its
+ * n_step steps), caller order, device out [n_orb][2].  A snapshot at step j is a call with n_step = j: this is the
+ * time-dependent wave function psi(t_j) the paper's solver can dump (WFT, Table 7), and
+ * what the windowed parity protocol of SURVEY.md 8(d)(3) downloads.  TBPM_EINVAL if the handle has not propagated on
+ * that workspace, TBPM_EINDEX if state >= the n_state of that call. */
 int tbpm_get_state(const tbpm_ham *H, const void *workspace, int state, double *psi_out, void *stream);
 
-/* Number of kernels the last tbpm_propagate / tbpm_ldos call launched (host counter kept in the handle's library). */
-int64_t tbpm_last_launch_count(void);
+/* Number of kernels the last tbpm_propagate / tbpm_ldos call on this handle launched (host counter kept in the handle). */
+int64_t tbpm_last_launch_count(const tbpm_ham *H);
 /* Kernels launched by this library in this process since it was loaded (build + propagate + get_state). */
 int64_t tbpm_total_launch_count(void);
 

@@ -23,8 +23,9 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile every csrc/*.cu to an object file (in parallel) and link libtbpm.so."""
+def build(force: bool = False, verbose: bool = False, experiment: bool = False) -> str:
+    """Compile every csrc/*.cu to an object file (in parallel) and link libtbpm.so.  experiment=True adds -DTBPM_EXPERIMENT
+    (run-time tuning knobs for sweeps; tbpm_version() then ends in "+exp"); the product build has no such knobs."""
     if not force and not needs_build():
         return LIB
     from concurrent.futures import ThreadPoolExecutor
@@ -32,6 +33,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
     if verbose:
         flags = flags + ["-Xptxas=-v"]
+    if experiment:
+        flags = flags + ["-DTBPM_EXPERIMENT"]
     objdir = os.path.join(_DIR, "build")
     os.makedirs(objdir, exist_ok=True)
     hdrs = glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(_DIR, "..", "include", "tbpm.h")]
@@ -51,4 +54,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv, experiment="--experiment" in sys.argv))

@@ -3,7 +3,7 @@
 #include <cstdio>
 #include <cstring>
 
-#include "tbpm_internal.h"
+#include "term.h"
 
 using namespace tbpm_detail;
 
@@ -18,6 +18,47 @@ void tbpm_detail::note_cuda_error(cudaError_t e)
 }
 
 void tbpm_detail::count_launches(int n) { g_total_launches.fetch_add(n, std::memory_order_relaxed); }
+long long tbpm_detail::total_launches() { return g_total_launches.load(std::memory_order_relaxed); }
+
+#ifdef TBPM_EXPERIMENT
+// Experiment build only: a process-wide table of tuning knobs, set through tbpm_set_knob (not part of include/tbpm.h).
+namespace {
+struct KnobEntry { char name[32]; int value; };
+KnobEntry g_knobs[64];
+int g_n_knobs = 0;
+}
+int tbpm_detail::knob(const char *name, int dflt)
+{
+    for (int i = 0; i < g_n_knobs; ++i)
+        if (std::strcmp(g_knobs[i].name, name) == 0) return g_knobs[i].value;
+    return dflt;
+}
+extern "C" void tbpm_clear_knobs(void) { g_n_knobs = 0; }
+extern "C" int tbpm_set_knob(const char *name, int value)
+{
+    if (!name || std::strlen(name) >= sizeof(g_knobs[0].name)) return TBPM_EINVAL;
+    for (int i = 0; i < g_n_knobs; ++i)
+        if (std::strcmp(g_knobs[i].name, name) == 0) { g_knobs[i].value = value; return TBPM_OK; }
+    if (g_n_knobs >= 64) return TBPM_ENOMEM;
+    std::strcpy(g_knobs[g_n_knobs].name, name);
+    g_knobs[g_n_knobs++].value = value;
+    return TBPM_OK;
+}
+#endif
+
+// Does the phased kernel have an instantiation for this term whose stages fit one SM?  (see term.h)
+bool tbpm_detail::term_ph_supported(int bt, const TermParams &p)
+{
+    if (p.n_table <= 0 || (p.flags & F_SKIP_H)) return false;
+    if (bt != 1 && bt != 2 && bt != 4 && bt != 8) return false;
+    const bool red = p.flags & F_REDUCE, wy = p.flags & F_WRITE_Y;
+    if (red == wy) return false;
+    if (!red && !(p.n_acc == 0 || p.n_acc == 3)) return false;
+    if (red && (p.n_acc < 1 || p.n_acc > 3)) return false;
+    const int lanes_per_row = bt >= 2 ? bt / 2 : 1;        // threads hold two states of a row (one at bt = 1)
+    const int rows_max = 31 * 32 / lanes_per_row;          // the widest tile any shape of this width uses
+    return 2 * (size_t)stage_geom(rows_max, p.max_row_off, true).stage_bytes <= kStageBudget;
+}
 
 extern "C" int64_t tbpm_total_launch_count(void) { return (int64_t)g_total_launches.load(std::memory_order_relaxed); }
 
@@ -36,7 +77,14 @@ extern "C" const char *tbpm_strerror(int code)
     return "unknown error code";
 }
 
-extern "C" const char *tbpm_version(void) { return "tbpm-b200 0.1 (sm_100a)"; }
+extern "C" const char *tbpm_version(void)
+{
+#ifdef TBPM_EXPERIMENT
+    return "tbpm-b200 0.2 (sm_100a) +exp";
+#else
+    return "tbpm-b200 0.2 (sm_100a)";
+#endif
+}
 
 namespace {
 
@@ -50,7 +98,7 @@ int arena_layout(int64_t n_orb, int64_t n_hop, int has_onsite, int n_state, int 
     if (n_state < 0 || n_step < 0) return TBPM_EINVAL;
     int rc = tbpm_build_bytes(n_orb, n_hop, has_onsite, flags, &A->persist_bytes, &A->scratch_bytes);
     if (rc) return rc;
-    tbpm_ham tmp;                                        // only n_orb matters for the workspace size
+    tbpm_ham tmp;                                        // only n_orb (and the default options) matter for the workspace size
     tmp.n_orb = n_orb;
     if ((rc = tbpm_propagate_bytes(&tmp, n_state, &A->workspace_bytes))) return rc;
     size_t o = 0;

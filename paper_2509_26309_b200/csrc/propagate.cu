@@ -22,6 +22,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 #include <vector>
 
 #include "term.h"
@@ -33,17 +34,6 @@ namespace {
 constexpr int kThreads = 256;
 constexpr size_t kHeaderBytes = 256;
 constexpr size_t kPartialBytes = sizeof(double) * 3 * kMaxBT * kMaxGrid;
-
-thread_local int64_t g_launches = 0;
-
-struct WsHeader {          // first bytes of the workspace; read by tbpm_get_state's kernel
-    int64_t n_orb;
-    int32_t n_state;
-    int32_t tile;          // states per full tile
-    int64_t vec0_off;      // byte offset of the first tile's buffers
-    int32_t final_slot;    // which of the three rotating buffers holds psi
-    int32_t pad;
-};
 
 __device__ __forceinline__ double2 ld_stream(const double2 *p) { return __ldcs(p); }     // read once: evict first
 __device__ __forceinline__ void st_stream(double2 *p, double2 v) { __stcs(p, v); }
@@ -213,37 +203,16 @@ __global__ void k_unit_states(const int64_t *__restrict__ sites, int state0, int
     bra[at] = make_double2(1.0, 0.0);
 }
 
-__global__ void k_write_header(WsHeader *h, WsHeader v) { *h = v; }
-
-__global__ void k_get_state(const char *ws, int state, double2 *out)
+// tbpm_get_state: one state of a tile buffer [row][bt] -> caller order
+__global__ void k_get_state(const double2 *__restrict__ psi, int64_t n_orb, int bt, int b, double2 *out)
 {
-    const WsHeader h = *reinterpret_cast<const WsHeader *>(ws);
-    const int tile = state / h.tile;
-    const int n_rest = h.n_state - tile * h.tile;
-    int bt = h.tile;
-    if (n_rest < h.tile) { bt = 1; while (bt < n_rest) bt <<= 1; }
-    const size_t full_vec = ((size_t)h.n_orb * h.tile * sizeof(double2) + kAlign - 1) / kAlign * kAlign;
-    const size_t this_vec = ((size_t)h.n_orb * bt * sizeof(double2) + kAlign - 1) / kAlign * kAlign;
-    const char *base = ws + h.vec0_off + (size_t)tile * 4 * full_vec + (size_t)h.final_slot * this_vec;
-    const double2 *psi = reinterpret_cast<const double2 *>(base);
-    const int b = state - tile * h.tile;
-    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < h.n_orb; row += (int64_t)gridDim.x * blockDim.x)
+    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n_orb; row += (int64_t)gridDim.x * blockDim.x)
         out[row] = psi[row * bt + b];
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------------------
-int tile_max()
-{
-    int t = 8;                                           // default: 8 states = one 128-byte line per row
-    if (const char *e = std::getenv("TBPM_TILE")) {
-        int v = std::atoi(e);
-        if (v == 1 || v == 2 || v == 4 || v == 8 || v == 16 || v == 32) t = v;
-    }
-    return t;
-}
-
 int pow2_ceil(int n)
 {
     int p = 1;
@@ -259,10 +228,10 @@ struct Plan {
     size_t sites_off, partial_off, vec0_off, total;
 };
 
-Plan make_plan(int64_t n_orb, int n_state)
+Plan make_plan(int64_t n_orb, int n_state, int tile_max)
 {
     Plan P{};
-    P.tile = std::min(tile_max(), pow2_ceil(std::max(n_state, 1)));
+    P.tile = std::min(tile_max, pow2_ceil(std::max(n_state, 1)));
     P.n_tile = (std::max(n_state, 1) + P.tile - 1) / P.tile;
     const int rest = std::max(n_state, 1) - (P.n_tile - 1) * P.tile;
     P.last_bt = pow2_ceil(rest);
@@ -278,56 +247,35 @@ Plan make_plan(int64_t n_orb, int n_state)
     return P;
 }
 
-int min_blocks()
-{
-    int m = 4;
-    if (const char *e = std::getenv("TBPM_MINB")) {
-        int v = std::atoi(e);
-        if (v == 3 || v == 4 || v == 6 || v == 8) m = v;
-    }
-    return m;
-}
-
-template <int BT, bool TABLE, int MINB>
+template <int BT, bool TABLE>
 int launch_term_t(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
-    static int blocks_per_sm = 0;
-    if (blocks_per_sm == 0) {
+    static int blocks_per_sm[kMaxDevices] = {0};           // per device
+    if (p.device < 0 || p.device >= kMaxDevices) return TBPM_EINVAL;
+    if (blocks_per_sm[p.device] == 0) {
         int nb = 0;
-        TBPM_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_cheb_term<BT, TABLE, MINB>, kThreads, 0));
-        blocks_per_sm = std::max(nb, 1);
+        TBPM_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_cheb_term<BT, TABLE, 4>, kThreads, 0));
+        blocks_per_sm[p.device] = std::max(nb, 1);
     }
     constexpr int kRowsPerBlock = kThreads / BT;
     const int64_t need = (p.n_orb + kRowsPerBlock - 1) / kRowsPerBlock;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>({need, (int64_t)num_sms * blocks_per_sm, (int64_t)kMaxGrid}));
-    k_cheb_term<BT, TABLE, MINB><<<grid, kThreads, 0, st>>>(p);
-    ++g_launches; count_launches(1);
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>({need, (int64_t)num_sms * blocks_per_sm[p.device], (int64_t)kMaxGrid}));
+    k_cheb_term<BT, TABLE, 4><<<grid, kThreads, 0, st>>>(p);
+    count_launches(1);
     *grid_out = grid;
     return TBPM_OK;
 }
 
-template <int BT, bool TABLE>
-int launch_term_m(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
+// One Chebyshev term.  Lattices with tiles of 8 states run on the rolling-window kernel (term_rw.cu) when their strides
+// allow it (TBPM_OPT_KERNEL = 2 turns that off).  The phased kernel (term_ph.cuh) runs whenever it has an instantiation for the term and its stages
+// fit (kernel layout with a value table, tiles of 1-8 states, rows of up to a few dozen entries); everything else -- no
+// table, tiles of 16 / 32 states, long rows, tau = 0 -- and every term under TBPM_OPT_KERNEL = 1 runs on the general
+// kernel k_cheb_term.
+int launch_term(int bt, bool table, int kernel_opt, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
-    switch (min_blocks()) {
-    case 3: return launch_term_t<BT, TABLE, 3>(p, num_sms, st, grid_out);
-    case 6: return launch_term_t<BT, TABLE, 6>(p, num_sms, st, grid_out);
-    case 8: return launch_term_t<BT, TABLE, 8>(p, num_sms, st, grid_out);
-    default: return launch_term_t<BT, TABLE, 4>(p, num_sms, st, grid_out);
-    }
-}
-
-
-int launch_term(int bt, bool table, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
-{
-    // phased kernel (term_ph.cuh) whenever it has an instantiation for this term; TBPM_KERNEL=0: the earlier
-    // warp-specialised kernel with staged vectors (term_ws.cu); else the direct kernel below
-    if (table && term_sg_supported(bt, p)) {               // vector rows staged in shared memory (uniform lattices, 8 states)
-        ++g_launches;
-        return launch_term_sg(p, num_sms, st, grid_out);
-    }
-    if (table && env_int("TBPM_KERNEL", 1) != 0 && term_ph_supported(bt, p)) {
-        ++g_launches;
+    const bool general_only = kernel_opt == 1;
+    if (table && kernel_opt == 0 && term_rw_supported(bt, p)) return launch_term_rw(p, num_sms, st, grid_out);
+    if (table && !general_only && term_ph_supported(bt, p)) {
         switch (bt) {
         case 1: return launch_term_ph_bt1(p, num_sms, st, grid_out);
         case 2: return launch_term_ph_bt2(p, num_sms, st, grid_out);
@@ -335,13 +283,9 @@ int launch_term(int bt, bool table, const TermParams &p, int num_sms, cudaStream
         case 8: return launch_term_ph_bt8(p, num_sms, st, grid_out);
         }
     }
-    if (table && term_ws_supported(bt, p)) {
-        ++g_launches;
-        return launch_term_ws(bt, p, num_sms, st, grid_out);
-    }
 #define TBPM_CASE(B)                                                                     \
     case B:                                                                              \
-        return table ? launch_term_m<B, true>(p, num_sms, st, grid_out) : launch_term_m<B, false>(p, num_sms, st, grid_out);
+        return table ? launch_term_t<B, true>(p, num_sms, st, grid_out) : launch_term_t<B, false>(p, num_sms, st, grid_out);
     switch (bt) {
         TBPM_CASE(1)
         TBPM_CASE(2)
@@ -354,21 +298,54 @@ int launch_term(int bt, bool table, const TermParams &p, int num_sms, cudaStream
     return TBPM_EINVAL;
 }
 
+// Launch parameters of the K - 1 Chebyshev terms of one time step (psi in `psi`, scratch `t1`, psi' built in `acc`).
+// T_k overwrites T_{k-2}: T_0 = psi, T_1 -> t1, T_2 -> psi's buffer, ...; psi' is touched on every third term and on
+// the last one, which also carries the reduction and does not store T_{K-1} (it is never read again).
+void step_terms(const TermParams &base, int K, const std::vector<double> &cf, double rescale, bool reverse_odd, double2 *psi,
+                double2 *t1, double2 *acc, std::vector<TermParams> &term)
+{
+    auto C = [&](int k) { return make_double2(cf[2 * k], cf[2 * k + 1]); };
+    term.assign((size_t)K, base);
+    int flushed = -1;                                     // highest term already added to psi'
+    for (int k = 1; k < K; ++k) {
+        TermParams &tp = term[k];
+        tp.x = (k % 2 == 1) ? psi : t1;                   // T_{k-1}
+        tp.y = (k % 2 == 1) ? t1 : psi;                   // T_{k-2} -> T_k
+        tp.acc = acc;
+        tp.a = (k == 1 ? 1.0 : 2.0) / rescale;
+        int flags = F_WRITE_Y | (k >= 2 ? F_SUB_Y : 0);
+        const bool last = (k == K - 1);
+        tp.n_acc = 0;
+        if (k % 3 == 2 || last) {                         // flush terms flushed+1 .. k (at most 3)
+            tp.n_acc = k - flushed;
+            tp.ca = C(k);
+            tp.cb = tp.n_acc >= 2 ? C(k - 1) : make_double2(0.0, 0.0);
+            tp.cc = tp.n_acc == 3 ? C(k - 2) : make_double2(0.0, 0.0);
+            if (flushed < 0) flags |= F_ACC_INIT;
+            flushed = k;
+        }
+        if (last) { flags |= F_REDUCE; flags &= ~F_WRITE_Y; }
+        tp.flags = flags;
+        tp.reverse = reverse_odd ? (k & 1) : 0;
+        if (tp.reverse) tp.pf_lead = -tp.pf_lead;
+    }
+}
+
 // Shared body of tbpm_propagate (psi0 != NULL) and tbpm_ldos (sites != NULL).
-int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int n_step, double dt, double rescale, double *corr,
+int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int n_step, double dt, double rescale, double *corr,
         double *norm2, void *workspace, size_t workspace_bytes, void *stream)
 {
     if (!H || n_state < 0 || n_step < 0 || !(rescale > 0.0) || !(dt >= 0.0) || !std::isfinite(dt) || !std::isfinite(rescale))
         return TBPM_EINVAL;
-    g_launches = 0;
-    ++env_epoch();                                        // re-read the TBPM_* switches for this call
+    const long long launches0 = total_launches();
+    H->last_launches = 0;
     if (n_state == 0 || n_step == 0) return TBPM_OK;
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || !corr || (!psi0 && !sites)) return TBPM_EINVAL;
     if (psi0 && (reinterpret_cast<uintptr_t>(psi0) & 15u)) return TBPM_EINVAL;
     if (sites)
         for (int b = 0; b < n_state; ++b)
             if (sites[b] < 0 || sites[b] >= H->n_orb) return TBPM_EINDEX;
-    const Plan P = make_plan(H->n_orb, n_state);
+    const Plan P = make_plan(H->n_orb, n_state, H->opt_tile);
     if (workspace_bytes < P.total) return TBPM_ENOMEM;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
 
@@ -377,7 +354,6 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     int K = 0;
     int rc = tbpm_cheb_coeff(rescale * dt, 1e-15, 8192, &K, cf.data());
     if (rc) return rc;
-    auto C = [&](int k) { return make_double2(cf[2 * k], cf[2 * k + 1]); };
 
     char *W = static_cast<char *>(workspace);
     double *partial = reinterpret_cast<double *>(W + P.partial_off);
@@ -386,12 +362,9 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
 
     // psi sits in slot p_n at the start of step n and moves p -> (p + 2) % 3 every step; start so that it ends in slot 0
     const int start_slot = n_step % 3;
-    WsHeader hdr{H->n_orb, n_state, P.tile, (int64_t)P.vec0_off, 0, 0};
-    k_write_header<<<1, 1, 0, st>>>(reinterpret_cast<WsHeader *>(W), hdr);
-    ++g_launches; count_launches(1);
 
     const bool table = H->n_table > 0;
-    TermParams tp{};
+        TermParams tp{};
     tp.orp = H->orp; tp.ocol = H->ocol; tp.oidx = H->oidx; tp.vtab = H->vtab; tp.diag = H->diag;
     tp.rowptr = H->rowptr; tp.col = H->col; tp.val = H->val;
     tp.n_orb = H->n_orb;
@@ -399,21 +372,21 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
     tp.n_table = H->n_table;
     tp.packed = H->packed;
     tp.single_real = H->single_real;
+    tp.device = H->device;
     tp.walk_stride = 0; tp.walk_run = 1;
     tp.n_lat_off = H->n_lat_off;
     for (int j = 0; j < H->n_lat_off; ++j) { tp.lat_off[j] = H->lat_off[j]; tp.lat_delta[j] = H->lat_delta[j]; }
-    if (const char *w = std::getenv("TBPM_WALK")) {          // "rows per lattice line,lines per run"
-        long long a = 0; int b = 1;
-        if (std::sscanf(w, "%lld,%d", &a, &b) >= 1) { tp.walk_stride = a; tp.walk_run = b; }
-    }
     tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
+    // L2 prefetch of the vector rows a few tiles ahead (term_ph.cuh, producer warp).  The leading edge of the gather
+    // window is the farthest neighbour: the largest lattice stride on uniform lattices, else the widest |col - row|.
+    tp.pf_dist = knob("pf", 0);
+    tp.pf_mask = knob("pf_mask", 3);
+    tp.pf_lead = H->n_lat_off > 0 ? H->lat_off[H->n_lat_off - 1] : H->halo_rows;
+    if (knob("pf_lead", -1) >= 0) tp.pf_lead = knob("pf_lead", -1);
+    const bool reverse_odd = knob("rev", 1) != 0;         // odd terms sweep backwards (term_ph.cuh)
 
-    bool fused_any = false;
     std::vector<TermParams> term;
-    int *pair_progress = reinterpret_cast<int *>(reinterpret_cast<char *>(partial) + kPartialBytes - 4 * sizeof(int) * kMaxGrid);   // [0,G): counters; [kMaxGrid]: error; [2 kMaxGrid, ..): per-warp scratch
-    TBPM_CUDA_TRY(cudaMemsetAsync(pair_progress + kMaxGrid, 0, sizeof(int), st));
-    const int rev_mode = env_int("TBPM_REV", 1);   // odd terms sweep backwards (term_ph.cuh)
     for (int t = 0; t < P.n_tile; ++t) {
         const int state0 = t * P.tile;
         const int n_valid = std::min(P.tile, n_state - state0);
@@ -433,94 +406,37 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
                 TBPM_CUDA_TRY(cudaMemsetAsync(bra, 0, sizeof(double2) * (size_t)n_el, st));
                 k_unit_states<<<1, kMaxBT, 0, st>>>(d_sites, state0, n_valid, bt, buf[start_slot], bra);
             }
-            ++g_launches; count_launches(1);
+            count_launches(1);
         }
         tp.psi0 = bra;
-        // Two terms per sweep when the gather halo and the lag between the two phases fit the L2 (see term_pair.cuh)
-        bool fuse = false;
-        {
-            const int fm = env_int("TBPM_FUSE", 0);       // 0: off, 1: when it pays, 2: always (tests)
-            TermParams probe = tp;
-            probe.flags = F_WRITE_Y; probe.n_acc = 0;
-            if (fm > 0 && table && (bt == 2 || bt == 4 || bt == 8) && term_ph_supported(bt, probe)) {
-                const int64_t tile_rows = 15 * 32 / (bt / 2);
-                const int64_t window = 3 * (int64_t)H->halo_rows + 2 * (int64_t)H->num_sms * tile_rows;      // rows alive in L2
-                const double mb = (double)window * bt * 16.0 * 2.0 / 1e6;
-                fuse = fm == 2 || (mb <= env_int("TBPM_FUSE_MB", 80) && H->n_orb >= 8 * window);
-            }
-        }
         int slot = start_slot;
         for (int n = 0; n < n_step; ++n) {
             double2 *psi = buf[slot], *t1 = buf[(slot + 1) % 3], *acc = buf[(slot + 2) % 3];
             int grid = 1;
             if (K == 1) {                                 // tau = 0: psi' = c_0 psi, no H application
-                tp.x = psi; tp.y = t1; tp.acc = acc; tp.a = 0.0;
-                tp.ca = C(0); tp.n_acc = 1; tp.flags = F_SKIP_H | F_ACC_INIT | F_REDUCE;
-                if ((rc = launch_term(bt, table, tp, H->num_sms, st, &grid))) return rc;
+                TermParams t0 = tp;
+                t0.x = psi; t0.y = t1; t0.acc = acc; t0.a = 0.0;
+                t0.ca = make_double2(cf[0], cf[1]); t0.n_acc = 1; t0.flags = F_SKIP_H | F_ACC_INIT | F_REDUCE;
+                if ((rc = launch_term(bt, table, 1, t0, H->num_sms, st, &grid))) return rc;
             }
-            int flushed = -1;                             // highest term already added to psi'
-            term.assign((size_t)K, TermParams{});        // term[k]: launch parameters of Chebyshev term k of this step
-            for (int k = 1; k < K; ++k) {
-                // buffers: T_k overwrites T_{k-2}; T_0 = psi, T_1 = t1, T_2 -> psi's buffer, ...
-                tp.x = (k % 2 == 1) ? psi : t1;           // T_{k-1}
-                tp.y = (k % 2 == 1) ? t1 : psi;           // T_{k-2} -> T_k
-                tp.acc = acc;
-                tp.a = (k == 1 ? 1.0 : 2.0) / rescale;
-                int flags = F_WRITE_Y | (k >= 2 ? F_SUB_Y : 0);
-                const bool last = (k == K - 1);
-                tp.n_acc = 0;
-                if (k % 3 == 2 || last) {                 // flush terms flushed+1 .. k (at most 3)
-                    tp.n_acc = k - flushed;
-                    tp.ca = C(k);
-                    tp.cb = tp.n_acc >= 2 ? C(k - 1) : make_double2(0.0, 0.0);
-                    tp.cc = tp.n_acc == 3 ? C(k - 2) : make_double2(0.0, 0.0);
-                    if (flushed < 0) flags |= F_ACC_INIT;
-                    flushed = k;
-                }
-                if (last) { flags |= F_REDUCE; flags &= ~F_WRITE_Y; }   // T_{K-1} is never read again
-                tp.flags = flags;
-                tp.reverse = 0;
-                term[k] = tp;
-            }
-            for (int k = 1; k < K;) {
-                if (fuse && k + 1 < K) {                  // two terms in one sweep (term_pair.cuh)
-                    PairParams pp{};
-                    pp.t = term[k];
-                    for (int f = 0; f < 2; ++f) {
-                        const TermParams &s = term[k + f];
-                        pp.ph[f] = PhaseParams{s.x, s.y, s.a, s.ca, s.cb, s.cc, (s.flags & F_SUB_Y) ? 1 : 0, s.n_acc,
-                                               (s.flags & F_ACC_INIT) ? 1 : 0, (s.flags & F_REDUCE) ? 1 : 0};
-                    }
-                    pp.halo = H->halo_rows;
-                    pp.progress = pair_progress;
-                    pp.error = pair_progress + kMaxGrid;
-                    ++g_launches;
-                    switch (bt) {
-                    case 2: rc = launch_term_pair_bt2(pp, H->num_sms, st, &grid); break;
-                    case 4: rc = launch_term_pair_bt4(pp, H->num_sms, st, &grid); break;
-                    default: rc = launch_term_pair_bt8(pp, H->num_sms, st, &grid); break;
-                    }
-                    if (rc) return rc;
-                    fused_any = true;
-                    k += 2;
-                } else {
-                    term[k].reverse = (rev_mode && !fuse) ? (k & 1) : 0;
-                    if ((rc = launch_term(bt, table, term[k], H->num_sms, st, &grid))) return rc;
-                    k += 1;
-                }
-            }
+            step_terms(tp, K, cf, rescale, reverse_odd, psi, t1, acc, term);
+            for (int k = 1; k < K; ++k)
+                if ((rc = launch_term(bt, table, H->opt_kernel, term[k], H->num_sms, st, &grid))) return rc;
             k_reduce_final<<<bt, 96, 0, st>>>(partial, grid, bt, n_valid, state0, n_step, n, corr, norm2);
-            ++g_launches; count_launches(1);
+            count_launches(1);
             slot = (slot + 2) % 3;                        // psi' (acc) is the next step's psi
         }
     }
     TBPM_CUDA_TRY(cudaGetLastError());
-    if (fused_any) {                                      // a dependency wait that gave up means the blocks were not co-resident
-        int err = 0;
-        TBPM_CUDA_TRY(cudaMemcpyAsync(&err, pair_progress + kMaxGrid, sizeof(int), cudaMemcpyDeviceToHost, st));
-        TBPM_CUDA_TRY(cudaStreamSynchronize(st));
-        if (err) return TBPM_ECUDA;
+    {
+        std::lock_guard<std::mutex> lock(H->mu);
+        RunRecord rec{workspace, n_state, P.tile, P.last_bt, P.vec0_off, P.full_vec};
+        bool found = false;
+        for (RunRecord &r : H->runs)
+            if (r.workspace == workspace) { r = rec; found = true; }
+        if (!found) H->runs.push_back(rec);
     }
+    H->last_launches = total_launches() - launches0;
     return TBPM_OK;
 }
 
@@ -529,18 +445,18 @@ int run(const tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state
 extern "C" int tbpm_propagate_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes)
 {
     if (!H || n_state < 0 || !workspace_bytes) return TBPM_EINVAL;
-    *workspace_bytes = make_plan(H->n_orb, n_state).total;
+    *workspace_bytes = make_plan(H->n_orb, n_state, H->opt_tile).total;
     return TBPM_OK;
 }
 
-extern "C" int tbpm_propagate(const tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale, double *corr,
+extern "C" int tbpm_propagate(tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale, double *corr,
                               double *norm2, void *workspace, size_t workspace_bytes, void *stream)
 {
     if (n_state > 0 && n_step > 0 && !psi0) return TBPM_EINVAL;
     return run(H, psi0, nullptr, n_state, n_step, dt, rescale, corr, norm2, workspace, workspace_bytes, stream);
 }
 
-extern "C" int tbpm_ldos(const tbpm_ham *H, const int64_t *sites, int n_site, int n_step, double dt, double rescale, double *corr,
+extern "C" int tbpm_ldos(tbpm_ham *H, const int64_t *sites, int n_site, int n_step, double dt, double rescale, double *corr,
                          double *norm2, void *workspace, size_t workspace_bytes, void *stream)
 {
     if (n_site > 0 && n_step > 0 && !sites) return TBPM_EINVAL;
@@ -550,13 +466,43 @@ extern "C" int tbpm_ldos(const tbpm_ham *H, const int64_t *sites, int n_site, in
 extern "C" int tbpm_get_state(const tbpm_ham *H, const void *workspace, int state, double *psi_out, void *stream)
 {
     if (!H || !workspace || !psi_out || state < 0) return TBPM_EINVAL;
+    RunRecord rec{};
+    {
+        std::lock_guard<std::mutex> lock(H->mu);
+        bool found = false;
+        for (const RunRecord &r : H->runs)
+            if (r.workspace == workspace) { rec = r; found = true; }
+        if (!found) return TBPM_EINVAL;                   // no tbpm_propagate / tbpm_ldos call of this handle used that workspace
+    }
+    if (state >= rec.n_state) return TBPM_EINDEX;
     if (H->n_orb == 0) return TBPM_OK;
+    const int tile = state / rec.tile;
+    const int n_tile = (rec.n_state + rec.tile - 1) / rec.tile;
+    const int bt = (tile == n_tile - 1) ? rec.last_bt : rec.tile;
+    // psi ends in slot 0 of its tile's buffers (run() starts it in slot n_step % 3)
+    const double2 *psi = reinterpret_cast<const double2 *>(static_cast<const char *>(workspace) + rec.vec0_off + (size_t)tile * 4 * rec.full_vec);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int grid = (int)std::min<int64_t>((H->n_orb + kThreads - 1) / kThreads, 4096);
-    k_get_state<<<grid, kThreads, 0, st>>>(static_cast<const char *>(workspace), state, reinterpret_cast<double2 *>(psi_out));
+    k_get_state<<<grid, kThreads, 0, st>>>(psi, H->n_orb, bt, state - tile * rec.tile, reinterpret_cast<double2 *>(psi_out));
     count_launches(1);
     TBPM_CUDA_TRY(cudaGetLastError());
     return TBPM_OK;
 }
 
-extern "C" int64_t tbpm_last_launch_count(void) { return g_launches; }
+extern "C" int64_t tbpm_last_launch_count(const tbpm_ham *H) { return H ? (int64_t)H->last_launches : 0; }
+
+extern "C" int tbpm_set_option(tbpm_ham *H, int option, int64_t value)
+{
+    if (!H) return TBPM_EINVAL;
+    switch (option) {
+    case TBPM_OPT_TILE:
+        if (value != 1 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32) return TBPM_EINVAL;
+        H->opt_tile = (int)value;
+        return TBPM_OK;
+    case TBPM_OPT_KERNEL:
+        if (value < 0 || value > 2) return TBPM_EINVAL;
+        H->opt_kernel = (int)value;
+        return TBPM_OK;
+    }
+    return TBPM_EINVAL;
+}

@@ -5,6 +5,10 @@
 #include <stddef.h>
 #include <stdint.h>
 
+#include <atomic>
+#include <mutex>
+#include <vector>
+
 #include "../../include/tbpm.h"
 
 #define TBPM_CUDA_TRY(expr)                      \
@@ -20,6 +24,7 @@ namespace tbpm_detail {
 
 void note_cuda_error(cudaError_t e);
 void count_launches(int n);   // process-wide kernel-launch counter (tbpm_total_launch_count)
+long long total_launches();
 
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a; }
@@ -38,6 +43,13 @@ enum StatusWord {
     ST_TAB_OVERFLOW = 5, // more than kTableMax distinct values (or a probe sequence gave up)
     ST_NEG_MIN_ROW = 6,  // 2^30 - (fewest entries in a row of the canonical CSR)
     ST_HALO = 7          // widest |col - row| (circular): how far a row reaches into the vector
+};
+
+// What the last tbpm_propagate / tbpm_ldos call of a handle left in a workspace (read by tbpm_get_state).
+struct RunRecord {
+    const void *workspace;
+    int n_state, tile, last_bt;
+    size_t vec0_off, full_vec;
 };
 
 }  // namespace tbpm_detail
@@ -74,4 +86,12 @@ struct tbpm_ham {
     double2 *vtab = nullptr;
     double *diag = nullptr;
     int32_t *status = nullptr;
+
+    // options (tbpm_set_option)
+    int opt_tile = 8;      // states per tile: 8 interleaved complex128 = one 128-byte line per row
+    int opt_kernel = 0;    // 1: every term on the general kernel
+    // bookkeeping of the propagate calls: written under `mu` (calls on distinct workspaces may run concurrently)
+    mutable std::mutex mu;
+    std::vector<tbpm_detail::RunRecord> runs;
+    std::atomic<long long> last_launches{0};
 };

@@ -1,9 +1,7 @@
-// term.h -- private: parameters shared by the fused Chebyshev-term kernels (term_ws.cu, propagate.cu).
+// term.h -- private: parameters shared by the fused Chebyshev-term kernels (term_ph.cuh, propagate.cu).
 #pragma once
 
-#include <cstdlib>
-#include <unordered_map>
-
+#include "knobs.h"
 #include "tbpm_internal.h"
 
 namespace tbpm_detail {
@@ -53,26 +51,10 @@ struct TermParams {
     int reverse;           // phased kernel: sweep the tiles from the last row block to the first
     int uniform;           // every row holds exactly max_row_off off-diagonal entries
     int single_real;       // the table holds one value and it is real
-};
-
-// Two consecutive Chebyshev terms in ONE sweep (term_pair.cuh).  Phase 0 is term k (x = T_{k-1}, y = T_{k-2} -> T_k), phase 1 is
-// term k+1 (x = T_k, y = T_{k-1} -> T_{k+1}); phase 1 of a tile runs a few hundred tiles behind phase 0, while T_k, T_{k-1} and the
-// matrix slices are still in L2, so the pair moves matrix + 4 vectors through DRAM where two launches move 2 x (matrix + 3).
-struct PhaseParams {
-    const double2 *x;
-    double2 *y;
-    double a;
-    double2 ca, cb, cc;
-    int sub_y, n_acc, acc_init, reduce;
-};
-
-struct PairParams {
-    TermParams t;          // matrix, n_orb, acc, psi0, partial, table / row-shape facts, stage geometry
-    PhaseParams ph[2];
-    int64_t halo;          // tiles: phase 1 of tile t needs phase 0 of every tile within +-halo (circular)
-    int lag;               // steps of a block's sequence between phase 0 and phase 1 of its tiles
-    int *progress;         // [grid] phase-0 tiles finished by each block (zeroed before the launch)
-    int *error;            // set when a dependency wait gave up (never, unless the blocks are not co-resident)
+    int device;            // CUDA device of the handle (per-device launch configuration caches)
+    int pf_dist;           // phased kernel: tiles ahead of the staged one whose vector rows are prefetched into L2 (0: off)
+    int pf_mask;           // 1: y / psi' / psi0 rows, 2: x rows at the leading edge
+    int64_t pf_lead;       // rows between a tile and the leading edge of its gather window (first touch of x)
 };
 
 // Table value of an entry: index in bits 0-14, bit 15 = take the conjugate (exact: only the sign bit of im changes).
@@ -90,45 +72,38 @@ __device__ __forceinline__ void cfma(double2 &h, double2 v, double2 x)   // h +=
     h.y = fma(v.y, x.x, h.y);
 }
 
-// Experiment switches (TBPM_*): read from the environment once per tbpm_propagate / tbpm_ldos call -- env_epoch() is bumped
-// at the start of every call -- not once per kernel launch.
-inline unsigned long long &env_epoch()
+// Shared-memory stage of the phased kernel: row offsets | column words | value indices | diagonal of one tile of R rows.
+constexpr size_t kSmemMax = 227 * 1024;      // opt-in dynamic shared memory of one block on sm_100
+constexpr size_t kStageBudget = 200 * 1024;  // what the stages of one block may take
+constexpr int kMaxDevices = 64;
+struct StageGeom { int cap_entries, off_col, off_idx, off_diag, stage_bytes; };
+inline StageGeom stage_geom(int R, int max_row_off, bool with_idx)
 {
-    static thread_local unsigned long long e = 1;
-    return e;
+    StageGeom g{};
+    g.cap_entries = ((R * (max_row_off > 1 ? max_row_off : 1) + 8 + 7) / 8) * 8;   // + alignment slack of the slice start
+    size_t o = (size_t)(((R + 1) * 4 + 15) & ~15);
+    g.off_col = (int)o;  o += (size_t)g.cap_entries * 4;
+    g.off_idx = (int)o;  o += with_idx ? (size_t)g.cap_entries * 2 : 0;
+    o = (o + 15) & ~size_t(15);
+    g.off_diag = (int)o; o += (size_t)((R * 8 + 15) & ~15);
+    g.stage_bytes = (int)((o + 127) & ~size_t(127));
+    return g;
 }
-inline int env_int(const char *name, int dflt)
-{
-    struct Entry { unsigned long long epoch; int value; };
-    static thread_local std::unordered_map<const char *, Entry> cache;   // keyed by the literal's address: one entry per call site
-    Entry &c = cache[name];
-    if (c.epoch != env_epoch()) {
-        const char *e = std::getenv(name);
-        c.value = e ? std::atoi(e) : dflt;
-        c.epoch = env_epoch();
-    }
-    return c.value;
-}
-
-// Warp-specialised bulk-copy (TMA) kernel, term_ws.cu.  Returns TBPM_EINVAL if (bt, flags) has no instantiation
-// (the caller then uses the direct kernel).  *grid_out = blocks launched (sizes the final reduction).
-bool term_ws_supported(int bt, const TermParams &p);
-int launch_term_ws(int bt, TermParams p, int num_sms, cudaStream_t st, int *grid_out);
 
 // Phased kernel (term_ph.cuh): matrix slices staged by bulk copies, vectors streamed directly; one file per tile width.
+// term_ph_supported: the tile width has an instantiation, the term is one of the five (n_acc, reduce) shapes, and two
+// stages of the widest tile fit the shared memory of an SM (rows of up to a few dozen entries); everything else runs
+// on the general kernel k_cheb_term (propagate.cu).
 bool term_ph_supported(int bt, const TermParams &p);
 int launch_term_ph_bt1(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 int launch_term_ph_bt2(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 int launch_term_ph_bt4(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 int launch_term_ph_bt8(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
-// Staged-gather kernel (term_sg.cu): tiles of 8 states on uniform lattices; false / TBPM_EINVAL when it does not apply.
-bool term_sg_supported(int bt, const TermParams &p);
-int launch_term_sg(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
-// Pair kernel, one file per tile width (2, 4, 8 states).
-int launch_term_pair_bt2(const PairParams &p, int num_sms, cudaStream_t st, int *grid_out);
-int launch_term_pair_bt4(const PairParams &p, int num_sms, cudaStream_t st, int *grid_out);
-int launch_term_pair_bt8(const PairParams &p, int num_sms, cudaStream_t st, int *grid_out);
+// Rolling-window kernel (term_rw.cu): tiles of 8 states on lattices whose largest stride is a whole number of 128-row
+// tiles; false / TBPM_EINVAL when it does not apply.
+bool term_rw_supported(int bt, const TermParams &p);
+int launch_term_rw(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
 }  // namespace tbpm_detail

@@ -22,6 +22,7 @@
 
 #include <algorithm>
 
+#include "ptx_helpers.cuh"
 #include "term.h"
 
 namespace tbpm_detail {
@@ -30,79 +31,7 @@ namespace ph {
 constexpr int kMaxStages = 8;
 constexpr int kNwA = 23, kNwB = 19;       // consumer warps of the short-row / six-entry shapes (see launch_bt)
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
-{
-    asm volatile("cp.async.bulk.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes),
-                 "r"(bar)
-                 : "memory");
-}
-__device__ __forceinline__ uint32_t lds_u32(uint32_t a)
-{
-    uint32_t v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ uint32_t lds_u32_if(uint32_t a, bool on)      // 0 when off
-{
-    uint32_t v;
-    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\nmov.u32 %0, 0;\n@q ld.shared.u32 %0, [%1];\n}" : "=r"(v) : "r"(a), "r"((int)on));
-    return v;
-}
-__device__ __forceinline__ uint32_t lds_u16_if(uint32_t a, bool on)
-{
-    uint32_t v;
-    asm volatile("{\n.reg .pred q;\n.reg .u16 h;\nsetp.ne.b32 q, %2, 0;\nmov.u16 h, 0;\n@q ld.shared.u16 h, [%1];\ncvt.u32.u16 %0, h;\n}"
-                 : "=r"(v)
-                 : "r"(a), "r"((int)on));
-    return v;
-}
-__device__ __forceinline__ uint32_t lds_u16(uint32_t a)
-{
-    uint32_t v;
-    asm volatile("{\n.reg .u16 h;\nld.shared.u16 h, [%1];\ncvt.u32.u16 %0, h;\n}" : "=r"(v) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ void lds_v2_u32(uint32_t a, uint32_t &x, uint32_t &y)
-{
-    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(x), "=r"(y) : "r"(a));
-}
-__device__ __forceinline__ void lds_v4_u32(uint32_t a, uint32_t &x, uint32_t &y, uint32_t &z, uint32_t &w)
-{
-    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(w) : "r"(a));
-}
-__device__ __forceinline__ double lds_f64(uint32_t a)
-{
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
-    return v;
-}
+using namespace ptx;
 
 // SPT consecutive complex128 values of one row
 template <int SPT> struct CVec;
@@ -249,10 +178,15 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
 
     if (tid >= kConsumers) {
         // ------------------------------------------------ producer warp ------------------------------------------------
-        if (tid != kConsumers) return;
+        // Lane 0 stages the matrix slices.  All 32 lanes then PREFETCH INTO L2 the vector rows that a tile `pf_dist` steps
+        // further along this block's walk will stream (y, psi', psi0) or touch first (x at the leading edge of the gather
+        // window): the consumers hold one row group per warp in registers, which keeps only ~30 KB of DRAM-bound loads
+        // in flight per SM where the HBM needs ~64 KB (microbenchmark, profiles/r2_probe.md); prefetches hold no
+        // registers, so they carry the DRAM latency and the consumers' loads become L2 hits.
+        const int lane = tid - kConsumers;
         uint32_t q_lo = 0, q_hi = 0;                        // offsets bounding the next tile to issue (prefetched)
         int64_t tile = first_tile;
-        if (tile < n_tiles) {
+        if (lane == 0 && tile < n_tiles) {
             const int64_t r0 = tile_rows(tile);
             q_lo = __ldg(p.orp + r0);
             q_hi = __ldg(p.orp + min(r0 + R, p.n_orb));
@@ -260,40 +194,67 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
         int s = 0, ci = 0;
         int64_t cu = blockIdx.x;
         uint32_t ph = 1;                                    // parity of the "empty" phase to wait for; first pass: free
+        // cursor of the prefetched tile, pf_dist steps ahead of the staged one
+        const int pfd = p.pf_dist;
+        int64_t ptile = first_tile, pu = blockIdx.x;
+        int pi = 0;
+        for (int k = 0; k < pfd && ptile < n_tiles; ++k) ptile = next_tile(ptile, pi, pu);
         for (; tile < n_tiles; tile = next_tile(tile, ci, cu)) {
-            const uint32_t c_lo = q_lo, c_hi = q_hi;
-            int cj = ci;
-            int64_t cv = cu;
-            const int64_t nt = next_tile(tile, cj, cv);
-            if (nt < n_tiles) {                             // bounds of the following tile: latency hidden behind this issue
-                const int64_t nr0 = tile_rows(nt);
-                q_lo = __ldg(p.orp + nr0);
-                q_hi = __ldg(p.orp + min(nr0 + R, p.n_orb));
+            if (lane == 0) {
+                const uint32_t c_lo = q_lo, c_hi = q_hi;
+                int cj = ci;
+                int64_t cv = cu;
+                const int64_t nt = next_tile(tile, cj, cv);
+                if (nt < n_tiles) {                         // bounds of the following tile: latency hidden behind this issue
+                    const int64_t nr0 = tile_rows(nt);
+                    q_lo = __ldg(p.orp + nr0);
+                    q_hi = __ldg(p.orp + min(nr0 + R, p.n_orb));
+                }
+                const uint32_t full = bar0 + 8 * s;
+                mbar_wait(bar0 + 8 * (kMaxStages + s), ph); // a fresh barrier reports the "previous" phase complete
+                const uint32_t st = smem0 + (uint32_t)s * (uint32_t)p.stage_bytes;
+                const int64_t r0 = tile_rows(tile);
+                const int rows = (int)min((int64_t)R, p.n_orb - r0);
+                const uint32_t col_lo = c_lo & ~3u, idx_lo = c_lo & ~7u;
+                const uint32_t nc = ((c_hi - col_lo) + 3u) & ~3u, ni = ((c_hi - idx_lo) + 7u) & ~7u;
+                lo_s[s][0] = col_lo;
+                lo_s[s][1] = idx_lo;
+                const uint32_t orp_bytes = (uint32_t)(((rows + 1) * 4 + 15) & ~15);
+                uint32_t tx = orp_bytes;
+                bulk_g2s(st, p.orp + r0, orp_bytes, full);
+                if (nc > 0) {
+                    bulk_g2s(st + p.off_col, p.ocol + col_lo, nc * 4, full);
+                    tx += nc * 4;
+                    if (VK == 0 || VK == 4) { bulk_g2s(st + p.off_idx, p.oidx + idx_lo, ni * 2, full); tx += ni * 2; }
+                }
+                if (has_diag) {
+                    const uint32_t db = (uint32_t)((rows * 8 + 15) & ~15);
+                    bulk_g2s(st + p.off_diag, p.diag + r0, db, full);
+                    tx += db;
+                }
+                mbar_expect_tx(full, tx);                   // release: also publishes lo_s[s]
+                if (++s == S) { s = 0; ph ^= 1u; }
             }
-            const uint32_t full = bar0 + 8 * s;
-            mbar_wait(bar0 + 8 * (kMaxStages + s), ph);     // a fresh barrier reports the "previous" phase complete
-            const uint32_t st = smem0 + (uint32_t)s * (uint32_t)p.stage_bytes;
-            const int64_t r0 = tile_rows(tile);
-            const int rows = (int)min((int64_t)R, p.n_orb - r0);
-            const uint32_t col_lo = c_lo & ~3u, idx_lo = c_lo & ~7u;
-            const uint32_t nc = ((c_hi - col_lo) + 3u) & ~3u, ni = ((c_hi - idx_lo) + 7u) & ~7u;
-            lo_s[s][0] = col_lo;
-            lo_s[s][1] = idx_lo;
-            const uint32_t orp_bytes = (uint32_t)(((rows + 1) * 4 + 15) & ~15);
-            uint32_t tx = orp_bytes;
-            bulk_g2s(st, p.orp + r0, orp_bytes, full);
-            if (nc > 0) {
-                bulk_g2s(st + p.off_col, p.ocol + col_lo, nc * 4, full);
-                tx += nc * 4;
-                if (VK == 0 || VK == 4) { bulk_g2s(st + p.off_idx, p.oidx + idx_lo, ni * 2, full); tx += ni * 2; }
+            __syncwarp();                                   // the prefetches follow the pace of the stages
+            if (pfd > 0 && ptile < n_tiles) {
+                const int64_t r0 = tile_rows(ptile);
+                const int64_t rows = min((int64_t)R, p.n_orb - r0);
+                const int n_lines = (int)((rows * BT * 16 + 127) >> 7);
+                const char *py = reinterpret_cast<const char *>(p.y + r0 * BT);
+                const char *pa = reinterpret_cast<const char *>(p.acc + r0 * BT);
+                const char *pz = reinterpret_cast<const char *>(p.psi0 + r0 * BT);
+                const int64_t x0 = r0 + p.pf_lead;          // leading edge of the gather window of that tile
+                const char *px = reinterpret_cast<const char *>(p.x + x0 * BT);
+                const bool x_ok = x0 >= 0 && x0 + rows <= p.n_orb;
+                const bool do_y = need_y && (p.pf_mask & 1), do_x = x_ok && (p.pf_mask & 2);
+                for (int o = lane; o < n_lines; o += 32) {
+                    if (do_y) prefetch_l2(py + (size_t)o * 128);
+                    if (do_x) prefetch_l2(px + (size_t)o * 128);
+                    if (NACC > 0 && need_acc) prefetch_l2(pa + (size_t)o * 128);
+                    if (REDUCE) prefetch_l2(pz + (size_t)o * 128);
+                }
+                ptile = next_tile(ptile, pi, pu);
             }
-            if (has_diag) {
-                const uint32_t db = (uint32_t)((rows * 8 + 15) & ~15);
-                bulk_g2s(st + p.off_diag, p.diag + r0, db, full);
-                tx += db;
-            }
-            mbar_expect_tx(full, tx);                       // release: also publishes lo_s[s]
-            if (++s == S) { s = 0; ph ^= 1u; }
         }
         return;
     }
@@ -525,30 +486,29 @@ int launch_one(TermParams p, int num_sms, cudaStream_t st, int *grid_out)
 {
     constexpr int kConsumers = NW * 32, kThreads = kConsumers + 32;
     constexpr int R = kConsumers / (BT / SPT);
-    p.n_stage = std::min(kMaxStages, std::max(2, env_int("TBPM_STAGES", 4)));
+    p.n_stage = std::min(kMaxStages, std::max(2, knob("stages", 4)));
     p.walk_d0 = 1;
-    p.walk_len = std::max(1, env_int("TBPM_CHUNK", 1));
+    p.walk_len = std::max(1, knob("chunk", 1));
     if (p.walk_stride > 0 && p.walk_stride % R == 0) {      // a lattice line is a whole number of tiles: walk across lines
         p.walk_d0 = p.walk_stride / R;
         p.walk_len = std::max(1, p.walk_run);
     }
-    p.pol = env_int("TBPM_POL", 1);
-    p.cap_entries = ((R * std::max(p.max_row_off, 1) + 8 + 7) / 8) * 8;          // + alignment slack of the slice start
-    size_t o = (size_t)(((R + 1) * 4 + 15) & ~15);
-    p.off_col = (int)o;  o += (size_t)p.cap_entries * 4;
-    p.off_idx = (int)o;  o += (VK == 0 || VK == 4) ? (size_t)p.cap_entries * 2 : 0;
-    o = (o + 15) & ~size_t(15);
-    p.off_diag = (int)o; o += (size_t)((R * 8 + 15) & ~15);
-    p.off_vec = 0;
-    p.stage_bytes = (int)((o + 127) & ~size_t(127));
-    p.n_stage = (int)std::max<size_t>(2, std::min<size_t>(p.n_stage, (size_t)160 * 1024 / p.stage_bytes));
-    const size_t dyn = (size_t)p.stage_bytes * p.n_stage + (VK == 4 ? (size_t)p.n_table * sizeof(double2) : 0);
+    p.pol = knob("pol", 1);
+    const StageGeom g = stage_geom(R, p.max_row_off, VK == 0 || VK == 4);
+    p.cap_entries = g.cap_entries; p.off_col = g.off_col; p.off_idx = g.off_idx; p.off_diag = g.off_diag; p.off_vec = 0;
+    p.stage_bytes = g.stage_bytes;
+    const size_t tab = VK == 4 ? (size_t)p.n_table * sizeof(double2) : 0;
+    const size_t room = std::min<size_t>(kStageBudget, kSmemMax - tab);
+    if ((size_t)p.stage_bytes * 2 > room) return TBPM_EINVAL;   // term_ph_supported / launch_bt rule this out
+    p.n_stage = (int)std::min<size_t>(p.n_stage, room / p.stage_bytes);
+    const size_t dyn = (size_t)p.stage_bytes * p.n_stage + tab;
     auto kern = k_term_ph<BT, SPT, CH, NACC, REDUCE, VK, UNI, NW>;
-    static size_t configured = 0;
-    if (dyn > configured) {
+    static size_t configured[kMaxDevices] = {0};            // per device: the attribute belongs to the device's copy of the function
+    if (p.device < 0 || p.device >= kMaxDevices) return TBPM_EINVAL;
+    if (dyn > configured[p.device]) {
         const size_t want = std::max(dyn, (size_t)64 * 1024);
         TBPM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)want));
-        configured = want;
+        configured[p.device] = want;
     }
     const int64_t need = (p.n_orb + R - 1) / R;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>({need, (int64_t)num_sms, (int64_t)kMaxGrid}));   // one block per SM
@@ -577,8 +537,8 @@ int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
     constexpr int SPT = BT >= 2 ? 2 : 1;
     const int n = p.max_row_off;
-    const bool uni = p.uniform && env_int("TBPM_UNI", 1);
-    const int vk = (p.single_real && env_int("TBPM_VK2", 1)) ? 2 : (p.packed ? 1 : 0);
+    const bool uni = p.uniform && knob("uni", 1);
+    const int vk = (p.single_real && knob("vk2", 1)) ? 2 : (p.packed ? 1 : 0);
     if (uni && vk == 2 && n == 6) {
         // Three-dimensional lattice: walk the tiles along the largest stride (the plane).  A run then re-uses the rows it
         // gathered one plane down as its own rows and as the plane-up neighbours of its next tiles (L1), and the window
@@ -586,7 +546,7 @@ int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
         // launches stop re-reading it (ncu: 9.7 -> 7.1 GB per launch on cfg5).  16 consumer warps: 2^k rows per tile.
         TermParams q = p;
         constexpr int R16 = 512 / (BT / SPT);
-        if (q.walk_stride == 0 && env_int("TBPM_AUTOWALK", 1))
+        if (q.walk_stride == 0 && knob("autowalk", 1))
             for (int j = 0; j < q.n_lat_off; ++j)
                 if (q.lat_off[j] % R16 == 0 && q.lat_off[j] * 4 <= q.n_orb) { q.walk_stride = q.lat_off[j]; q.walk_run = 64; }
         if (q.walk_stride > 0 && q.walk_stride % R16 == 0) return launch_variant<BT, SPT, 6, 2, true, 16>(q, num_sms, st, grid_out);
@@ -609,7 +569,9 @@ int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
         // Table small enough for shared memory (cfg4: 7,864 values = 126 KB): each block copies it once, the values are fetched
         // with LDS only when the gathers have returned (no registers held for them), which leaves room for all eight gathers
         // of a row in one round trip.  cfg4: 1955 -> 1885 us per launch.
-        const bool tab_smem = uni && (size_t)p.n_table * sizeof(double2) <= 150 * 1024 && env_int("TBPM_TAB_SMEM", 1);
+        const size_t tab = (size_t)p.n_table * sizeof(double2);
+        const size_t two_stages = 2 * (size_t)stage_geom(19 * 32 / (BT / SPT), n, true).stage_bytes;
+        const bool tab_smem = uni && tab <= 150 * 1024 && tab + two_stages <= kSmemMax && knob("tab_smem", 1);
         if (tab_smem && n % 8 == 0) return launch_variant<BT, SPT, 8, 4, true, 15>(p, num_sms, st, grid_out);
         if (tab_smem && n % 4 == 0) return launch_variant<BT, SPT, 4, 4, true, 19>(p, num_sms, st, grid_out);
     }

@@ -15,6 +15,7 @@ import torch
 from . import build as _build
 
 TBPM_VALIDATE, TBPM_HOPS_FULL, TBPM_NO_TABLE = 1, 2, 4
+TBPM_OPT_TILE, TBPM_OPT_KERNEL = 1, 2
 TBPM_OK, TBPM_EINVAL, TBPM_EINDEX, TBPM_EDIAG, TBPM_EDUP, TBPM_ENOMEM, TBPM_ECUDA, TBPM_EBOUND = 0, -1, -2, -3, -4, -5, -6, -7
 
 _lib = None
@@ -53,6 +54,8 @@ def lib() -> C.CDLL:
         L.tbpm_get_state.argtypes = [vp, vp, C.c_int, vp, vp]
         L.tbpm_dos.argtypes = [vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp]
         L.tbpm_last_launch_count.restype = i64
+        L.tbpm_last_launch_count.argtypes = [vp]
+        L.tbpm_set_option.argtypes = [vp, C.c_int, i64]
         L.tbpm_total_launch_count.restype = i64
         L.tbpm_corr_host_bytes.argtypes = [i64, i64, C.c_int, C.c_int, C.c_int, u32, P(sz)]
         L.tbpm_corr_host.argtypes = [i64, vp, i64, vp, vp, vp, u32, vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp, sz, vp, P(sz), P(sz)]
@@ -227,8 +230,12 @@ def tbpm_get_state(H: Hamiltonian, workspace: torch.Tensor, state: int) -> torch
     return out[: H.n_orb]
 
 
-def tbpm_last_launch_count() -> int:
-    return int(lib().tbpm_last_launch_count())
+def tbpm_last_launch_count(H: Hamiltonian) -> int:
+    return int(lib().tbpm_last_launch_count(H.handle))
+
+
+def tbpm_set_option(H: Hamiltonian, option: int, value: int) -> None:
+    _check(lib().tbpm_set_option(H.handle, option, value), "tbpm_set_option")
 
 
 def tbpm_total_launch_count() -> int:

@@ -206,6 +206,36 @@ def cubic_hops(L: int, t: float = -1.0, device="cpu"):
     return L ** 3, hop_i, hop_j, hop_val
 
 
+def square_range_hops(Lx: int, Ly: int, radius: float, n_phase: int = 1, device="cpu"):
+    """Square lattice with a hop to EVERY site within `radius` (third-neighbour-style models with long rows: 12 neighbours
+    at radius 2, 28 at 3, 48 at 4, 80 at 5).  Not one of BASELINE.json's configs: it exists to drive the kernels through rows
+    longer than the 8 entries the configs have.  <r'|H|r> = 0.3/d^2 * exp(i(0.4 dx - 0.7 dy)) * exp(i 2 pi (x mod n_phase)/n_phase dy):
+    n_phase sets the number of distinct values (table size).  Returns (n_orb, hop_i, hop_j, hop_val, row_sum) with
+    row_sum = sum_j |H_ij| (the same for every row: a valid `rescale`)."""
+    r = int(math.floor(radius))
+    if Lx < 2 * r + 1 or Ly < 2 * r + 1:
+        raise ValueError("periodic extents must exceed 2*radius (wrap-around duplicates, reading #15)")
+    if Lx % n_phase != 0:
+        raise ValueError("n_phase must divide Lx")
+    y = torch.arange(Ly, dtype=torch.int64, device=device).view(Ly, 1)
+    x = torch.arange(Lx, dtype=torch.int64, device=device).view(1, Lx)
+    src = (y * Lx + x).reshape(-1)
+    xf = (x % n_phase).to(torch.float64).expand(Ly, Lx).reshape(-1) * (2.0 * math.pi / n_phase)
+    his, hjs, hvs = [], [], []
+    row_sum = 0.0
+    for dx in range(0, r + 1):
+        for dy in range(-r, r + 1):
+            if dx * dx + dy * dy > radius * radius or (dx == 0 and dy <= 0):
+                continue                                     # each pair once: dx > 0, or dx == 0 and dy > 0
+            amp = 0.3 / (dx * dx + dy * dy)
+            ang = xf * dy + (0.4 * dx - 0.7 * dy)
+            his.append((((y + dy) % Ly) * Lx + ((x + dx) % Lx)).reshape(-1))
+            hjs.append(src)
+            hvs.append(torch.complex(torch.cos(ang) * amp, torch.sin(ang) * amp))
+            row_sum += 2.0 * amp
+    return Lx * Ly, torch.cat(his).to(torch.int32), torch.cat(hjs).to(torch.int32), torch.cat(hvs), row_sum
+
+
 def chain_hops(L: int, t: float = -1.0, device="cpu"):
     """1-D periodic chain (used for the closed-form DOS pin 1/(pi sqrt(4t^2-E^2)))."""
     if L < 3:

@@ -130,10 +130,12 @@ def test_table_overflow_falls_back_to_full_values(dev, oracle_mod):
 # ---------------------------------------------------------------------------------------------------------------------
 # a1-a7: propagate, every element against the serial oracle
 # ---------------------------------------------------------------------------------------------------------------------
-def run_parity(dev, oracle_mod, w, n_state, n_step, flags=0, dt=None, check_state=True):
+def run_parity(dev, oracle_mod, w, n_state, n_step, flags=0, dt=None, check_state=True, options=None):
     dt = w.dt if dt is None else dt
     psi0 = w.psi0(device=dev, n_state=n_state)
     H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val, flags)
+    for opt, value in (options or {}).items():
+        tbpm.tbpm_set_option(H, opt, value)
     corr, norm2, ws = tbpm.tbpm_propagate(H, psi0, n_step, dt, w.rescale)
     hi, hj, hv, on = to_np(w)
     ref, refn, reff = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0.cpu().numpy(), n_step, dt, w.rescale, return_state=True)
@@ -153,7 +155,7 @@ def test_config1_full_length(dev, oracle_mod):
     H, _, corr, _ = run_parity(dev, oracle_mod, w, 1, 256)
     assert corr.shape == (1, 256)
     assert H.n_table == 1                                            # t and conj(t) = (t, -0.0) share the entry
-    assert tbpm.tbpm_last_launch_count() == 256 * 21 + 2             # 20 terms + 1 final reduction per step
+    assert tbpm.tbpm_last_launch_count(H) == 256 * 21 + 1            # 20 terms + 1 final reduction per step, + set-up
 
 
 @pytest.mark.parametrize("cfg,over,n_state,n_step", [
@@ -173,38 +175,85 @@ def test_small_configs_every_element(dev, oracle_mod, cfg, over, n_state, n_step
     run_parity(dev, oracle_mod, w, n_state, n_step, flags)
 
 
-@pytest.mark.parametrize("cfg,over,n_state,n_step", [
-    (2, dict(Na=96, Nb=70), 4, 12),                                  # honeycomb shape, tile of 4
-    (4, dict(Lx=64, Ly=48, phi_den=32), 8, 10),                      # table shape, two chunks per row
-    (5, dict(L=17), 16, 9),                                          # cubic shape, odd number of terms' worth of flushes
-    (3, dict(Na=100, Nb=60), 2, 7),                                  # irregular rows, tile of 2
-])
-def test_two_terms_per_sweep(dev, oracle_mod, cfg, over, n_state, n_step, monkeypatch):
-    """term_pair.cuh (experimental, TBPM_FUSE): phase 1 of a tile waits for phase 0 of its halo; same 1e-10 bar."""
-    monkeypatch.setenv("TBPM_FUSE", "2")
+# lattices on which the rolling-window kernel (term_rw.cu) applies: tiles of 8 states, largest stride a multiple of 128 rows
+RW_CASES = [
+    (5, dict(L=32), 8, 7),                                           # cubic 32^3: W = 1024 rows, +-line neighbours by LDG, diagonal
+    (5, dict(L=16, W=0.0), 16, 6),                                   # cubic 16^3 (W = 256), no diagonal, two tiles
+    (4, dict(Lx=128, Ly=24, phi_den=32), 8, 9),                      # square + flux: W = 128, 8 entries, table of values
+    (4, dict(Lx=256, Ly=12, phi_den=64), 13, 5),                     # W = 256: two tiles per line; tile of 8 + padded tile of 8
+]
+
+
+@pytest.mark.parametrize("cfg,over,n_state,n_step", RW_CASES)
+@pytest.mark.parametrize("kernel", [0, 1, 2])
+def test_lattice_kernels_agree_with_oracle(dev, oracle_mod, cfg, over, n_state, n_step, kernel):
+    """The same lattices on the rolling-window kernel (default), the general kernel (TBPM_OPT_KERNEL = 1) and the phased
+    kernel (2): every element against the serial oracle; seams of the periodic lattice fall back to LDG inside term_rw."""
     w = W.make_workload(cfg, device=dev, **over)
-    run_parity(dev, oracle_mod, w, n_state, n_step)
+    run_parity(dev, oracle_mod, w, n_state, n_step, options={tbpm.TBPM_OPT_KERNEL: kernel})
+
+
+def test_square_nn_lattice_rolling_window(dev, oracle_mod):
+    """4 entries per row (t' = 0): the third instantiated shape of term_rw, with one real hopping value and with phases."""
+    n, hi, hj, hv = W.square_peierls_hops(128, 20, -1.0, 0.0, 1, 32, dev)
+    keep = hv.abs() > 0                                              # drop the t' = 0 entries
+    w = W.Workload("square-nn-flux", n, hi[keep].contiguous(), hj[keep].contiguous(), hv[keep].contiguous(), None, 8, 6, 4.0)
+    run_parity(dev, oracle_mod, w, 8, 6)
+    w.hop_val = torch.full_like(w.hop_val, -1.0)
+    run_parity(dev, oracle_mod, w, 8, 6)
+
+
+@pytest.mark.parametrize("radius,n_phase,n_state", [
+    (2, 1, 8), (2, 16, 1), (2, 1, 4),                                # 12 entries per row: phased kernel, chunked rows
+    (4, 8, 8), (4, 1, 2),                                            # 48 entries: phased kernel at 8 states, general kernel at 2
+    (5, 4, 8), (5, 32, 3),                                           # 80 entries: general kernel with the value table
+])
+@pytest.mark.parametrize("diag", [False, True])
+def test_long_rows(dev, oracle_mod, radius, n_phase, n_state, diag):
+    """Rows of 12 / 48 / 80 entries (hops to every site within a radius; BASELINE.json's configs stop at 8): covers the
+    chunked row loop of term_ph.cuh, its stage-size dispatch, and k_cheb_term<..., TABLE = true> on long rows."""
+    n, hi, hj, hv, row_sum = W.square_range_hops(32, 24, radius, n_phase, dev)
+    onsite = torch.linspace(-0.5, 0.5, n, dtype=torch.float64, device=dev) if diag else None
+    w = W.Workload(f"range{radius}", n, hi, hj, hv, onsite, n_state, 5, row_sum + 0.5)
+    H, _, _, _ = run_parity(dev, oracle_mod, w, n_state, 5)
+    assert H.max_row_nnz == {2: 12, 4: 48, 5: 80}[radius] + int(diag) and H.n_table > 0
+    run_parity(dev, oracle_mod, w, n_state, 3, tbpm.TBPM_NO_TABLE)
 
 
 @pytest.mark.parametrize("cfg,over,n_state,n_step", [
-    (4, dict(Lx=64, Ly=48, phi_den=32), 8, 10),                      # table shape: three segments, rows at the boundary fall back
-    (5, dict(L=17), 16, 9),                                          # cubic shape: five segments, two tiles of states
-    (5, dict(L=32), 8, 6),                                           # tiles wholly inside a lattice line: the LDS-only path
+    (2, dict(Na=96, Nb=70), 4, 8), (3, dict(Na=100, Nb=60), 2, 7), (4, dict(Lx=64, Ly=48, phi_den=32), 8, 6), (5, dict(L=17), 11, 5),
 ])
-def test_staged_gathers(dev, oracle_mod, cfg, over, n_state, n_step, monkeypatch):
-    """term_sg.cu (experimental, TBPM_SG): vector rows of a tile staged in shared memory by bulk copies of lattice runs."""
-    monkeypatch.setenv("TBPM_SG", "1")
+def test_general_kernel_every_shape(dev, oracle_mod, cfg, over, n_state, n_step):
+    """TBPM_OPT_KERNEL = 1: every term on k_cheb_term (the path of tables > 32768 values, tiles of 16 / 32 states, long rows)."""
     w = W.make_workload(cfg, device=dev, **over)
-    run_parity(dev, oracle_mod, w, n_state, n_step)
+    run_parity(dev, oracle_mod, w, n_state, n_step, options={tbpm.TBPM_OPT_KERNEL: 1})
 
 
-@pytest.mark.parametrize("tile", ["1", "2", "4", "16", "32"])
-def test_other_tile_widths(dev, oracle_mod, tile, monkeypatch):
-    monkeypatch.setenv("TBPM_TILE", tile)
+@pytest.mark.parametrize("tile", [1, 2, 4, 16, 32])
+def test_other_tile_widths(dev, oracle_mod, tile):
     w = W.make_workload(5, device=dev, L=13)
-    run_parity(dev, oracle_mod, w, 35 if tile in ("16", "32") else 7, 6)
+    run_parity(dev, oracle_mod, w, 35 if tile >= 16 else 7, 6, options={tbpm.TBPM_OPT_TILE: tile})
     w = W.make_workload(4, device=dev, Lx=48, Ly=32, phi_den=16)
-    run_parity(dev, oracle_mod, w, 33 if tile == "32" else 6, 5, tbpm.TBPM_NO_TABLE)
+    run_parity(dev, oracle_mod, w, 33 if tile == 32 else 6, 5, tbpm.TBPM_NO_TABLE, options={tbpm.TBPM_OPT_TILE: tile})
+
+
+def test_options_and_get_state_checks(dev):
+    w = W.make_workload(2, device=dev, Na=24, Nb=20)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    for opt, bad in ((tbpm.TBPM_OPT_TILE, 3), (tbpm.TBPM_OPT_TILE, 64), (tbpm.TBPM_OPT_KERNEL, 7), (99, 0)):
+        with pytest.raises(tbpm.TbpmError) as ei:
+            tbpm.tbpm_set_option(H, opt, bad)
+        assert ei.value.code == tbpm.TBPM_EINVAL
+    psi0 = w.psi0(device=dev, n_state=3)
+    _, _, ws = tbpm.tbpm_propagate(H, psi0, 2, w.dt, w.rescale)
+    tbpm.tbpm_get_state(H, ws, 2)
+    with pytest.raises(tbpm.TbpmError) as ei:                        # state beyond the call's n_state
+        tbpm.tbpm_get_state(H, ws, 3)
+    assert ei.value.code == tbpm.TBPM_EINDEX
+    other = torch.empty(ws.numel(), dtype=torch.uint8, device=dev)
+    with pytest.raises(tbpm.TbpmError) as ei:                        # a workspace this handle never propagated on
+        tbpm.tbpm_get_state(H, other, 0)
+    assert ei.value.code == tbpm.TBPM_EINVAL
 
 
 @pytest.mark.parametrize("tau,K", [(0.0, 1), (1e-9, None), (math.pi / 2, 16), (2 * math.pi, 28), (1.0, None), (5.3, None)])
