@@ -158,3 +158,82 @@ def dos_from_corr(corr: np.ndarray, rescale: float):
     ph = np.exp(1j * np.pi * np.outer(E / rescale, n))
     D = (1.0 + 2.0 * np.real(ph @ (w * corr))) / (2.0 * rescale)
     return E, D
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# NEXT-3: quasi-eigenstates (QE) and the time-dependent wave function (WFT)
+# ---------------------------------------------------------------------------------------------------------------------
+def quasi_eigenstates(n_orb, onsite, hop_i, hop_j, hop_val, psi0, energies, n_step, dt, rescale, *, hops_full=False, form="hops"):
+    """Quasi-eigenstates of the TBPM solver ("quasi-eigenstates (QE)", Table 7).
+
+    The paper prints no formula (it defers the TBPM mathematics to the v1.3 article); reading #28:
+    the Fourier transform of the time-dependent wave function at the requested energies, one-sided, Hann-windowed like
+    the DOS (reading #27), NOT normalised:
+
+        qe[b][e] = sum_{n=0}^{n_step} w_n exp(+i E_e n dt) psi_b(n dt),   w_n = (1 + cos(pi n / n_step)) / 2,  psi_b(0) = psi0[b]
+
+    psi_b(n dt) is the oracle's own propagation, one time step at a time (oracle_propagate with n_step = 1 started from the
+    previous psi), so that this function adds nothing but the plain loop above.  Returns complex128 [B][n_E][n_orb]."""
+    psi0 = np.atleast_2d(_c128(psi0))
+    E = np.asarray(energies, dtype=np.float64).ravel()
+    B = psi0.shape[0]
+    qe = np.zeros((B, E.size, n_orb), dtype=np.complex128)
+    for b in range(B):
+        psi = psi0[b].copy()
+        for e in range(E.size):
+            qe[b, e] += psi                                           # n = 0: w_0 = 1, phase 1
+        for n in range(1, n_step + 1):
+            _, _, fin = propagate(n_orb, onsite, hop_i, hop_j, hop_val, psi0[b], 1, dt, rescale, psi_start=psi,
+                                  hops_full=hops_full, form=form, return_state=True)
+            psi = fin[0]
+            w = 0.5 * (1.0 + np.cos(np.pi * n / n_step))
+            for e in range(E.size):
+                qe[b, e] += (w * np.exp(1j * E[e] * n * dt)) * psi
+    return qe
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# NEXT-2: Haydock recursion (Lanczos three-term recurrence from a site) and the continued-fraction LDOS
+# ---------------------------------------------------------------------------------------------------------------------
+def haydock(n_orb, onsite, hop_i, hop_j, hop_val, sites, n_iter, *, hops_full=False):
+    """Recursion coefficients of the Haydock method ("LDOS using Haydock recursive method"; capability list
+    PAPER.md:24, 544).  The paper prints no formula; reading #29 -- the textbook recursion from |phi_0> = |site>:
+
+        a_n = <phi_n| H |phi_n>                                   (real: H is Hermitian)
+        w   = H phi_n - a_n phi_n - b_n phi_{n-1}                 (b_0 phi_{-1} = 0)
+        b_{n+1} = ||w||,   phi_{n+1} = w / b_{n+1}
+
+    Returns a [n_site][n_iter] (a_0 .. a_{n_iter-1}) and b [n_site][n_iter] (b_1 .. b_{n_iter}).  A breakdown (b = 0: the
+    Krylov space is exhausted) ends the recursion of that site; the remaining entries are 0."""
+    sites = np.asarray(sites, dtype=np.int64).ravel()
+    a = np.zeros((sites.size, n_iter), dtype=np.float64)
+    b = np.zeros((sites.size, n_iter), dtype=np.float64)
+    for s, site in enumerate(sites):
+        prev = np.zeros(n_orb, dtype=np.complex128)
+        phi = np.zeros(n_orb, dtype=np.complex128)
+        phi[site] = 1.0
+        b_n = 0.0
+        for n in range(n_iter):
+            w = apply_h(n_orb, onsite, hop_i, hop_j, hop_val, phi, hops_full)
+            a_n = float(np.vdot(phi, w).real)
+            w = w - a_n * phi - b_n * prev
+            b_next = float(np.sqrt(np.vdot(w, w).real))
+            a[s, n], b[s, n] = a_n, b_next
+            if b_next == 0.0:
+                break
+            prev, phi, b_n = phi, w / b_next, b_next
+    return a, b
+
+
+def haydock_ldos(a, b, energies, eta):
+    """LDOS from the recursion coefficients: G(z) = 1 / (z - a_0 - b_1^2 / (z - a_1 - b_2^2 / (...))) at z = E + i eta,
+    the fraction cut after a_{n_iter-1} (b_{n_iter} is not used: the chain is simply finite), ldos = -Im G / pi.
+    a, b: [n_iter] of one site (haydock() above).  Evaluated from the bottom up."""
+    a = np.asarray(a, dtype=np.float64).ravel()
+    b = np.asarray(b, dtype=np.float64).ravel()
+    z = np.asarray(energies, dtype=np.float64).ravel() + 1j * eta
+    g = np.zeros_like(z)
+    for n in range(a.size - 1, -1, -1):
+        tail = (b[n] ** 2) * g if n < a.size - 1 else 0.0
+        g = 1.0 / (z - a[n] - tail)
+    return -g.imag / np.pi
