@@ -397,8 +397,40 @@ __global__ void k_tab_lookup(int64_t n_orb, int has_onsite, const int64_t *__res
     }
 }
 
+
+// Lattice strides, step 1: the column words of kSampleRows scattered rows (uniform rows of n_off entries) and the first table
+// value, gathered into one small buffer so that the host needs ONE copy.  out: int32[kSampleRows][n_off] | double2 at byte 8192.
+constexpr int kSampleRows = 64;
+constexpr size_t kSampleBytes = 8192 + 16;
+__global__ void k_sample_rows(int64_t n_orb, int n_off, const int32_t *__restrict__ ocol, const double2 *__restrict__ vtab, int32_t *out)
+{
+    const int i = threadIdx.x / 16, j = threadIdx.x % 16;
+    if (i < kSampleRows && j < n_off) {
+        const int64_t row = (int64_t)(((unsigned long long)(i + 1) * 0x9E3779B97F4A7C15ull >> 11) % (unsigned long long)n_orb);
+        out[i * n_off + j] = ocol[row * n_off + j];
+    }
+    if (threadIdx.x == 0 && vtab) *reinterpret_cast<double2 *>(reinterpret_cast<char *>(out) + 8192) = vtab[0];
+}
+
+struct LatDelta { int64_t d[16]; };
+// Lattice strides, step 2: bit r of lat_flags = "the entries of row r sit exactly where the lattice puts them"
+// (ocol[r][j] == r + delta[j] for every j); status[ST_NREG] counts such rows.  The lattice kernels skip the column words of
+// these rows; all other rows (periodic seams, or a matrix that does not follow the lattice) are gathered entry by entry.
+__global__ void k_lat_flags(int64_t n_orb, int n_off, const int32_t *__restrict__ ocol, LatDelta dl, uint32_t *lat_flags, int32_t *status)
+{
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool ok = r < n_orb;
+    if (ok)
+        for (int j = 0; j < n_off; ++j) ok = ok && (int64_t)(ocol[r * n_off + j] & 0x7fffffff) == r + dl.d[j];
+    const uint32_t bits = __ballot_sync(0xffffffffu, ok);
+    if ((threadIdx.x & 31) == 0) {
+        if (r < n_orb) lat_flags[r >> 5] = bits;
+        if (bits) atomicAdd(&status[ST_NREG], __popc(bits));
+    }
+}
+
 struct PersistLayout {
-    size_t status, rowptr, col, val, orp, ocol, oidx, vtab, diag, total;
+    size_t status, rowptr, col, val, orp, ocol, oidx, vtab, diag, latflag, total;
 };
 
 PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint32_t flags)
@@ -417,12 +449,13 @@ PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint3
     L.oidx = take(sizeof(uint16_t) * nnz_off);
     L.vtab = take(sizeof(double2) * kTableMax);
     L.diag = has_onsite ? take(sizeof(double) * (size_t)n_orb) : 0;
+    L.latflag = take(sizeof(uint32_t) * ((size_t)n_orb / 32 + 2));
     L.total = o;
     return L;
 }
 
 struct ScratchLayout {
-    size_t cnt, cur, bsum, slots, flag, slot_id, keys, ckeys, rank, total;
+    size_t cnt, cur, bsum, slots, flag, slot_id, keys, ckeys, rank, sample, total;
 };
 
 ScratchLayout scratch_layout(int64_t n_orb)
@@ -440,6 +473,7 @@ ScratchLayout scratch_layout(int64_t n_orb)
     L.keys = take(sizeof(unsigned long long) * kHashSlots);
     L.ckeys = take(sizeof(unsigned long long) * kTableMax);
     L.rank = take(sizeof(int32_t) * kTableMax);
+    L.sample = take(kSampleBytes);
     L.total = o;
     return L;
 }
@@ -501,6 +535,7 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
     H->oidx = reinterpret_cast<uint16_t *>(P + PL.oidx);
     H->vtab = reinterpret_cast<double2 *>(P + PL.vtab);
     H->diag = has_onsite ? reinterpret_cast<double *>(P + PL.diag) : nullptr;
+    H->lat_flags = reinterpret_cast<uint32_t *>(P + PL.latflag);
     int32_t *cnt = reinterpret_cast<int32_t *>(S + SL.cnt);
     int32_t *cur = reinterpret_cast<int32_t *>(S + SL.cur);
     int64_t *bsum = reinterpret_cast<int64_t *>(S + SL.bsum);
@@ -510,6 +545,7 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
     unsigned long long *keys = reinterpret_cast<unsigned long long *>(S + SL.keys);
     unsigned long long *ckeys = reinterpret_cast<unsigned long long *>(S + SL.ckeys);
     int32_t *rank = reinterpret_cast<int32_t *>(S + SL.rank);
+    int32_t *sample = reinterpret_cast<int32_t *>(S + SL.sample);
 
     auto fail = [&](int code) { delete H; return code; };
 #define TRY_OR_FAIL(expr)                                                       \
@@ -566,45 +602,53 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
         TRY_OR_FAIL(cudaStreamSynchronize(st));
         H->packed = pack;
         H->single_real = 0;
-        if (n_table == 1) {   // one hopping value; if it is real the kernels sum the neighbours and scale once
-            double2 v0;
-            TRY_OR_FAIL(cudaMemcpyAsync(&v0, H->vtab, sizeof(double2), cudaMemcpyDeviceToHost, st));
-            TRY_OR_FAIL(cudaStreamSynchronize(st));
-            H->single_real = v0.y == 0.0;
-        }
         H->n_table = hst[ST_NTAB];
     }
     // Lattice strides: on a matrix whose rows all have the same length, the column offsets (col - row) of a typical row are
-    // the strides of the lattice (1, a line, a plane).  64 rows spread over the matrix are sampled and the most frequent tuple
-    // of offsets wins (a single sample could sit on the periodic boundary).  propagate walks its tiles along the largest
-    // usable stride, and the staged-gather kernel takes its segments from the tuple.
+    // the strides of the lattice (1, a line, a plane).  64 rows spread over the matrix are sampled (one gather kernel, one
+    // copy) and the most frequent tuple of offsets wins (a single sample could sit on the periodic boundary).  propagate walks
+    // its tiles along the largest usable stride; k_lat_flags then marks the rows that follow the tuple exactly.
     {
         const int n_off = H->max_row_nnz - (has_onsite ? 1 : 0);
-        if (n_orb > 0 && H->min_row_nnz == H->max_row_nnz && n_off > 0 && n_off <= 16) {
-            constexpr int kSamples = 64;
-            std::vector<int32_t> cw((size_t)kSamples * n_off);
-            std::vector<int64_t> rows(kSamples);
-            for (int i = 0; i < kSamples; ++i) {
-                rows[i] = (int64_t)(((unsigned long long)(i + 1) * 0x9E3779B97F4A7C15ull >> 11) % (unsigned long long)n_orb);   // scattered
-                TRY_OR_FAIL(cudaMemcpyAsync(cw.data() + (size_t)i * n_off, H->ocol + rows[i] * n_off, sizeof(int32_t) * n_off,
-                                            cudaMemcpyDeviceToHost, st));
-            }
+        const bool uniform = n_orb > 0 && H->min_row_nnz == H->max_row_nnz && n_off > 0 && n_off <= 16 && H->n_table > 0;
+        if (uniform || H->n_table == 1) {
+            std::vector<int32_t> host(kSampleBytes / sizeof(int32_t));
+            k_sample_rows<<<1, kSampleRows * 16, 0, st>>>(n_orb, uniform ? n_off : 0, H->ocol, H->n_table > 0 ? H->vtab : nullptr, sample);
+            count_launches(1);
+            TRY_OR_FAIL(cudaMemcpyAsync(host.data(), sample, kSampleBytes, cudaMemcpyDeviceToHost, st));
             TRY_OR_FAIL(cudaStreamSynchronize(st));
-            std::vector<std::vector<int64_t>> tup(kSamples, std::vector<int64_t>(n_off));
-            for (int i = 0; i < kSamples; ++i)
-                for (int j = 0; j < n_off; ++j) tup[i][j] = (int64_t)(cw[(size_t)i * n_off + j] & 0x7fffffff) - rows[i];
-            int best = 0, best_count = 0;
-            for (int i = 0; i < kSamples; ++i) {
-                int c = 0;
-                for (int k = 0; k < kSamples; ++k) c += tup[k] == tup[i];
-                if (c > best_count) { best_count = c; best = i; }
+            if (H->n_table == 1) {   // one hopping value; if it is real the kernels sum the neighbours and scale once
+                double2 v0;
+                std::memcpy(&v0, reinterpret_cast<const char *>(host.data()) + 8192, sizeof(double2));
+                H->single_real = v0.y == 0.0;
             }
-            for (int j = 0; j < n_off; ++j) {
-                const int64_t dlt = tup[best][j];
-                H->lat_delta[H->n_lat_off] = dlt;           // signed, in the order of the row's entries
-                H->lat_off[H->n_lat_off++] = dlt > 0 ? dlt : -dlt;
+            if (uniform) {
+                std::vector<std::vector<int64_t>> tup(kSampleRows, std::vector<int64_t>(n_off));
+                for (int i = 0; i < kSampleRows; ++i) {
+                    const int64_t row = (int64_t)(((unsigned long long)(i + 1) * 0x9E3779B97F4A7C15ull >> 11) % (unsigned long long)n_orb);
+                    for (int j = 0; j < n_off; ++j) tup[i][j] = (int64_t)(host[(size_t)i * n_off + j] & 0x7fffffff) - row;
+                }
+                int best = 0, best_count = 0;
+                for (int i = 0; i < kSampleRows; ++i) {
+                    int c = 0;
+                    for (int k = 0; k < kSampleRows; ++k) c += tup[k] == tup[i];
+                    if (c > best_count) { best_count = c; best = i; }
+                }
+                LatDelta dl{};
+                for (int j = 0; j < n_off; ++j) {
+                    const int64_t dlt = tup[best][j];
+                    dl.d[j] = dlt;
+                    H->lat_delta[H->n_lat_off] = dlt;           // signed, in the order of the row's entries
+                    H->lat_off[H->n_lat_off++] = dlt > 0 ? dlt : -dlt;
+                }
+                std::sort(H->lat_off, H->lat_off + H->n_lat_off);
+                k_lat_flags<<<gr, kThreads, 0, st>>>(n_orb, n_off, H->ocol, dl, H->lat_flags, H->status);
+                count_launches(1);
+                int32_t n_reg = 0;
+                TRY_OR_FAIL(cudaMemcpyAsync(&n_reg, H->status + ST_NREG, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+                TRY_OR_FAIL(cudaStreamSynchronize(st));
+                H->n_regular = n_reg;
             }
-            std::sort(H->lat_off, H->lat_off + H->n_lat_off);
         }
     }
 #undef TRY_OR_FAIL

@@ -274,7 +274,8 @@ int launch_term_t(const TermParams &p, int num_sms, cudaStream_t st, int *grid_o
 int launch_term(int bt, bool table, int kernel_opt, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
     const bool general_only = kernel_opt == 1;
-    if (table && kernel_opt == 0 && term_rw_supported(bt, p)) return launch_term_rw(p, num_sms, st, grid_out);
+    if (table && kernel_opt == 0 && term_l3_supported(bt, p)) return launch_term_l3(p, num_sms, st, grid_out);
+    if (table && (kernel_opt == 0 || kernel_opt == 3) && term_rw_supported(bt, p)) return launch_term_rw(p, num_sms, st, grid_out);
     if (table && !general_only && term_ph_supported(bt, p)) {
         switch (bt) {
         case 1: return launch_term_ph_bt1(p, num_sms, st, grid_out);
@@ -376,6 +377,8 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
     tp.walk_stride = 0; tp.walk_run = 1;
     tp.n_lat_off = H->n_lat_off;
     for (int j = 0; j < H->n_lat_off; ++j) { tp.lat_off[j] = H->lat_off[j]; tp.lat_delta[j] = H->lat_delta[j]; }
+    tp.lat_flags = H->lat_flags;
+    tp.n_regular = H->n_regular;
     tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
     // L2 prefetch of the vector rows a few tiles ahead (term_ph.cuh, producer warp).  The leading edge of the gather
@@ -500,7 +503,7 @@ extern "C" int tbpm_set_option(tbpm_ham *H, int option, int64_t value)
         H->opt_tile = (int)value;
         return TBPM_OK;
     case TBPM_OPT_KERNEL:
-        if (value < 0 || value > 2) return TBPM_EINVAL;
+        if (value < 0 || value > 3) return TBPM_EINVAL;
         H->opt_kernel = (int)value;
         return TBPM_OK;
     }

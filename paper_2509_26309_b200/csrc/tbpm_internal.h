@@ -42,7 +42,8 @@ enum StatusWord {
     ST_NTAB = 4,         // number of distinct off-diagonal values inserted into the hash table
     ST_TAB_OVERFLOW = 5, // more than kTableMax distinct values (or a probe sequence gave up)
     ST_NEG_MIN_ROW = 6,  // 2^30 - (fewest entries in a row of the canonical CSR)
-    ST_HALO = 7          // widest |col - row| (circular): how far a row reaches into the vector
+    ST_HALO = 7,         // widest |col - row| (circular): how far a row reaches into the vector
+    ST_NREG = 8          // rows whose entries sit exactly at the lattice offsets (k_lat_flags)
 };
 
 // What the last tbpm_propagate / tbpm_ldos call of a handle left in a workspace (read by tbpm_get_state).
@@ -69,6 +70,7 @@ struct tbpm_ham {
     int32_t n_lat_off = 0;     // uniform rows: |col - row| of the entries of one sample row (lattice strides), ascending
     int64_t lat_off[16] = {0};
     int64_t lat_delta[16] = {0};   // the same offsets signed, in the order of the sample row's entries (slot j -> col - row)
+    int64_t n_regular = 0;         // rows that follow lat_delta exactly (bits of lat_flags)
     double gershgorin = 0.0;
     int32_t n_table = 0;   // 0: kernels read complex128 values from the canonical CSR
     int32_t packed = 0;    // n_table == 1: bit 31 of every ocol word = "conjugate of the table value" (oidx is not read by the kernels)
@@ -85,6 +87,7 @@ struct tbpm_ham {
     uint16_t *oidx = nullptr;
     double2 *vtab = nullptr;
     double *diag = nullptr;
+    uint32_t *lat_flags = nullptr;   // uniform lattices: bit r = row r follows lat_delta exactly
     int32_t *status = nullptr;
 
     // options (tbpm_set_option)

@@ -47,11 +47,16 @@ struct TermParams {
     int n_lat_off;         // lattice strides found by the builder (uniform rows only), ascending
     int64_t lat_off[16];
     int64_t lat_delta[16]; // signed offsets of the sample row's entries, in slot order
+    const uint32_t *lat_flags;  // bit r: row r follows lat_delta exactly (build.cu, k_lat_flags)
+    int64_t n_regular;     // number of such rows
     int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
     int reverse;           // phased kernel: sweep the tiles from the last row block to the first
     int uniform;           // every row holds exactly max_row_off off-diagonal entries
     int single_real;       // the table holds one value and it is real
     int device;            // CUDA device of the handle (per-device launch configuration caches)
+    int zero;              // always 0, but known only at run time: the kernels AND it into the address of the barrier that hands a
+                           // shared-memory stage back, together with the registers their LDS filled, so that the hand-back cannot be
+                           // issued before those loads have returned
     int pf_dist;           // phased kernel: tiles ahead of the staged one whose vector rows are prefetched into L2 (0: off)
     int pf_mask;           // 1: y / psi' / psi0 rows, 2: x rows at the leading edge
     int64_t pf_lead;       // rows between a tile and the leading edge of its gather window (first touch of x)
@@ -105,5 +110,10 @@ int launch_term_ph_bt8(const TermParams &p, int num_sms, cudaStream_t st, int *g
 // tiles; false / TBPM_EINVAL when it does not apply.
 bool term_rw_supported(int bt, const TermParams &p);
 int launch_term_rw(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
+
+// Three-dimensional lattice kernel (term_l3.cu): tiles of 8 states on lattices with offsets {+-1, +-S1, +-S2} and one real hopping
+// value (simple cubic and its anisotropic relatives); two-dimensional tiles with TMA-fed halos, walked along S2.
+bool term_l3_supported(int bt, const TermParams &p);
+int launch_term_l3(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
 }  // namespace tbpm_detail

@@ -357,8 +357,13 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
             }
         }
         if (c0 + CH >= nmax) {                              // last chunk of every row of this warp: the stage is free again
+            // ... once its reads have RETURNED: the barrier address depends on every register they filled (p.zero is 0 at run time)
+            uint32_t rel = (uint32_t)__double2hiint(d);
+#pragma unroll
+            for (int j = 0; j < CH; ++j) rel ^= w[j] ^ id[j];
+            rel &= (uint32_t)p.zero;
             __syncwarp();
-            if ((tid & 31) == 0) mbar_arrive(bar0 + 8 * (kMaxStages + s));
+            if ((tid & 31) == 0) mbar_arrive(bar0 + 8 * (kMaxStages + s) + rel);
             if (++s == S) { s = 0; ph ^= 1u; so = 0; } else so += stage_bytes;
         }
 #pragma unroll

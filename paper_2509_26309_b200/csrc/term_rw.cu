@@ -31,7 +31,7 @@ namespace rw {
 
 using namespace ph;
 
-constexpr int kBT = 8, kNW = 16, kConsumers = kNW * 32, kThreads = kConsumers + 32, kR = kConsumers / 4;   // 128 rows per tile
+constexpr int kBT = 8, kNW = 16, kConsumers = kNW * 32, kThreads = kConsumers + 64, kR = kConsumers / 4;   // 128 rows per tile; two producer warps
 constexpr int kHalo = 1;                                   // halo rows on each side of a ring slot
 constexpr int kRowBytes = kBT * 16;
 constexpr int kSlotBytes = (kR + 2 * kHalo) * kRowBytes;   // 16,640
@@ -48,6 +48,7 @@ struct Geom {
     int slot_src[kMaxSlot];     // where entry j is read: ring slot of tile j-1 / j / j+1, or global memory
     int slot_shift[kMaxSlot];   // row shift inside the ring slot, in [-kHalo, kHalo]
     int lat;                    // which Lat<> the (src, shift) pattern is, -1: none
+    int far_na;                 // far neighbours loaded without L1 allocation
     int off_y, off_col, off_idx, off_diag, stage_bytes;
 };
 
@@ -65,6 +66,10 @@ __device__ __forceinline__ void lds_c_if(double2 &v, uint32_t a, bool on)     //
 __device__ __forceinline__ void ldg_pair(double2 &lo, double2 &hi, const double2 *p)
 {
     asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(lo.x), "=d"(lo.y), "=d"(hi.x), "=d"(hi.y) : "l"(p));
+}
+__device__ __forceinline__ void ldg_pair_na(double2 &lo, double2 &hi, const double2 *p)   // no L1 allocation
+{
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(lo.x), "=d"(lo.y), "=d"(hi.x), "=d"(hi.y) : "l"(p));
 }
 __device__ __forceinline__ void ldg_pair_if(double2 &lo, double2 &hi, const double2 *p, bool on)   // keeps lo / hi when off
 {
@@ -141,42 +146,55 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_rw(const TermParams p, con
     const int64_t n_runs = g.d0 * ((g.n_lines + g.len - 1) / g.len);
 
     if (tid >= kConsumers) {
-        // ------------------------------------------------ producer: one thread ------------------------------------------------
-        if (tid != kConsumers) return;
-        RingPos rp{0u, 1u};                                 // next ring load: slot, parity of its "empty" phase (first pass: free)
-        int s = 0;
-        uint32_t sph = 1;
-        auto ring_load = [&](int64_t row0) {               // rows [row0 - halo, row0 + R + halo) of x, clipped to the vector
-            mbar_wait(b_rempty + 8 * rp.i, rp.ph);
-            const uint32_t full = b_rfull + 8 * rp.i;
-            const int64_t lo = max(row0 - kHalo, (int64_t)0), hi = min(row0 + kR + kHalo, p.n_orb);
-            uint32_t bytes = 0;
-            if (row0 >= 0 && row0 < p.n_orb && hi > lo) {
-                bytes = (uint32_t)(hi - lo) * kRowBytes;
-                bulk_g2s(ring0 + rp.i * kSlotBytes + (uint32_t)(lo - (row0 - kHalo)) * kRowBytes, p.x + lo * kBT, bytes, full);
+        // ------------------------------- producers: one thread of each of the two producer warps -------------------------------
+        // Warp kNW feeds the ring (rows of x, shared by three tiles each), warp kNW + 1 the stages (matrix slices and y of
+        // one tile).  They wait on different "empty" barriers, so neither holds the other back: the ring runs n_ring - 3
+        // tiles ahead of the consumers, the stages n_stage.
+        if ((tid & 31) != 0) return;
+        if (tid == kConsumers) {
+            RingPos rp{0u, 1u};                             // next ring load: slot, parity of its "empty" phase (first pass: free)
+            auto ring_load = [&](int64_t row0) {           // rows [row0 - halo, row0 + R + halo) of x, clipped to the vector
+                mbar_wait(b_rempty + 8 * rp.i, rp.ph);
+                const uint32_t full = b_rfull + 8 * rp.i;
+                const int64_t lo = max(row0 - kHalo, (int64_t)0), hi = min(row0 + kR + kHalo, p.n_orb);
+                uint32_t bytes = 0;
+                if (row0 >= 0 && row0 < p.n_orb && hi > lo) {
+                    bytes = (uint32_t)(hi - lo) * kRowBytes;
+                    bulk_g2s(ring0 + rp.i * kSlotBytes + (uint32_t)(lo - (row0 - kHalo)) * kRowBytes, p.x + lo * kBT, bytes, full);
+                }
+                mbar_expect_tx(full, bytes);
+                rp.adv(NR);
+            };
+            for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
+                const int64_t lb = u / g.d0, pos = u - lb * g.d0;
+                const int64_t line0 = lb * g.len;
+                const int len_u = (int)min((int64_t)g.len, g.n_lines - line0);
+                const int64_t r_first = line0 * g.W + pos * kR;
+                ring_load(r_first - g.W);
+                ring_load(r_first);
+                for (int j = 0; j < len_u; ++j) ring_load(r_first + (int64_t)(j + 1) * g.W);
             }
-            mbar_expect_tx(full, bytes);
-            rp.adv(NR);
-        };
-        for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
-            const int64_t lb = u / g.d0, pos = u - lb * g.d0;
-            const int64_t line0 = lb * g.len;
-            const int len_u = (int)min((int64_t)g.len, g.n_lines - line0);
-            const int64_t r_first = line0 * g.W + pos * kR;
-            for (int j = 0; j < len_u; ++j) {
-                const int64_t r0 = r_first + (int64_t)j * g.W;
-                if (j == 0) { ring_load(r0 - g.W); ring_load(r0); }
-                ring_load(r0 + g.W);
-                mbar_wait(b_sempty + 8 * s, sph);
-                const uint32_t full = b_sfull + 8 * s;
-                const uint32_t st = stage0 + (uint32_t)s * (uint32_t)g.stage_bytes;
-                uint32_t tx = kR * CH * 4;
-                bulk_g2s(st + g.off_col, p.ocol + r0 * CH, kR * CH * 4, full);
-                if (VK == 0) { bulk_g2s(st + g.off_idx, p.oidx + r0 * CH, kR * CH * 2, full); tx += kR * CH * 2; }
-                if (has_diag) { bulk_g2s(st + g.off_diag, p.diag + r0, kR * 8, full); tx += kR * 8; }
-                if (need_y) { bulk_g2s(st + g.off_y, p.y + r0 * kBT, kR * kRowBytes, full); tx += kR * kRowBytes; }
-                mbar_expect_tx(full, tx);
-                if (++s == S) { s = 0; sph ^= 1u; }
+        } else {
+            int s = 0;
+            uint32_t sph = 1;
+            for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
+                const int64_t lb = u / g.d0, pos = u - lb * g.d0;
+                const int64_t line0 = lb * g.len;
+                const int len_u = (int)min((int64_t)g.len, g.n_lines - line0);
+                const int64_t r_first = line0 * g.W + pos * kR;
+                for (int j = 0; j < len_u; ++j) {
+                    const int64_t r0 = r_first + (int64_t)j * g.W;
+                    mbar_wait(b_sempty + 8 * s, sph);
+                    const uint32_t full = b_sfull + 8 * s;
+                    const uint32_t st = stage0 + (uint32_t)s * (uint32_t)g.stage_bytes;
+                    uint32_t tx = kR * CH * 4;
+                    if (need_y) { bulk_g2s(st + g.off_y, p.y + r0 * kBT, kR * kRowBytes, full); tx += kR * kRowBytes; }
+                    bulk_g2s(st + g.off_col, p.ocol + r0 * CH, kR * CH * 4, full);
+                    if (VK == 0) { bulk_g2s(st + g.off_idx, p.oidx + r0 * CH, kR * CH * 2, full); tx += kR * CH * 2; }
+                    if (has_diag) { bulk_g2s(st + g.off_diag, p.diag + r0, kR * 8, full); tx += kR * 8; }
+                    mbar_expect_tx(full, tx);
+                    if (++s == S) { s = 0; sph ^= 1u; }
+                }
             }
         }
         return;
@@ -212,7 +230,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_rw(const TermParams p, con
         for (int k = 0; k < NG; ++k) {
             int64_t c = row + d_far[k];
             c = c < 0 ? 0 : (c > last_row ? last_row : c);  // a clamped prediction is never confirmed (see the check below)
-            ldg_pair(fa[k], fb[k], p.x + c * kBT + 2 * q);
+            if (g.far_na) ldg_pair_na(fa[k], fb[k], p.x + c * kBT + 2 * q); else ldg_pair(fa[k], fb[k], p.x + c * kBT + 2 * q);
         }
     };
     if (NG > 0 && (int64_t)blockIdx.x < n_runs) {
@@ -341,13 +359,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_rw(const TermParams p, con
                 if (nrow >= 0) far_request(nrow);
             }
             if (VK == 2) { ha.x *= t0.x; ha.y *= t0.x; hb.x *= t0.x; hb.y *= t0.x; }
-            // make sure the LDS results the epilogue needs have arrived before the stage is handed back
-            asm volatile("" ::"d"(ya.x), "d"(yb.x), "d"(xra.x), "d"(xrb.x), "d"(d), "d"(ha.x), "d"(hb.x) : "memory");
+            // Every shared-memory read of this tile must have RETURNED before the stage and the oldest ring slot are handed back to
+            // the producers.  A load has returned once an instruction has read its destination register, so the barrier addresses
+            // below are made to depend on all of them (`rel` is 0: p.zero is 0, but only at run time).
+            const uint32_t rel = (uint32_t)(__double2hiint(ya.x) ^ __double2hiint(yb.x) ^ __double2hiint(xra.x) ^ __double2hiint(xrb.x) ^
+                                            __double2hiint(d) ^ __double2hiint(ha.x) ^ __double2hiint(hb.x)) & (uint32_t)p.zero;
             __syncwarp();
             if ((tid & 31) == 0) {
-                mbar_arrive(b_sempty + 8 * s);
-                mbar_arrive(b_rempty + 8 * r0p.i);
-                if (j == len_u - 1) { mbar_arrive(b_rempty + 8 * r1p.i); mbar_arrive(b_rempty + 8 * r2p.i); }
+                mbar_arrive(b_sempty + 8 * s + rel);
+                mbar_arrive(b_rempty + 8 * r0p.i + rel);
+                if (j == len_u - 1) { mbar_arrive(b_rempty + 8 * r1p.i + rel); mbar_arrive(b_rempty + 8 * r2p.i + rel); }
             }
             if (++s == S) { s = 0; sph ^= 1u; st = stage0; } else st += (uint32_t)g.stage_bytes;
             r0p.adv(NR); r1p.adv(NR); r2p.adv(NR);
@@ -462,6 +483,7 @@ bool make_geom(const TermParams &p, Geom &g)
     g.off_idx = (int)o; o += with_idx ? (size_t)kR * n * 2 : 0;
     g.off_diag = (int)o; o += (size_t)kR * 8;
     g.stage_bytes = (int)((o + 127) & ~size_t(127));
+    g.far_na = knob("rw_far_na", 1);
     g.n_ring = std::min(kMaxRing, std::max(4, knob("rw_ring", 5)));
     g.n_stage = std::min(kMaxStages, std::max(2, knob("rw_stages", 4)));
     while ((size_t)g.n_ring * kSlotBytes + (size_t)g.n_stage * g.stage_bytes > kSmemMax - 4096) {

@@ -175,20 +175,24 @@ def test_small_configs_every_element(dev, oracle_mod, cfg, over, n_state, n_step
     run_parity(dev, oracle_mod, w, n_state, n_step, flags)
 
 
-# lattices on which the rolling-window kernel (term_rw.cu) applies: tiles of 8 states, largest stride a multiple of 128 rows
+# lattices on which the lattice kernels apply (tiles of 8 states): term_l3.cu on three-dimensional lattices whose line is a
+# multiple of 32 rows and whose plane a multiple of 4 lines; term_rw.cu when the largest stride is a multiple of 128 rows
 RW_CASES = [
-    (5, dict(L=32), 8, 7),                                           # cubic 32^3: W = 1024 rows, +-line neighbours by LDG, diagonal
-    (5, dict(L=16, W=0.0), 16, 6),                                   # cubic 16^3 (W = 256), no diagonal, two tiles
+    (5, dict(L=32), 8, 7),                                           # cubic 32^3: one tile per line, 8 tile rows per plane, diagonal
+    (5, dict(L=32, W=0.0), 11, 5),                                   # no diagonal; tile of 8 + padded tile of 4 (phased kernel)
+    (5, dict(L=64), 8, 3),                                           # cubic 64^3: two tiles per line, runs of 64 planes
+    (5, dict(L=16, W=0.0), 16, 6),                                   # cubic 16^3 (line of 16 rows: term_rw only, W = 256), two tiles
     (4, dict(Lx=128, Ly=24, phi_den=32), 8, 9),                      # square + flux: W = 128, 8 entries, table of values
     (4, dict(Lx=256, Ly=12, phi_den=64), 13, 5),                     # W = 256: two tiles per line; tile of 8 + padded tile of 8
 ]
 
 
 @pytest.mark.parametrize("cfg,over,n_state,n_step", RW_CASES)
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
 def test_lattice_kernels_agree_with_oracle(dev, oracle_mod, cfg, over, n_state, n_step, kernel):
-    """The same lattices on the rolling-window kernel (default), the general kernel (TBPM_OPT_KERNEL = 1) and the phased
-    kernel (2): every element against the serial oracle; seams of the periodic lattice fall back to LDG inside term_rw."""
+    """The same lattices on the lattice kernels (default: term_l3 where it applies, else term_rw), the general kernel
+    (TBPM_OPT_KERNEL = 1), the phased kernel (2) and term_rw alone (3): every element against the serial oracle; rows on the
+    seams of the periodic lattice are gathered entry by entry inside the lattice kernels."""
     w = W.make_workload(cfg, device=dev, **over)
     run_parity(dev, oracle_mod, w, n_state, n_step, options={tbpm.TBPM_OPT_KERNEL: kernel})
 
