@@ -413,15 +413,37 @@ __global__ void k_sample_rows(int64_t n_orb, int n_off, const int32_t *__restric
 }
 
 struct LatDelta { int64_t d[16]; };
-// Lattice strides, step 2: bit r of lat_flags = "the entries of row r sit exactly where the lattice puts them"
-// (ocol[r][j] == r + delta[j] for every j); status[ST_NREG] counts such rows.  The lattice kernels skip the column words of
-// these rows; all other rows (periodic seams, or a matrix that does not follow the lattice) are gathered entry by entry.
-__global__ void k_lat_flags(int64_t n_orb, int n_off, const int32_t *__restrict__ ocol, LatDelta dl, uint32_t *lat_flags, int32_t *status)
+// Lattice strides, step 2: bit r of lat_flags = "the entries of row r sit exactly where the lattice puts them"; status[ST_NREG]
+// counts such rows.  The lattice kernels skip the column words of these rows; all other rows (a matrix that merely resembles a
+// lattice) are gathered entry by entry.  periodic3 = 0: ocol[r][j] == r + delta[j] for every j (rows on a periodic seam fail).
+// periodic3 = 1 (offsets {-S2, -S1, -1, +1, +S1, +S2}): the six columns are the neighbours of site (x, y, z) = (r % S1,
+// (r / S1) % (S2 / S1), r / S2) on the PERIODIC lattice -- x +- 1 within the line, y +- 1 within the plane, z +- 1 within the
+// volume -- in ascending order; term_l3.cu brings the wrapped halo rows into shared memory, so seam rows need no special path.
+__global__ void k_lat_flags(int64_t n_orb, int n_off, const int32_t *__restrict__ ocol, LatDelta dl, int periodic3, uint32_t *lat_flags,
+                            int32_t *status)
 {
     const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     bool ok = r < n_orb;
-    if (ok)
+    if (ok && !periodic3) {
         for (int j = 0; j < n_off; ++j) ok = ok && (int64_t)(ocol[r * n_off + j] & 0x7fffffff) == r + dl.d[j];
+    } else if (ok) {
+        const int64_t S1 = dl.d[4], S2 = dl.d[5];
+        const int64_t x = r % S1, yz = r / S1, Ly = S2 / S1, y = yz % Ly;
+        int64_t c[6];
+        c[0] = x > 0 ? r - 1 : r - 1 + S1;
+        c[1] = x < S1 - 1 ? r + 1 : r + 1 - S1;
+        c[2] = y > 0 ? r - S1 : r - S1 + S2;
+        c[3] = y < Ly - 1 ? r + S1 : r + S1 - S2;
+        c[4] = r >= S2 ? r - S2 : r - S2 + n_orb;
+        c[5] = r + S2 < n_orb ? r + S2 : r + S2 - n_orb;
+        for (int i = 1; i < 6; ++i) {                       // ascending, as the canonical row is
+            const int64_t v = c[i];
+            int k = i - 1;
+            while (k >= 0 && c[k] > v) { c[k + 1] = c[k]; --k; }
+            c[k + 1] = v;
+        }
+        for (int j = 0; j < 6; ++j) ok = ok && (int64_t)(ocol[r * 6 + j] & 0x7fffffff) == c[j];
+    }
     const uint32_t bits = __ballot_sync(0xffffffffu, ok);
     if ((threadIdx.x & 31) == 0) {
         if (r < n_orb) lat_flags[r >> 5] = bits;
@@ -642,7 +664,11 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
                     H->lat_off[H->n_lat_off++] = dlt > 0 ? dlt : -dlt;
                 }
                 std::sort(H->lat_off, H->lat_off + H->n_lat_off);
-                k_lat_flags<<<gr, kThreads, 0, st>>>(n_orb, n_off, H->ocol, dl, H->lat_flags, H->status);
+                // three-dimensional periodic lattice (a line of S1 rows, a plane of S2, whole planes): wrap-aware bits for term_l3.cu
+                const bool p3 = n_off == 6 && dl.d[2] == -1 && dl.d[3] == 1 && dl.d[4] > 1 && dl.d[5] > dl.d[4] && dl.d[1] == -dl.d[4] &&
+                                dl.d[0] == -dl.d[5] && dl.d[5] % dl.d[4] == 0 && n_orb % dl.d[5] == 0;
+                H->lat_periodic3 = p3 ? 1 : 0;
+                k_lat_flags<<<gr, kThreads, 0, st>>>(n_orb, n_off, H->ocol, dl, p3 ? 1 : 0, H->lat_flags, H->status);
                 count_launches(1);
                 int32_t n_reg = 0;
                 TRY_OR_FAIL(cudaMemcpyAsync(&n_reg, H->status + ST_NREG, sizeof(int32_t), cudaMemcpyDeviceToHost, st));

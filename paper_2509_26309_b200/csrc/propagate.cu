@@ -379,6 +379,7 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
     for (int j = 0; j < H->n_lat_off; ++j) { tp.lat_off[j] = H->lat_off[j]; tp.lat_delta[j] = H->lat_delta[j]; }
     tp.lat_flags = H->lat_flags;
     tp.n_regular = H->n_regular;
+    tp.lat_periodic3 = H->lat_periodic3;
     tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
     // L2 prefetch of the vector rows a few tiles ahead (term_ph.cuh, producer warp).  The leading edge of the gather

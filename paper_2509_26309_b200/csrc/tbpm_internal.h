@@ -71,6 +71,7 @@ struct tbpm_ham {
     int64_t lat_off[16] = {0};
     int64_t lat_delta[16] = {0};   // the same offsets signed, in the order of the sample row's entries (slot j -> col - row)
     int64_t n_regular = 0;         // rows that follow lat_delta exactly (bits of lat_flags)
+    int32_t lat_periodic3 = 0;     // the bits were computed for the periodic three-dimensional lattice (wrapped neighbours count)
     double gershgorin = 0.0;
     int32_t n_table = 0;   // 0: kernels read complex128 values from the canonical CSR
     int32_t packed = 0;    // n_table == 1: bit 31 of every ocol word = "conjugate of the table value" (oidx is not read by the kernels)

@@ -49,6 +49,7 @@ struct TermParams {
     int64_t lat_delta[16]; // signed offsets of the sample row's entries, in slot order
     const uint32_t *lat_flags;  // bit r: row r follows lat_delta exactly (build.cu, k_lat_flags)
     int64_t n_regular;     // number of such rows
+    int lat_periodic3;     // the bits are those of the periodic three-dimensional lattice (wrapped neighbours count as regular)
     int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
     int reverse;           // phased kernel: sweep the tiles from the last row block to the first
     int uniform;           // every row holds exactly max_row_off off-diagonal entries

@@ -112,12 +112,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_l3(const TermParams p, con
     // blocks sweep neighbouring positions of the same planes together (the halos they share are L2 hits).
     const int64_t n_chunks = (g.n_planes + g.len - 1) / g.len;
     const int64_t n_runs = g.n_pos * n_chunks;
-    auto run_row0 = [&](int64_t u, int &len_u) -> int64_t {   // first row of the run's first tile
+    struct Run { int64_t plane0, yg, xg, row0; int len; };   // first plane, tile row and tile column, first row of the first tile
+    auto run_of = [&](int64_t u) -> Run {
+        Run r;
         const int64_t chunk = u / g.n_pos, pos = u - chunk * g.n_pos;
-        const int64_t yg = pos / g.nxg, xg = pos - yg * g.nxg;
-        const int64_t plane0 = chunk * g.len;
-        len_u = (int)min((int64_t)g.len, g.n_planes - plane0);
-        return plane0 * g.S2 + yg * kTY * g.S1 + xg * kTX;
+        r.yg = pos / g.nxg; r.xg = pos - r.yg * g.nxg;
+        r.plane0 = chunk * g.len;
+        r.len = (int)min((int64_t)g.len, g.n_planes - r.plane0);
+        r.row0 = r.plane0 * g.S2 + r.yg * kTY * g.S1 + r.xg * kTX;
+        return r;
     };
 
     if (tid >= kConsumers) {
@@ -125,39 +128,45 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_l3(const TermParams p, con
         if ((tid & 31) != 0) return;
         if (tid == kConsumers) {
             RingPos rp{0u, 1u};                             // next ring load: slot, parity of its "empty" phase (first pass: free)
-            auto ring_load = [&](int64_t row0) {           // the tile at row0 with its halo, clipped to the vector
+            const int64_t Ly = g.S2 / g.S1;
+            // the tile at (plane, yg, xg) with its halo; planes, lines and in-line positions wrap round the periodic lattice, so
+            // the rows on its seams find their neighbours in the slot like everybody else
+            auto ring_load = [&](int64_t plane, int64_t yg, int64_t xg) {
                 mbar_wait(b_rempty + 8 * rp.i, rp.ph);
                 const uint32_t full = b_rfull + 8 * rp.i;
                 const uint32_t slot = ring0 + rp.i * kSlotBytes;
-                uint32_t bytes = 0;
+                if (plane < 0) plane += g.n_planes;
+                if (plane >= g.n_planes) plane -= g.n_planes;
+                const int64_t x0 = xg * kTX;
+                const bool wrap_lo = x0 == 0, wrap_hi = x0 + kTX == g.S1;
 #pragma unroll 1
                 for (int sgm = 0; sgm < kSegs; ++sgm) {
-                    const int64_t g0 = row0 + (int64_t)(sgm - 1) * g.S1 - 1;
-                    const int64_t lo = max(g0, (int64_t)0), hi = min(g0 + kSegRows, p.n_orb);
-                    if (hi > lo) {
-                        const uint32_t nb = (uint32_t)(hi - lo) * kRowBytes;
-                        bulk_g2s(slot + (uint32_t)sgm * kSegBytes + (uint32_t)(lo - g0) * kRowBytes, p.x + lo * kBT, nb, full);
-                        bytes += nb;
-                    }
+                    int64_t yl = yg * kTY - 1 + sgm;
+                    if (yl < 0) yl += Ly;
+                    if (yl >= Ly) yl -= Ly;
+                    const double2 *line = p.x + (plane * g.S2 + yl * g.S1) * kBT;
+                    const uint32_t dst = slot + (uint32_t)sgm * kSegBytes;
+                    const int lo = wrap_lo ? 0 : -1, hi = wrap_hi ? kTX : kTX + 1;       // in-line rows [x0 + lo, x0 + hi) in one piece
+                    bulk_g2s(dst + (uint32_t)(lo + 1) * kRowBytes, line + (x0 + lo) * kBT, (uint32_t)(hi - lo) * kRowBytes, full);
+                    if (wrap_lo) bulk_g2s(dst, line + (g.S1 - 1) * kBT, kRowBytes, full);
+                    if (wrap_hi) bulk_g2s(dst + (uint32_t)(kTX + 1) * kRowBytes, line, kRowBytes, full);
                 }
-                mbar_expect_tx(full, bytes);
+                mbar_expect_tx(full, kSlotBytes);
                 rp.adv(NR);
             };
             for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
-                int len_u;
-                const int64_t r_first = run_row0(u, len_u);
-                ring_load(r_first - g.S2);
-                ring_load(r_first);
-                for (int j = 0; j < len_u; ++j) ring_load(r_first + (int64_t)(j + 1) * g.S2);
+                const Run r = run_of(u);
+                ring_load(r.plane0 - 1, r.yg, r.xg);
+                ring_load(r.plane0, r.yg, r.xg);
+                for (int j = 0; j < r.len; ++j) ring_load(r.plane0 + j + 1, r.yg, r.xg);
             }
         } else {
             int s = 0;
             uint32_t sph = 1;
             for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
-                int len_u;
-                const int64_t r_first = run_row0(u, len_u);
-                for (int j = 0; j < len_u; ++j) {
-                    const int64_t r0 = r_first + (int64_t)j * g.S2;
+                const Run run = run_of(u);
+                for (int j = 0; j < run.len; ++j) {
+                    const int64_t r0 = run.row0 + (int64_t)j * g.S2;
                     mbar_wait(b_sempty + 8 * s, sph);
                     const uint32_t full = b_sfull + 8 * s;
                     const uint32_t st = stage0 + (uint32_t)s * (uint32_t)g.stage_bytes;
@@ -219,19 +228,31 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_l3(const TermParams p, con
         return h;
     };
 
+    // the regular-row bits of a tile's two segments are fetched one tile ahead (an L2 round trip off the critical path)
+    uint32_t fwA = 0, fwB = 0;
+    if ((int64_t)blockIdx.x < n_runs) {
+        const int64_t r0 = run_of(blockIdx.x).row0;
+        fwA = __ldg(p.lat_flags + ((r0 + roff0) >> 5)); fwB = __ldg(p.lat_flags + ((r0 + roff1) >> 5));
+    }
 #pragma unroll 1
     for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
-        int len_u;
-        int64_t row0 = run_row0(u, len_u);
+        const Run run = run_of(u);
+        const int len_u = run.len;
+        int64_t row0 = run.row0;
+        const int64_t next_run_row0 = u + gridDim.x < n_runs ? run_of(u + gridDim.x).row0 : -1;
 #pragma unroll 1
         for (int j = 0; j < len_u; ++j, row0 += g.S2) {
             const int64_t rowA = row0 + roff0, rowB = row0 + roff1;
             const int64_t eA = rowA * kBT + sb, eB = rowB * kBT + sb;
-            // ---- operands that are not staged (HBM latency: issue first): psi', psi0, the regular-row bits of the two segments
+            // ---- operands that are not staged (HBM latency: issue first): psi', psi0
             double2 aoldA, aoldB, zA, zB;
             if (NACC > 0) { aoldA = ldg_stream_if(p.acc + eA, need_acc); aoldB = ldg_stream_if(p.acc + eB, need_acc); }
             if (REDUCE) { zA = ldg_stream_if(p.psi0 + eA, true); zB = ldg_stream_if(p.psi0 + eB, true); }
-            const uint32_t fwA = __ldg(p.lat_flags + (rowA >> 5)), fwB = __ldg(p.lat_flags + (rowB >> 5));
+            const bool bitA = (fwA >> (rowA & 31)) & 1u, bitB = (fwB >> (rowB & 31)) & 1u;
+            {
+                const int64_t nr0 = j + 1 < len_u ? row0 + g.S2 : next_run_row0;
+                if (nr0 >= 0) { fwA = __ldg(p.lat_flags + ((nr0 + roff0) >> 5)); fwB = __ldg(p.lat_flags + ((nr0 + roff1) >> 5)); }
+            }
             // ---- wait: the ring slots of this tile (the first tile of a run waits for all three), then the stage
             if (j == 0) {
                 mbar_wait(b_rfull + 8 * r0p.i, r0p.ph);
@@ -240,8 +261,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_l3(const TermParams p, con
             mbar_wait(b_rfull + 8 * r2p.i, r2p.ph);
             mbar_wait(b_sfull + 8 * s, sph);
             const uint32_t bp = ring0 + r0p.i * kSlotBytes, bo = ring0 + r1p.i * kSlotBytes, bn = ring0 + r2p.i * kSlotBytes;
-            const bool fastA = __all_sync(0xffffffffu, (fwA >> (rowA & 31)) & 1u);
-            const bool fastB = __all_sync(0xffffffffu, (fwB >> (rowB & 31)) & 1u);
+            const bool fastA = __all_sync(0xffffffffu, bitA);
+            const bool fastB = __all_sync(0xffffffffu, bitB);
             double2 hA, hB;
             if (fastA) hA = gather_fast(bp, bo, bn, own0); else hA = gather_slow(rowA);
             if (fastB) hB = gather_fast(bp, bo, bn, own1); else hB = gather_slow(rowB);
@@ -312,7 +333,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_l3(const TermParams p, con
 // Strides and stage layout from the sample row's offsets.  false when they do not describe a lattice this kernel is meant for.
 bool make_geom(const TermParams &p, Geom &g)
 {
-    if (!p.uniform || !p.single_real || p.max_row_off != kCH || p.n_lat_off != kCH || !p.lat_flags) return false;
+    if (!p.uniform || !p.single_real || p.max_row_off != kCH || p.n_lat_off != kCH || !p.lat_flags || !p.lat_periodic3) return false;
     if (p.n_orb <= 0 || p.n_orb >= ((int64_t)1 << 31)) return false;
     const int64_t S1 = p.lat_delta[4], S2 = p.lat_delta[5];
     if (!(p.lat_delta[0] == -S2 && p.lat_delta[1] == -S1 && p.lat_delta[2] == -1 && p.lat_delta[3] == 1 && S1 > 1 && S2 > S1)) return false;
