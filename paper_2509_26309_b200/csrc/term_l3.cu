@@ -124,34 +124,35 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_l3(const TermParams p, con
     };
 
     if (tid >= kConsumers) {
-        // ------------------------------- producers: one thread of each of the two producer warps -------------------------------
-        if ((tid & 31) != 0) return;
-        if (tid == kConsumers) {
+        // ------------------------------------------------ two producer warps ------------------------------------------------
+        // Warp kNW feeds the ring, warp kNW + 1 the stages.  A single thread would need ~2,500 cycles for the address arithmetic
+        // and the 6-18 bulk copies of one ring slot -- as long as the consumers need for the tile -- so the copies of a slot are
+        // issued by one LANE per segment (ring: kTY + 2 lanes, stage: kTY lanes); lane 0 posts the byte count.
+        const int lane = tid & 31;
+        if (tid < kConsumers + 32) {
             RingPos rp{0u, 1u};                             // next ring load: slot, parity of its "empty" phase (first pass: free)
             const int64_t Ly = g.S2 / g.S1;
             // the tile at (plane, yg, xg) with its halo; planes, lines and in-line positions wrap round the periodic lattice, so
             // the rows on its seams find their neighbours in the slot like everybody else
             auto ring_load = [&](int64_t plane, int64_t yg, int64_t xg) {
-                mbar_wait(b_rempty + 8 * rp.i, rp.ph);
-                const uint32_t full = b_rfull + 8 * rp.i;
-                const uint32_t slot = ring0 + rp.i * kSlotBytes;
-                if (plane < 0) plane += g.n_planes;
-                if (plane >= g.n_planes) plane -= g.n_planes;
-                const int64_t x0 = xg * kTX;
-                const bool wrap_lo = x0 == 0, wrap_hi = x0 + kTX == g.S1;
-#pragma unroll 1
-                for (int sgm = 0; sgm < kSegs; ++sgm) {
-                    int64_t yl = yg * kTY - 1 + sgm;
+                if (lane < kSegs) {
+                    mbar_wait(b_rempty + 8 * rp.i, rp.ph);
+                    const uint32_t full = b_rfull + 8 * rp.i;
+                    if (lane == 0) mbar_expect_tx(full, kSlotBytes);
+                    if (plane < 0) plane += g.n_planes;
+                    if (plane >= g.n_planes) plane -= g.n_planes;
+                    const int64_t x0 = xg * kTX;
+                    const bool wrap_lo = x0 == 0, wrap_hi = x0 + kTX == g.S1;
+                    int64_t yl = yg * kTY - 1 + lane;
                     if (yl < 0) yl += Ly;
                     if (yl >= Ly) yl -= Ly;
                     const double2 *line = p.x + (plane * g.S2 + yl * g.S1) * kBT;
-                    const uint32_t dst = slot + (uint32_t)sgm * kSegBytes;
+                    const uint32_t dst = ring0 + rp.i * kSlotBytes + (uint32_t)lane * kSegBytes;
                     const int lo = wrap_lo ? 0 : -1, hi = wrap_hi ? kTX : kTX + 1;       // in-line rows [x0 + lo, x0 + hi) in one piece
                     bulk_g2s(dst + (uint32_t)(lo + 1) * kRowBytes, line + (x0 + lo) * kBT, (uint32_t)(hi - lo) * kRowBytes, full);
                     if (wrap_lo) bulk_g2s(dst, line + (g.S1 - 1) * kBT, kRowBytes, full);
                     if (wrap_hi) bulk_g2s(dst + (uint32_t)(kTX + 1) * kRowBytes, line, kRowBytes, full);
                 }
-                mbar_expect_tx(full, kSlotBytes);
                 rp.adv(NR);
             };
             for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
@@ -163,21 +164,19 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_l3(const TermParams p, con
         } else {
             int s = 0;
             uint32_t sph = 1;
+            const uint32_t tx = (need_y ? kR * kRowBytes : 0u) + (has_diag ? kR * 8u : 0u);
             for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
                 const Run run = run_of(u);
                 for (int j = 0; j < run.len; ++j) {
-                    const int64_t r0 = run.row0 + (int64_t)j * g.S2;
-                    mbar_wait(b_sempty + 8 * s, sph);
-                    const uint32_t full = b_sfull + 8 * s;
-                    const uint32_t st = stage0 + (uint32_t)s * (uint32_t)g.stage_bytes;
-                    uint32_t tx = 0;
-#pragma unroll
-                    for (int ty = 0; ty < kTY; ++ty) {
-                        const int64_t r = r0 + (int64_t)ty * g.S1;
-                        if (need_y) { bulk_g2s(st + g.off_y + ty * (kTX * kRowBytes), p.y + r * kBT, kTX * kRowBytes, full); tx += kTX * kRowBytes; }
-                        if (has_diag) { bulk_g2s(st + g.off_diag + ty * (kTX * 8), p.diag + r, kTX * 8, full); tx += kTX * 8; }
+                    if (lane < kTY) {
+                        const int64_t r = run.row0 + (int64_t)j * g.S2 + (int64_t)lane * g.S1;
+                        mbar_wait(b_sempty + 8 * s, sph);
+                        const uint32_t full = b_sfull + 8 * s;
+                        const uint32_t st = stage0 + (uint32_t)s * (uint32_t)g.stage_bytes;
+                        if (lane == 0) mbar_expect_tx(full, tx);
+                        if (need_y) bulk_g2s(st + g.off_y + lane * (kTX * kRowBytes), p.y + r * kBT, kTX * kRowBytes, full);
+                        if (has_diag) bulk_g2s(st + g.off_diag + lane * (kTX * 8), p.diag + r, kTX * 8, full);
                     }
-                    mbar_expect_tx(full, tx);
                     if (++s == S) { s = 0; sph ^= 1u; }
                 }
             }
