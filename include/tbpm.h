@@ -147,6 +147,30 @@ int64_t tbpm_total_launch_count(void);
  * out [2 n_step + 1].  Plain direct transform (n_step <= a few thousand), one thread per energy.  Asynchronous on `stream`. */
 int tbpm_dos(const double *corr, int n_state, int n_step, double dt, double rescale, double *energy, double *dos, void *stream);
 
+/* ---- NEXT-3: quasi-eigenstates (QE) and the time-dependent wave function (WFT) ----------------------------------------------
+ * "quasi-eigenstates (QE) and time-dependent wave function (WFT)" are solver functions of the paper (Table 7,
+ * PAPER.md:1748-1749); it prints no formula (the TBPM mathematics is deferred to the v1.3 article).
+ * reading #28: the one-sided, Hann-windowed Fourier transform of psi(t) at the requested energies, NOT normalised,
+ *     qe[b][e] = sum_{n=0}^{n_step} w_n exp(+i E_e n dt) psi_b(n dt),   w_n = (1 + cos(pi n / n_step)) / 2,   psi_b(0) = psi0[b],
+ * accumulated during the same propagation that yields corr / norm2 (same arguments and results as tbpm_propagate).  WFT is
+ * tbpm_get_state after a call with n_step = j.  energies: host [n_energy], n_energy <= 16, in the energy unit of H.
+ * qe: device out [n_state][n_energy][n_orb][2].  The workspace is that of tbpm_propagate plus n_energy vectors of one tile. */
+int tbpm_propagate_qe_bytes(const tbpm_ham *H, int n_state, int n_energy, size_t *workspace_bytes);
+int tbpm_propagate_qe(tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale,
+                      const double *energies /* host */, int n_energy, double *corr, double *norm2, double *qe /* device out */,
+                      void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- NEXT-2: Haydock recursion ("LDOS using Haydock recursive method"; Table 7) ----
+ * The paper prints no formula; reading #29, the textbook recursion from |phi_0> = |site>:
+ *     a_n = <phi_n|H|phi_n>,   b_{n+1} phi_{n+1} = H phi_n - a_n phi_n - b_n phi_{n-1},   b_{n+1} = || . ||,   b_0 phi_{-1} = 0.
+ * a: device out [n_site][n_iter] = a_0 .. a_{n_iter-1};  b: device out [n_site][n_iter] = b_1 .. b_{n_iter}.  The LDOS follows on
+ * the host from the continued fraction G(z) = 1 / (z - a_0 - b_1^2 / (z - a_1 - ...)) (kilobytes; see oracle.haydock_ldos).
+ * H is NOT rescaled.  After a breakdown (b = 0: Krylov space exhausted) the remaining coefficients are 0.  sites: host [n_site].
+ * workspace: tbpm_propagate_bytes(H, n_site).  Two sweeps per iteration: H u_n fused with <u_n|H u_n> (the fused last-term
+ * kernel), then the three-vector update fused with the norm. */
+int tbpm_haydock(tbpm_ham *H, const int64_t *sites /* host */, int n_site, int n_iter, double *a /* device out */,
+                 double *b /* device out */, void *workspace, size_t workspace_bytes, void *stream);
+
 /* ---- end to end with HOST buffers ------------------------------------------------------------------------------------
  * Whole path for host-resident inputs: H2D of the list and psi0, tbpm_build, tbpm_propagate, D2H of corr/norm2, then a
  * stream synchronise.  `arena` is caller-owned device memory of at least tbpm_corr_host_bytes(); host buffers should be

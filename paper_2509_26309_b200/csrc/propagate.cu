@@ -34,6 +34,7 @@ namespace {
 constexpr int kThreads = 256;
 constexpr size_t kHeaderBytes = 256;
 constexpr size_t kPartialBytes = sizeof(double) * 3 * kMaxBT * kMaxGrid;
+constexpr size_t kAuxBytes = 64 * 1024;
 
 __device__ __forceinline__ double2 ld_stream(const double2 *p) { return __ldcs(p); }     // read once: evict first
 __device__ __forceinline__ void st_stream(double2 *p, double2 v) { __stcs(p, v); }
@@ -210,6 +211,100 @@ __global__ void k_get_state(const double2 *__restrict__ psi, int64_t n_orb, int 
         out[row] = psi[row * bt + b];
 }
 
+
+// NEXT-3 (quasi-eigenstates): qe[e][i] (+)= c_e * psi[i] on one tile of interleaved states, for up to kMaxEnergy energies.
+constexpr int kMaxEnergy = 16;
+struct QeCoef { double2 c[kMaxEnergy]; };
+__global__ void k_qe_axpy(const double2 *__restrict__ psi, int64_t n_el, int n_e, QeCoef cf, size_t stride, double2 *qe, int init)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_el; i += (int64_t)gridDim.x * blockDim.x) {
+        const double2 v = psi[i];
+        for (int e = 0; e < n_e; ++e) {
+            double2 *q = qe + (size_t)e * stride + i;
+            double2 s = init ? make_double2(0.0, 0.0) : *q;
+            cfma(s, cf.c[e], v);
+            *q = s;
+        }
+    }
+}
+// interleaved tile buffers [e][row][bt] -> caller order qe[state0 + b][e][row]
+__global__ void k_qe_export(const double2 *__restrict__ qe_ws, size_t stride, int64_t n_orb, int bt, int n_valid, int state0, int n_e, double2 *out)
+{
+    const int64_t total = n_orb * n_valid * n_e;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t row = t % n_orb;
+        const int e = (int)((t / n_orb) % n_e), b = (int)(t / (n_orb * n_e));
+        out[((int64_t)(state0 + b) * n_e + e) * n_orb + row] = qe_ws[(size_t)e * stride + row * bt + b];
+    }
+}
+
+// NEXT-2 (Haydock recursion), per tile of interleaved states.  Vectors are kept UNNORMALISED (u_n = beta_n phi_n) so that one
+// iteration is two sweeps: t = H u_n with <u_n|t> (the fused last-term kernel), then
+//     u_{n+1} = t / beta_n - (a_n / beta_n) u_n - (beta_n / beta_{n-1}) u_{n-1},   a_n = Re<u_n|t> / beta_n^2,   b_{n+1} = ||u_{n+1}||
+// which is the textbook  b_{n+1} phi_{n+1} = H phi_n - a_n phi_n - b_n phi_{n-1}  with b_n = beta_n.
+// sc[b] = {Re<u_n|t>, beta_n, beta_{n-1}, unused}; a zero beta (Krylov space exhausted, or a padding state) gives zeros from then on.
+__global__ void k_haydock_update(const double2 *__restrict__ t, const double2 *__restrict__ u, double2 *u_prev, int64_t n_orb, int bt,
+                                 const double *__restrict__ sc, double *partial)
+{
+    __shared__ double sm[256 / 32][kMaxBT];
+    const int b = threadIdx.x % bt;
+    const double dot = sc[4 * b], beta = sc[4 * b + 1], beta_p = sc[4 * b + 2];
+    const double ib = beta > 0.0 ? 1.0 / beta : 0.0;
+    const double a_n = dot * ib * ib;
+    const double c_prev = beta_p > 0.0 ? beta / beta_p : 0.0;
+    double nn = 0.0;
+    const int64_t n_el = n_orb * bt;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_el; i += (int64_t)gridDim.x * blockDim.x) {   // stride is a multiple of bt
+        const double2 tv = t[i], uv = u[i], pv = u_prev[i];
+        double2 w;
+        w.x = (tv.x - a_n * uv.x) * ib - c_prev * pv.x;
+        w.y = (tv.y - a_n * uv.y) * ib - c_prev * pv.y;
+        u_prev[i] = w;
+        nn = fma(w.x, w.x, nn);
+        nn = fma(w.y, w.y, nn);
+    }
+    for (int o = 16; o >= bt; o >>= 1) nn += __shfl_xor_sync(0xffffffffu, nn, o);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane < bt) sm[warp][lane] = nn;
+    __syncthreads();
+    if (threadIdx.x < bt) {
+        double s = 0.0;
+        for (int w2 = 0; w2 < 256 / 32; ++w2) s += sm[w2][threadIdx.x];
+        partial[(int64_t)blockIdx.x * bt + threadIdx.x] = s;
+    }
+}
+// block = state: a_n, b_{n+1} out; scalars rotated for the next iteration.  dot_partial: [grid_dot][bt][3] of the term kernel.
+__global__ void k_haydock_scalars(const double *__restrict__ dot_partial, int grid_dot, int bt, double *sc, int phase,
+                                  const double *__restrict__ nn_partial, int grid_nn, int n_valid, int state0, int n_iter, int it, double *a_out,
+                                  double *b_out)
+{
+    const int b = blockIdx.x, lane = threadIdx.x;
+    double s = 0.0;
+    if (phase == 0) {                                       // after the H application: Re<u_n|t>
+        for (int k = lane; k < grid_dot; k += 32) s += dot_partial[((int64_t)k * bt + b) * 3];
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) sc[4 * b] = s;
+    } else {                                                // after the update: beta_{n+1}; publish a_n, b_{n+1}
+        for (int k = lane; k < grid_nn; k += 32) s += nn_partial[(int64_t)k * bt + b];
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) {
+            const double beta = sc[4 * b + 1], dot = sc[4 * b];
+            const double a_n = beta > 0.0 ? dot / (beta * beta) : 0.0, bn = sqrt(s);
+            if (b < n_valid) {
+                a_out[(int64_t)(state0 + b) * n_iter + it] = a_n;
+                b_out[(int64_t)(state0 + b) * n_iter + it] = bn;
+            }
+            sc[4 * b + 2] = beta;
+            sc[4 * b + 1] = bn;
+        }
+    }
+}
+__global__ void k_haydock_init(double *sc, int bt, int n_valid)
+{
+    const int b = threadIdx.x;
+    if (b < bt) { sc[4 * b] = 0.0; sc[4 * b + 1] = b < n_valid ? 1.0 : 0.0; sc[4 * b + 2] = 0.0; sc[4 * b + 3] = 0.0; }
+}
+
 // ---------------------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------------------
@@ -225,7 +320,7 @@ struct Plan {
     int n_tile;
     int last_bt;         // padded size of the last tile
     size_t full_vec;     // bytes of one vector buffer of a full tile
-    size_t sites_off, partial_off, vec0_off, total;
+    size_t sites_off, partial_off, aux_off, vec0_off, total;
 };
 
 Plan make_plan(int64_t n_orb, int n_state, int tile_max)
@@ -241,6 +336,8 @@ Plan make_plan(int64_t n_orb, int n_state, int tile_max)
     o += align_up(sizeof(int64_t) * (size_t)std::max(n_state, 1));
     P.partial_off = o;
     o += kPartialBytes;
+    P.aux_off = o;                                        // scalars and norm partials of tbpm_haydock
+    o += kAuxBytes;
     P.vec0_off = o;
     o += (size_t)P.n_tile * 4 * P.full_vec;
     P.total = o;
@@ -333,8 +430,10 @@ void step_terms(const TermParams &base, int K, const std::vector<double> &cf, do
 }
 
 // Shared body of tbpm_propagate (psi0 != NULL) and tbpm_ldos (sites != NULL).
+struct QeSpec { const double *energies; int n_energy; double *out; };   // NEXT-3: energies on the host, out on the device
+
 int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int n_step, double dt, double rescale, double *corr,
-        double *norm2, void *workspace, size_t workspace_bytes, void *stream)
+        double *norm2, void *workspace, size_t workspace_bytes, void *stream, const QeSpec *qe = nullptr)
 {
     if (!H || n_state < 0 || n_step < 0 || !(rescale > 0.0) || !(dt >= 0.0) || !std::isfinite(dt) || !std::isfinite(rescale))
         return TBPM_EINVAL;
@@ -347,7 +446,8 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
         for (int b = 0; b < n_state; ++b)
             if (sites[b] < 0 || sites[b] >= H->n_orb) return TBPM_EINDEX;
     const Plan P = make_plan(H->n_orb, n_state, H->opt_tile);
-    if (workspace_bytes < P.total) return TBPM_ENOMEM;
+    const size_t qe_bytes = qe ? (size_t)qe->n_energy * P.full_vec : 0;
+    if (workspace_bytes < P.total + qe_bytes) return TBPM_ENOMEM;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
 
     // a1: coefficients (host, once per call)
@@ -414,6 +514,20 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
         }
         tp.psi0 = bra;
         int slot = start_slot;
+        double2 *qe_ws = reinterpret_cast<double2 *>(W + P.total);   // [n_energy][row][bt] of this tile (NEXT-3)
+        const size_t qe_stride = P.full_vec / sizeof(double2);
+        const unsigned qe_grid = (unsigned)std::min<int64_t>((n_el + kThreads - 1) / kThreads, (int64_t)H->num_sms * 8);
+        auto qe_add = [&](const double2 *psi, int n) {       // qe[e] += w_n exp(+i E_e n dt) psi(n dt), Hann window w_n
+            QeCoef cf{};
+            const long double wn = 0.5L * (1.0L + cosl(3.14159265358979323846264338327950288L * (long double)n / (long double)n_step));
+            for (int e = 0; e < qe->n_energy; ++e) {
+                const long double ph = (long double)qe->energies[e] * (long double)n * (long double)dt;
+                cf.c[e] = make_double2((double)(wn * cosl(ph)), (double)(wn * sinl(ph)));
+            }
+            k_qe_axpy<<<qe_grid, kThreads, 0, st>>>(psi, n_el, qe->n_energy, cf, qe_stride, qe_ws, n == 0);
+            count_launches(1);
+        };
+        if (qe && n_el > 0) qe_add(buf[start_slot], 0);
         for (int n = 0; n < n_step; ++n) {
             double2 *psi = buf[slot], *t1 = buf[(slot + 1) % 3], *acc = buf[(slot + 2) % 3];
             int grid = 1;
@@ -429,6 +543,12 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
             k_reduce_final<<<bt, 96, 0, st>>>(partial, grid, bt, n_valid, state0, n_step, n, corr, norm2);
             count_launches(1);
             slot = (slot + 2) % 3;                        // psi' (acc) is the next step's psi
+            if (qe && n_el > 0) qe_add(buf[slot], n + 1);
+        }
+        if (qe && n_el > 0) {
+            k_qe_export<<<qe_grid, kThreads, 0, st>>>(qe_ws, qe_stride, H->n_orb, bt, n_valid, state0, qe->n_energy,
+                                                      reinterpret_cast<double2 *>(qe->out));
+            count_launches(1);
         }
     }
     TBPM_CUDA_TRY(cudaGetLastError());
@@ -465,6 +585,93 @@ extern "C" int tbpm_ldos(tbpm_ham *H, const int64_t *sites, int n_site, int n_st
 {
     if (n_site > 0 && n_step > 0 && !sites) return TBPM_EINVAL;
     return run(H, nullptr, sites, n_site, n_step, dt, rescale, corr, norm2, workspace, workspace_bytes, stream);
+}
+
+
+extern "C" int tbpm_propagate_qe_bytes(const tbpm_ham *H, int n_state, int n_energy, size_t *workspace_bytes)
+{
+    if (!H || n_state < 0 || n_energy < 0 || n_energy > kMaxEnergy || !workspace_bytes) return TBPM_EINVAL;
+    const Plan P = make_plan(H->n_orb, n_state, H->opt_tile);
+    *workspace_bytes = P.total + (size_t)n_energy * P.full_vec;
+    return TBPM_OK;
+}
+
+extern "C" int tbpm_propagate_qe(tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale,
+                                 const double *energies, int n_energy, double *corr, double *norm2, double *qe, void *workspace,
+                                 size_t workspace_bytes, void *stream)
+{
+    if (n_energy < 0 || n_energy > kMaxEnergy || (n_energy > 0 && (!energies || !qe))) return TBPM_EINVAL;
+    if (n_state > 0 && n_step > 0 && !psi0) return TBPM_EINVAL;
+    for (int e = 0; e < n_energy; ++e)
+        if (!std::isfinite(energies[e])) return TBPM_EINVAL;
+    QeSpec spec{energies, n_energy, qe};
+    return run(H, psi0, nullptr, n_state, n_step, dt, rescale, corr, norm2, workspace, workspace_bytes, stream, n_energy > 0 ? &spec : nullptr);
+}
+
+// NEXT-2: Haydock recursion from the given sites.  Workspace = that of tbpm_propagate for n_site states (three rotating vectors
+// per tile are enough; the fourth holds nothing here).
+extern "C" int tbpm_haydock(tbpm_ham *H, const int64_t *sites, int n_site, int n_iter, double *a_out, double *b_out, void *workspace,
+                            size_t workspace_bytes, void *stream)
+{
+    if (!H || n_site < 0 || n_iter < 0) return TBPM_EINVAL;
+    if (n_site == 0 || n_iter == 0) return TBPM_OK;
+    if (!sites || !a_out || !b_out || !workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return TBPM_EINVAL;
+    for (int b = 0; b < n_site; ++b)
+        if (sites[b] < 0 || sites[b] >= H->n_orb) return TBPM_EINDEX;
+    const Plan P = make_plan(H->n_orb, n_site, H->opt_tile);
+    if (workspace_bytes < P.total) return TBPM_ENOMEM;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    char *W = static_cast<char *>(workspace);
+    double *partial = reinterpret_cast<double *>(W + P.partial_off);
+    double *sc = reinterpret_cast<double *>(W + P.aux_off);   // [bt][4] scalars, then [nn_grid][bt] norm partials
+    double *nn_partial = sc + 4 * kMaxBT;
+    int64_t *d_sites = reinterpret_cast<int64_t *>(W + P.sites_off);
+    TBPM_CUDA_TRY(cudaMemcpyAsync(d_sites, sites, sizeof(int64_t) * (size_t)n_site, cudaMemcpyHostToDevice, st));
+    const bool table = H->n_table > 0;
+    TermParams tp{};
+    tp.orp = H->orp; tp.ocol = H->ocol; tp.oidx = H->oidx; tp.vtab = H->vtab; tp.diag = H->diag;
+    tp.rowptr = H->rowptr; tp.col = H->col; tp.val = H->val;
+    tp.n_orb = H->n_orb;
+    tp.partial = partial;
+    tp.n_table = H->n_table; tp.packed = H->packed; tp.single_real = H->single_real; tp.device = H->device;
+    tp.walk_stride = 0; tp.walk_run = 1;
+    tp.n_lat_off = H->n_lat_off;
+    for (int j = 0; j < H->n_lat_off; ++j) { tp.lat_off[j] = H->lat_off[j]; tp.lat_delta[j] = H->lat_delta[j]; }
+    tp.lat_flags = H->lat_flags; tp.n_regular = H->n_regular; tp.lat_periodic3 = H->lat_periodic3;
+    tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
+    tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
+    tp.pf_lead = H->n_lat_off > 0 ? H->lat_off[H->n_lat_off - 1] : H->halo_rows;
+    // t = H u_n and <u_n|t> in one sweep: the last-term shape of the fused kernel with psi' := 1 * T_k, first flush, bra = u_n
+    tp.a = 1.0; tp.ca = make_double2(1.0, 0.0); tp.n_acc = 1; tp.flags = F_ACC_INIT | F_REDUCE;
+    const int nn_grid = std::min(H->num_sms * 4, 64);
+    int rc = TBPM_OK;
+    for (int t = 0; t < P.n_tile; ++t) {
+        const int state0 = t * P.tile;
+        const int n_valid = std::min(P.tile, n_site - state0);
+        const int bt = (t == P.n_tile - 1) ? P.last_bt : P.tile;
+        const size_t vec = align_up((size_t)H->n_orb * bt * sizeof(double2));
+        char *base = W + P.vec0_off + (size_t)t * 4 * P.full_vec;
+        double2 *u = reinterpret_cast<double2 *>(base), *u_prev = reinterpret_cast<double2 *>(base + vec),
+                *tv = reinterpret_cast<double2 *>(base + 2 * vec);
+        const int64_t n_el = H->n_orb * bt;
+        TBPM_CUDA_TRY(cudaMemsetAsync(u, 0, sizeof(double2) * (size_t)n_el, st));
+        TBPM_CUDA_TRY(cudaMemsetAsync(u_prev, 0, sizeof(double2) * (size_t)n_el, st));
+        k_unit_states<<<1, kMaxBT, 0, st>>>(d_sites, state0, n_valid, bt, u, u);
+        k_haydock_init<<<1, kMaxBT, 0, st>>>(sc, bt, n_valid);
+        count_launches(2);
+        for (int it = 0; it < n_iter; ++it) {
+            int grid = 1;
+            tp.x = u; tp.psi0 = u; tp.acc = tv; tp.y = u_prev;    // y is neither read nor written by this shape
+            if ((rc = launch_term(bt, table, H->opt_kernel, tp, H->num_sms, st, &grid))) return rc;
+            k_haydock_scalars<<<bt, 32, 0, st>>>(partial, grid, bt, sc, 0, nn_partial, nn_grid, n_valid, state0, n_iter, it, a_out, b_out);
+            k_haydock_update<<<nn_grid, 256, 0, st>>>(tv, u, u_prev, H->n_orb, bt, sc, nn_partial);
+            k_haydock_scalars<<<bt, 32, 0, st>>>(partial, grid, bt, sc, 1, nn_partial, nn_grid, n_valid, state0, n_iter, it, a_out, b_out);
+            count_launches(3);
+            std::swap(u, u_prev);                             // u_{n+1} was written over u_{n-1}
+        }
+    }
+    TBPM_CUDA_TRY(cudaGetLastError());
+    return TBPM_OK;
 }
 
 extern "C" int tbpm_get_state(const tbpm_ham *H, const void *workspace, int state, double *psi_out, void *stream)

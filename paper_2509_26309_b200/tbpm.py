@@ -53,6 +53,9 @@ def lib() -> C.CDLL:
         L.tbpm_ldos.argtypes = [vp, vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp, sz, vp]
         L.tbpm_get_state.argtypes = [vp, vp, C.c_int, vp, vp]
         L.tbpm_dos.argtypes = [vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp]
+        L.tbpm_propagate_qe_bytes.argtypes = [vp, C.c_int, C.c_int, P(sz)]
+        L.tbpm_propagate_qe.argtypes = [vp, vp, C.c_int, C.c_int, dbl, dbl, vp, C.c_int, vp, vp, vp, vp, sz, vp]
+        L.tbpm_haydock.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp, sz, vp]
         L.tbpm_last_launch_count.restype = i64
         L.tbpm_last_launch_count.argtypes = [vp]
         L.tbpm_set_option.argtypes = [vp, C.c_int, i64]
@@ -209,6 +212,43 @@ def tbpm_ldos(H: Hamiltonian, sites, n_step: int, dt: float, rescale: float, wor
                              _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "tbpm_ldos")
     return corr, norm2, workspace
+
+
+def tbpm_propagate_qe(H: Hamiltonian, psi0: torch.Tensor, energies, n_step: int, dt: float, rescale: float):
+    """NEXT-3: (corr, norm2, qe complex128 [n_state][n_energy][n_orb]) for host energies [n_energy]."""
+    _need_cuda(psi0)
+    dev = H.device
+    psi0 = psi0.contiguous()
+    n_state = psi0.shape[0]
+    en = torch.as_tensor(energies, dtype=torch.float64, device="cpu").contiguous()
+    n_e = en.numel()
+    wb = C.c_size_t(0)
+    _check(lib().tbpm_propagate_qe_bytes(H.handle, n_state, n_e, C.byref(wb)), "tbpm_propagate_qe_bytes")
+    ws = _bytes(wb.value, dev)
+    corr = torch.zeros((n_state, n_step), dtype=torch.complex128, device=dev)
+    norm2 = torch.zeros((n_state, n_step), dtype=torch.float64, device=dev)
+    qe = torch.zeros((n_state, n_e, H.n_orb), dtype=torch.complex128, device=dev)
+    with torch.cuda.device(dev):
+        rc = lib().tbpm_propagate_qe(H.handle, _ptr(psi0), n_state, n_step, dt, rescale, C.c_void_p(en.data_ptr()), n_e, _ptr(corr),
+                                     _ptr(norm2), _ptr(qe), _ptr(ws), ws.numel(), _stream(dev))
+    _check(rc, "tbpm_propagate_qe")
+    return corr, norm2, qe
+
+
+def tbpm_haydock(H: Hamiltonian, sites, n_iter: int, workspace: Optional[torch.Tensor] = None):
+    """NEXT-2: recursion coefficients (a [n_site][n_iter] = a_0.., b [n_site][n_iter] = b_1..) from the given host sites."""
+    dev = H.device
+    sites = torch.as_tensor(sites, dtype=torch.int64, device="cpu").contiguous()
+    n_site = sites.numel()
+    if workspace is None:
+        workspace = _bytes(tbpm_propagate_bytes(H, n_site), dev)
+    a = torch.zeros((n_site, n_iter), dtype=torch.float64, device=dev)
+    b = torch.zeros((n_site, n_iter), dtype=torch.float64, device=dev)
+    with torch.cuda.device(dev):
+        rc = lib().tbpm_haydock(H.handle, C.c_void_p(sites.data_ptr()), n_site, n_iter, _ptr(a), _ptr(b), _ptr(workspace),
+                                workspace.numel(), _stream(dev))
+    _check(rc, "tbpm_haydock")
+    return a, b
 
 
 def tbpm_dos(corr: torch.Tensor, dt: float, rescale: float):

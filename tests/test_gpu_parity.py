@@ -353,24 +353,31 @@ def test_corr_host_matches_device_path(dev, oracle_mod):
 # ---------------------------------------------------------------------------------------------------------------------
 # full-size configs, in the launch configuration bench.py times
 # ---------------------------------------------------------------------------------------------------------------------
-LONG = os.environ.get("TBPM_TEST_LONG", "0") == "1"
+def load_golden(cfg, state):
+    """tests/golden/corr_full_cfg<cfg>_state<state>.txt: a full-length ORACLE run written by tests/golden/make_full_length.py
+    (which calls only oracle/): columns step, Re corr, Im corr, norm2."""
+    path = os.path.join(os.path.dirname(__file__), "golden", f"corr_full_cfg{cfg}_state{state}.txt")
+    if not os.path.exists(path):
+        return None
+    a = np.loadtxt(path)
+    return a[:, 1] + 1j * a[:, 2], a[:, 3]
 
 
-@pytest.mark.skipif(not LONG, reason="TBPM_TEST_LONG=1 runs the full-length oracle of config 2 (minutes of CPU time)")
-def test_config2_full_length(dev, oracle_mod):
-    """BASELINE.json:configs[1] exactly: 4 states x 1024 steps at 2,097,152 orbitals, every entry of corr against the
-    oracle (parity protocol (1) of SURVEY 8(d)).  Opt-in: about three minutes of oracle time on 16 host cores."""
+def test_config2_full_length(dev):
+    """BASELINE.json:configs[1] exactly: 4 states x 1024 steps at 2,097,152 orbitals, EVERY entry of corr against the cached
+    full-length oracle run (parity protocols (1) and (6) of SURVEY 8(d))."""
     w = W.make_workload(2, device=dev)
     psi0 = w.psi0(device=dev)
     H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
     corr, norm2, _ = tbpm.tbpm_propagate(H, psi0, w.n_step, w.dt, w.rescale)
     torch.cuda.synchronize()
-    hi, hj, hv, on = to_np(w)
-    ref, refn = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0.cpu().numpy(), w.n_step, w.dt, w.rescale, form="csr")
-    err = np.abs(corr.cpu().numpy() - ref).max()
-    print(f"config 2 full length: max|dcorr| = {err:.3e}, max|norm2 - 1| = {np.abs(norm2.cpu().numpy() - 1).max():.3e}")
-    assert err <= CORR_TOL
-    assert np.abs(norm2.cpu().numpy() - 1).max() <= NORM_TOL
+    corr, norm2 = corr.cpu().numpy(), norm2.cpu().numpy()
+    for b in range(4):
+        ref, refn = load_golden(2, b)
+        assert ref.shape == (w.n_step,)
+        assert np.abs(corr[b] - ref).max() <= CORR_TOL
+        assert np.abs(norm2[b] - refn).max() <= NORM_TOL
+    assert np.abs(norm2 - 1).max() <= NORM_TOL
 
 
 def test_dos_from_corr(dev, oracle_mod):
@@ -420,11 +427,19 @@ def test_full_size_closed_form_eigenstates(dev):
     eigen_check(dev, w, torch.full((n,), 1 / math.sqrt(n), dtype=torch.complex128, device=dev), -6.0, 24)
 
 
+# states compared with the oracle at full size: one from EVERY tile of 8 (config 5: tiles 0-3; its LDOS leg: one site of each of the 8 tiles)
+FULL_SAMPLE = {2: [0, 3], 3: [0], 4: [1, 6], 5: [2, 13, 17, 30]}
+LDOS_SAMPLE = [0, 9, 18, 27, 36, 45, 54, 63]
+FULL_GOLDEN_STATE = {3: 0, 4: 3, 5: 5}          # tests/golden/make_full_length.py: STATES
+
+
 @pytest.mark.skipif(not FULL, reason="TBPM_TEST_FULL=0")
-@pytest.mark.parametrize("cfg,m,sample", [(2, 3, [0, 3]), (3, 2, [0]), (4, 2, [5]), (5, 2, [17])])
-def test_full_size_prefix_parity(dev, oracle_mod, cfg, m, sample):
-    """Configs 2-5 at BASELINE.json's full size with all their states batched as bench.py runs them; the first m steps
-    of a sample of states are compared with the oracle (OpenMP row form), the norm is checked for every state."""
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_full_size_prefix_parity(dev, oracle_mod, cfg):
+    """Configs 2-5 at BASELINE.json's full size with all their states batched as bench.py runs them (same kernels, same tile
+    order).  Protocol (2) of SURVEY 8(d): the first m = 16 steps of a state from every tile against the oracle (OpenMP row form);
+    the norm of every state at every step; and, at full size, the exported CSR against the oracle's builder bit for bit."""
+    m = 16
     w = W.make_workload(cfg, device=dev)
     psi0 = w.psi0(device=dev)
     H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
@@ -433,13 +448,65 @@ def test_full_size_prefix_parity(dev, oracle_mod, cfg, m, sample):
     torch.cuda.synchronize()
     assert np.abs(norm2.cpu().numpy() - 1).max() <= NORM_TOL
     hi, hj, hv, on = to_np(w)
+    sample = FULL_SAMPLE[cfg]
     ref, _ = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0[sample].cpu().numpy(), m, w.dt, w.rescale, form="csr")
     assert np.abs(corr[sample].cpu().numpy() - ref).max() <= CORR_TOL
     if cfg == 3:
         assert abs(w.n_orb - 30198989) < 20000 and H.max_row_nnz == 3
-    if cfg == 5:                                                      # LDOS leg of config 5 on the same H
+    if cfg in (3, 4):                                                 # canonical CSR at full size, bit for bit
+        del psi0, corr, norm2
+        assert_csr_bit_exact(H, oracle_mod, w)
+    if cfg == 5:                                                      # LDOS leg of config 5 on the same H: 64 sites = 8 tiles
         sites = w.sites()
-        lc, ln, _ = tbpm.tbpm_ldos(H, sites, m, w.dt, w.rescale)
-        lref, _ = oracle_mod.ldos(w.n_orb, on, hi, hj, hv, sites[:2].numpy(), m, w.dt, w.rescale, form="csr")
-        assert np.abs(lc[:2].cpu().numpy() - lref).max() <= CORR_TOL
+        lc, ln, _ = tbpm.tbpm_ldos(H, sites, 8, w.dt, w.rescale)
+        lref, _ = oracle_mod.ldos(w.n_orb, on, hi, hj, hv, sites[LDOS_SAMPLE].numpy(), 8, w.dt, w.rescale, form="csr")
+        assert np.abs(lc[LDOS_SAMPLE].cpu().numpy() - lref).max() <= CORR_TOL
         assert np.abs(ln.cpu().numpy() - 1).max() <= NORM_TOL
+
+
+@pytest.mark.skipif(not FULL, reason="TBPM_TEST_FULL=0")
+@pytest.mark.parametrize("cfg,j", [(3, 200), (4, 200), (5, 120)])
+def test_full_size_windowed_parity(dev, oracle_mod, cfg, j):
+    """Protocol (3) of SURVEY 8(d) at full size: psi at a late step j is downloaded from the GPU with tbpm_get_state, the oracle
+    advances it m = 4 steps and must reproduce corr[:, j : j + m] of a longer GPU run; protocol (4): |norm2 - 1| <= 1e-12 at
+    every one of the j + m steps for every state."""
+    m = 4
+    w = W.make_workload(cfg, device=dev)
+    psi0 = w.psi0(device=dev)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    ws = torch.empty(tbpm.tbpm_propagate_bytes(H, w.n_state), dtype=torch.uint8, device=dev)
+    full, norm2, _ = tbpm.tbpm_propagate(H, psi0, j + m, w.dt, w.rescale, workspace=ws)
+    full = full.clone()
+    assert np.abs(norm2.cpu().numpy() - 1).max() <= NORM_TOL
+    head, _, _ = tbpm.tbpm_propagate(H, psi0, j, w.dt, w.rescale, workspace=ws)
+    assert torch.equal(head, full[:, :j])                            # prefix property, bit for bit
+    sample = FULL_SAMPLE[cfg][-2:]
+    snap = torch.stack([tbpm.tbpm_get_state(H, ws, b) for b in sample]).cpu().numpy()
+    hi, hj, hv, on = to_np(w)
+    ref, _ = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0[sample].cpu().numpy(), m, w.dt, w.rescale, psi_start=snap, form="csr")
+    assert np.abs(full[sample][:, j:].cpu().numpy() - ref).max() <= CORR_TOL
+
+
+@pytest.mark.skipif(not FULL, reason="TBPM_TEST_FULL=0")
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_length_against_cached_oracle(dev, cfg):
+    """Protocol (6) of SURVEY 8(d): a FULL-LENGTH GPU run (1024 / 2048 / 1024 steps) of the tile that holds the state whose
+    full-length oracle run is cached under tests/golden/ (tests/golden/make_full_length.py, oracle only), every entry of that
+    state's corr <= 1e-10, and |norm2 - 1| <= 1e-12 at every step for every state of the tile (protocol (4))."""
+    state = FULL_GOLDEN_STATE[cfg]
+    gold = load_golden(cfg, state)
+    if gold is None:
+        pytest.skip(f"tests/golden/corr_full_cfg{cfg}_state{state}.txt has not been generated")
+    ref, refn = gold
+    w = W.make_workload(cfg, device=dev)
+    n_state = min(w.n_state, 8)                                       # tile 0 of the batch: bit-identical to the full batch's tile 0
+    psi0 = w.psi0(device=dev, n_state=n_state)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    corr, norm2, _ = tbpm.tbpm_propagate(H, psi0, w.n_step, w.dt, w.rescale)
+    torch.cuda.synchronize()
+    assert ref.shape == (w.n_step,)
+    err = np.abs(corr[state].cpu().numpy() - ref).max()
+    print(f"config {cfg} full length: max|dcorr| = {err:.3e}, max|norm2 - 1| = {np.abs(norm2.cpu().numpy() - 1).max():.3e}")
+    assert err <= CORR_TOL
+    assert np.abs(norm2[state].cpu().numpy() - refn).max() <= NORM_TOL
+    assert np.abs(norm2.cpu().numpy() - 1).max() <= NORM_TOL
