@@ -261,17 +261,20 @@ class Runner:
         achieved_strict = bytes_term_strict / (avg_launch_s * n_tile) / 1e9
         achieved_tile = bytes_tile / avg_launch_s / 1e9
         traffic, tsrc = ncu_traffic(w.name, self.K)
-        lattice = self.cfg in (4, 5)
-        return {"bound": "hbm", "kernel": "k_term_rw (fused Chebyshev term, rolling window, term_rw.cu)" if lattice else
-                "k_term_ph (fused Chebyshev term, term_ph.cuh)",
+        kernel = {5: "k_term_l3 (fused Chebyshev term, three-dimensional lattice kernel, term_l3.cu)",
+                  4: "k_term_rw (fused Chebyshev term, rolling window, term_rw.cu)"}.get(self.cfg, "k_term_ph (fused Chebyshev term, term_ph.cuh)")
+        return {"bound": "hbm", "kernel": kernel,
                 "achieved": achieved_strict, "peak": peak, "unit": "GB/s", "frac": achieved_strict / peak,
                 "traffic": traffic, "traffic_source": tsrc, "peak_source": peak_src,
+                "frac_traffic": None if traffic is None else traffic / avg_launch_s / 1e9 / peak,
                 "bytes_per_launch": bytes_tile, "avg_launch_us": avg_launch_s * 1e6, "launches_per_step": term_launches,
                 "count": "strict: matrix_bytes_as_stored + 3*16*N*n_state once per term for all states (SURVEY 8(d)), over the time of "
                          "the n_tile launches that make one term; *_per_tile counts the matrix once per launch (one tile of <= 8 states)",
                 "achieved_per_tile": achieved_tile, "frac_per_tile": achieved_tile / peak, "n_tile": n_tile,
                 "frac_of_nominal_8000": achieved_strict / 8000.0,
-                "note": "avg launch = CUDA-event time of tbpm_propagate / term launches (includes the <1% of tiny kernels)"}
+                "note": "avg launch = CUDA-event time of tbpm_propagate / term launches (includes the <1% of tiny kernels); traffic = DRAM "
+                        "bytes per launch measured by ncu (read + write), frac_traffic = traffic / avg launch / peak: the lattice kernels "
+                        "do not read the column words of rows that sit on the lattice, so traffic can be BELOW the counted bytes"}
 
 
 def timed_steps(r, n, barrier):
