@@ -412,6 +412,7 @@ __global__ void k_sample_rows(int64_t n_orb, int n_off, const int32_t *__restric
     if (threadIdx.x == 0 && vtab) *reinterpret_cast<double2 *>(reinterpret_cast<char *>(out) + 8192) = vtab[0];
 }
 
+constexpr int64_t kSq8MaxLine = 65536;                    // longest line of the square-lattice table (term_sq.cu)
 struct LatDelta { int64_t d[16]; };
 // Lattice strides, step 2: bit r of lat_flags = "the entries of row r sit exactly where the lattice puts them"; status[ST_NREG]
 // counts such rows.  The lattice kernels skip the column words of these rows; all other rows (a matrix that merely resembles a
@@ -451,8 +452,49 @@ __global__ void k_lat_flags(int64_t n_orb, int n_off, const int32_t *__restrict_
     }
 }
 
+// Square lattice with next-nearest neighbours (offsets {-W-1, -W, -W+1, -1, +1, W-1, W, W+1}; term_sq.cu).  Direction k of site
+// (x, y) = (r % W, r / W) points to ((x + dx_k) mod W, (y + dy_k) mod Ly), k in the order of the offsets above.
+__device__ __forceinline__ int64_t sq8_neighbour(int64_t x, int64_t y, int64_t W, int64_t Ly, int k)
+{
+    const int dx = (k == 0 || k == 3 || k == 5) ? -1 : ((k == 1 || k == 6) ? 0 : 1);
+    const int dy = k < 3 ? -1 : (k < 5 ? 0 : 1);
+    int64_t xx = x + dx, yy = y + dy;
+    if (xx < 0) xx += W;
+    if (xx >= W) xx -= W;
+    if (yy < 0) yy += Ly;
+    if (yy >= Ly) yy -= Ly;
+    return yy * W + xx;
+}
+// pass 0 (rows of line y = 0 only): dline[x][k] = value index of the entry of row x that points in direction k.
+// pass 1 (every row): the row's eight columns are exactly its eight periodic neighbours AND the value index in direction k
+// equals dline[x][k], i.e. the hoppings depend on the position along the line only (Peierls phases in the Landau gauge).
+// status[ST_SQ8_BAD] counts the warps holding a row that fails.  When it stays 0 the lattice kernel needs neither the column
+// words nor the per-entry value indices: the whole matrix is the W x 8 table dline + the value table.
+__global__ void k_sq8(int64_t n_orb, int64_t W, const int32_t *__restrict__ ocol, const uint16_t *__restrict__ oidx, int pass, uint16_t *dline,
+                      int32_t *status)
+{
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool bad = false;
+    if (r < (pass == 0 ? W : n_orb)) {
+        const int64_t Ly = n_orb / W, x = r % W, y = r / W;
+        int32_t c[8];
+        uint16_t id[8];
+        for (int j = 0; j < 8; ++j) { c[j] = ocol[r * 8 + j] & 0x7fffffff; id[j] = oidx[r * 8 + j]; }
+        for (int k = 0; k < 8; ++k) {
+            const int64_t nb = sq8_neighbour(x, y, W, Ly, k);
+            int found = -1;
+            for (int j = 0; j < 8; ++j)
+                if ((int64_t)c[j] == nb) found = j;
+            if (found < 0) { bad = true; continue; }
+            if (pass == 0) dline[x * 8 + k] = id[found];
+            else bad = bad || dline[x * 8 + k] != id[found];
+        }
+    }
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicAdd(&status[ST_SQ8_BAD], 1);
+}
+
 struct PersistLayout {
-    size_t status, rowptr, col, val, orp, ocol, oidx, vtab, diag, latflag, total;
+    size_t status, rowptr, col, val, orp, ocol, oidx, vtab, diag, latflag, dline, total;
 };
 
 PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint32_t flags)
@@ -472,6 +514,7 @@ PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint3
     L.vtab = take(sizeof(double2) * kTableMax);
     L.diag = has_onsite ? take(sizeof(double) * (size_t)n_orb) : 0;
     L.latflag = take(sizeof(uint32_t) * ((size_t)n_orb / 32 + 2));
+    L.dline = take(sizeof(uint16_t) * 8 * (size_t)kSq8MaxLine);
     L.total = o;
     return L;
 }
@@ -558,6 +601,7 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
     H->vtab = reinterpret_cast<double2 *>(P + PL.vtab);
     H->diag = has_onsite ? reinterpret_cast<double *>(P + PL.diag) : nullptr;
     H->lat_flags = reinterpret_cast<uint32_t *>(P + PL.latflag);
+    H->dline = reinterpret_cast<uint16_t *>(P + PL.dline);
     int32_t *cnt = reinterpret_cast<int32_t *>(S + SL.cnt);
     int32_t *cur = reinterpret_cast<int32_t *>(S + SL.cur);
     int64_t *bsum = reinterpret_cast<int64_t *>(S + SL.bsum);
@@ -670,10 +714,21 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
                 H->lat_periodic3 = p3 ? 1 : 0;
                 k_lat_flags<<<gr, kThreads, 0, st>>>(n_orb, n_off, H->ocol, dl, p3 ? 1 : 0, H->lat_flags, H->status);
                 count_launches(1);
-                int32_t n_reg = 0;
-                TRY_OR_FAIL(cudaMemcpyAsync(&n_reg, H->status + ST_NREG, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+                // square lattice with next-nearest neighbours whose hoppings depend on the in-line position only (term_sq.cu)
+                const int64_t Wq = n_off == 8 ? dl.d[6] : 0;
+                const bool sq8 = n_off == 8 && H->n_table > 1 && !H->packed && Wq >= 4 && Wq <= kSq8MaxLine && n_orb % Wq == 0 && n_orb / Wq >= 4 &&
+                                 dl.d[0] == -Wq - 1 && dl.d[1] == -Wq && dl.d[2] == -Wq + 1 && dl.d[3] == -1 && dl.d[4] == 1 && dl.d[5] == Wq - 1 &&
+                                 dl.d[7] == Wq + 1;
+                if (sq8) {
+                    k_sq8<<<blocks_for(Wq, kThreads), kThreads, 0, st>>>(n_orb, Wq, H->ocol, H->oidx, 0, H->dline, H->status);
+                    k_sq8<<<gr, kThreads, 0, st>>>(n_orb, Wq, H->ocol, H->oidx, 1, H->dline, H->status);
+                    count_launches(2);
+                }
+                int32_t back[2] = {0, 0};                   // ST_NREG, ST_SQ8_BAD are neighbours
+                TRY_OR_FAIL(cudaMemcpyAsync(back, H->status + ST_NREG, sizeof(back), cudaMemcpyDeviceToHost, st));
                 TRY_OR_FAIL(cudaStreamSynchronize(st));
-                H->n_regular = n_reg;
+                H->n_regular = back[0];
+                H->sq8_line = (sq8 && back[1] == 0) ? Wq : 0;
             }
         }
     }

@@ -372,6 +372,7 @@ int launch_term(int bt, bool table, int kernel_opt, const TermParams &p, int num
 {
     const bool general_only = kernel_opt == 1;
     if (table && kernel_opt == 0 && term_l3_supported(bt, p)) return launch_term_l3(p, num_sms, st, grid_out);
+    if (table && kernel_opt == 0 && term_sq_supported(bt, p)) return launch_term_sq(p, num_sms, st, grid_out);
     if (table && (kernel_opt == 0 || kernel_opt == 3) && term_rw_supported(bt, p)) return launch_term_rw(p, num_sms, st, grid_out);
     if (table && !general_only && term_ph_supported(bt, p)) {
         switch (bt) {
@@ -480,6 +481,7 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
     tp.lat_flags = H->lat_flags;
     tp.n_regular = H->n_regular;
     tp.lat_periodic3 = H->lat_periodic3;
+    tp.sq8_line = H->sq8_line; tp.dline = H->dline;
     tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
     // L2 prefetch of the vector rows a few tiles ahead (term_ph.cuh, producer warp).  The leading edge of the gather
@@ -638,6 +640,7 @@ extern "C" int tbpm_haydock(tbpm_ham *H, const int64_t *sites, int n_site, int n
     tp.n_lat_off = H->n_lat_off;
     for (int j = 0; j < H->n_lat_off; ++j) { tp.lat_off[j] = H->lat_off[j]; tp.lat_delta[j] = H->lat_delta[j]; }
     tp.lat_flags = H->lat_flags; tp.n_regular = H->n_regular; tp.lat_periodic3 = H->lat_periodic3;
+    tp.sq8_line = H->sq8_line; tp.dline = H->dline;
     tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
     tp.pf_lead = H->n_lat_off > 0 ? H->lat_off[H->n_lat_off - 1] : H->halo_rows;

@@ -49,6 +49,8 @@ struct TermParams {
     int64_t lat_delta[16]; // signed offsets of the sample row's entries, in slot order
     const uint32_t *lat_flags;  // bit r: row r follows lat_delta exactly (build.cu, k_lat_flags)
     int64_t n_regular;     // number of such rows
+    int64_t sq8_line;      // > 0: periodic square lattice with next-nearest neighbours whose hoppings depend on the in-line position
+    const uint16_t *dline; // only (build.cu, k_sq8): line length in rows and the [x][8] table of value indices by direction
     int lat_periodic3;     // the bits are those of the periodic three-dimensional lattice (wrapped neighbours count as regular)
     int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
     int reverse;           // phased kernel: sweep the tiles from the last row block to the first
@@ -111,6 +113,11 @@ int launch_term_ph_bt8(const TermParams &p, int num_sms, cudaStream_t st, int *g
 // tiles; false / TBPM_EINVAL when it does not apply.
 bool term_rw_supported(int bt, const TermParams &p);
 int launch_term_rw(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
+
+// Square-lattice kernel (term_sq.cu): tiles of 8 states on the periodic square lattice with next-nearest neighbours whose hopping
+// values depend on the in-line position only; neither column words nor value indices are read per row.
+bool term_sq_supported(int bt, const TermParams &p);
+int launch_term_sq(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
 // Three-dimensional lattice kernel (term_l3.cu): tiles of 8 states on lattices with offsets {+-1, +-S1, +-S2} and one real hopping
 // value (simple cubic and its anisotropic relatives); two-dimensional tiles with TMA-fed halos, walked along S2.
