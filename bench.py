@@ -67,16 +67,17 @@ def load_peaks():
 
 
 def ncu_traffic(workload_name: str, K: int):
-    """Average DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per term launch over one time step, from the
-    `ncu --set full` captures of THIS round's kernels summarised in profiles/r2_dram_traffic.csv (one row per workload and
-    kind of launch: first term, first flush, plain term, flush, last term).  None when the file has no row for the workload."""
+    """Average DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per term launch over one time step, from the ncu
+    captures of THIS round's final kernels (profiles/r2_terms.md: all 20 launches of a time step per workload) summarised in
+    profiles/r2_dram_traffic.csv (one row per workload and kind of launch: first term, first flush, plain term, flush, last
+    term).  None when the file has no row for the workload."""
     if not os.path.exists(TRAFFIC_CSV) or K < 4:
         return None, None
     rows = {}
     src = None
     with open(TRAFFIC_CSV) as f:
         for r in csv.DictReader(l for l in f if not l.startswith("#")):
-            if r["workload"] == workload_name.split(":")[0]:
+            if r["workload"] == workload_name.split(":")[0] + ("-ldos" if workload_name.endswith("-ldos") else ""):
                 rows[r["launch"]] = float(r["dram_mbytes"])
                 src = r["source"]
     need = ("first", "first_flush", "plain", "flush", "last")
@@ -250,31 +251,41 @@ class Runner:
         return self.n_state * self.block * (self.K - 1) * self.H.nnz
 
     def roofline(self, prop_ms_per_step, peak, peak_src):
-        """Algorithmic bytes (matrix as stored + 3 vectors) against the measured launch time of the fused term."""
+        """Algorithmic bytes (matrix as stored + 3 vectors) against the measured launch time of the fused term.
+        The matrix bytes are those of the layout the running kernel reads: on the two lattices the builder recognises (tiles of 8
+        states) that is a few bytes per row, not the general kernel layout; the figure with the general layout is given beside it."""
         H, w = self.H, self.w
         tile = min(8, 1 << max(self.n_state - 1, 0).bit_length())
         n_tile = -(-self.n_state // tile)
         term_launches = n_tile * self.block * (self.K - 1)
         avg_launch_s = prop_ms_per_step * 1e-3 / term_launches
-        bytes_tile = H.matrix_bytes_per_term + 48 * w.n_orb * min(tile, self.n_state)     # what ONE launch (one tile of states) must move
-        bytes_term_strict = H.matrix_bytes_per_term + 48 * w.n_orb * self.n_state          # one term for ALL states, matrix counted once
+        lattice = tile == 8 and H.lattice_kind != 0
+        m_launch = H.lattice_bytes_per_term if lattice else H.matrix_bytes_per_term     # what ONE launch reads of H
+        bytes_tile = m_launch + 48 * w.n_orb * min(tile, self.n_state)                    # one launch = one tile of states
+        bytes_term_strict = m_launch + 48 * w.n_orb * self.n_state                        # one term for ALL states, matrix counted once
+        bytes_term_general = H.matrix_bytes_per_term + 48 * w.n_orb * self.n_state        # the same with the general kernel layout
         achieved_strict = bytes_term_strict / (avg_launch_s * n_tile) / 1e9
         achieved_tile = bytes_tile / avg_launch_s / 1e9
-        traffic, tsrc = ncu_traffic(w.name, self.K)
-        kernel = {5: "k_term_l3 (fused Chebyshev term, three-dimensional lattice kernel, term_l3.cu)",
-                  4: "k_term_rw (fused Chebyshev term, rolling window, term_rw.cu)"}.get(self.cfg, "k_term_ph (fused Chebyshev term, term_ph.cuh)")
+        traffic, tsrc = ncu_traffic(w.name + ("-ldos" if self.ldos else ""), self.K)
+        kernel = {2: "k_term_l3 (fused Chebyshev term, three-dimensional lattice kernel, term_l3.cu)",
+                  3: "k_term_sq (fused Chebyshev term, square lattice with in-line hoppings, term_sq.cu)"}.get(
+                      H.lattice_kind if lattice else 0, "k_term_ph (fused Chebyshev term, term_ph.cuh)")
         return {"bound": "hbm", "kernel": kernel,
                 "achieved": achieved_strict, "peak": peak, "unit": "GB/s", "frac": achieved_strict / peak,
                 "traffic": traffic, "traffic_source": tsrc, "peak_source": peak_src,
                 "frac_traffic": None if traffic is None else traffic / avg_launch_s / 1e9 / peak,
                 "bytes_per_launch": bytes_tile, "avg_launch_us": avg_launch_s * 1e6, "launches_per_step": term_launches,
-                "count": "strict: matrix_bytes_as_stored + 3*16*N*n_state once per term for all states (SURVEY 8(d)), over the time of "
-                         "the n_tile launches that make one term; *_per_tile counts the matrix once per launch (one tile of <= 8 states)",
+                "matrix_bytes_per_launch": m_launch, "matrix_bytes_general_layout": H.matrix_bytes_per_term,
+                "count": "strict: matrix bytes the running kernel's layout stores + 3*16*N*n_state once per term for all states "
+                         "(SURVEY 8(d)), over the time of the n_tile launches that make one term; *_per_tile counts the matrix once "
+                         "per launch (one tile of <= 8 states); *_general_layout counts the general kernel layout (orp/ocol/oidx/diag), "
+                         "which the lattice kernels do not read",
                 "achieved_per_tile": achieved_tile, "frac_per_tile": achieved_tile / peak, "n_tile": n_tile,
+                "frac_general_layout": bytes_term_general / (avg_launch_s * n_tile) / 1e9 / peak,
                 "frac_of_nominal_8000": achieved_strict / 8000.0,
-                "note": "avg launch = CUDA-event time of tbpm_propagate / term launches (includes the <1% of tiny kernels); traffic = DRAM "
-                        "bytes per launch measured by ncu (read + write), frac_traffic = traffic / avg launch / peak: the lattice kernels "
-                        "do not read the column words of rows that sit on the lattice, so traffic can be BELOW the counted bytes"}
+                "note": "avg launch = CUDA-event time of tbpm_propagate / term launches (includes the <1% of tiny kernels); traffic = "
+                        "DRAM bytes per launch measured by ncu (read + write) averaged over the launches of a time step, "
+                        "frac_traffic = traffic / avg launch / peak"}
 
 
 def timed_steps(r, n, barrier):
@@ -377,6 +388,7 @@ def main_ours(args):
     # the other >= 16 M-orbital workloads, in the same process, for >= per_workload_seconds each (sustained clocks)
     if world == 1 and not args.no_per_workload and args.workload == "5":
         per = [{"workload": r.name, "value": value, "frac": roofline["frac"], "frac_per_tile": roofline["frac_per_tile"],
+                "frac_general_layout": roofline["frac_general_layout"], "frac_traffic": roofline["frac_traffic"], "kernel": roofline["kernel"],
                 "avg_launch_us": roofline["avg_launch_us"], "clocks": clocks, "max_norm_dev": norm_dev,
                 "seconds": total_ms * 1e-3, "n_step_per_bench_step": r.block}]
         del r
@@ -396,6 +408,7 @@ def main_ours(args):
             rf = q.roofline(prp / n, peak, peak_src)
             nd = float((q.norm2 - 1).abs().max())
             per.append({"workload": q.name, "value": n * q.units_per_step() / (tot * 1e-3), "frac": rf["frac"], "frac_per_tile": rf["frac_per_tile"],
+                        "frac_general_layout": rf["frac_general_layout"], "frac_traffic": rf["frac_traffic"],
                         "avg_launch_us": rf["avg_launch_us"], "bytes_per_launch": rf["bytes_per_launch"], "kernel": rf["kernel"],
                         "traffic": rf["traffic"], "clocks": ck, "max_norm_dev": nd, "norm_ok": bool(nd <= 1e-12),
                         "seconds": tot * 1e-3, "n_step_per_bench_step": q.block})

@@ -89,6 +89,15 @@ int tbpm_build(int64_t n_orb, const double *onsite /* device [n_orb] or NULL */,
 int tbpm_ham_info(const tbpm_ham *H, int64_t *n_orb, int64_t *nnz, int32_t *max_row_nnz, size_t *matrix_bytes_per_term,
                   int32_t *n_table, double *gershgorin);
 
+/* Lattices the builder recognises: tiles of 8 states then run on a kernel that reads no column words and
+ * no per-entry value indices for the rows that sit on the lattice.  kind: 0 none, TBPM_LATTICE_CUBIC (offsets {+-1, +-S1, +-S2},
+ * one real hopping value: BASELINE.json:configs[4]), TBPM_LATTICE_SQUARE8 (periodic square lattice with next-nearest neighbours,
+ * hoppings that depend on the in-line position only: configs[3]).  bytes_per_term = the bytes of H THAT kernel reads per
+ * Chebyshev term (what bench.py counts as the matrix when it runs on it); 0 when kind is 0.  Outputs may be NULL. */
+#define TBPM_LATTICE_CUBIC 2
+#define TBPM_LATTICE_SQUARE8 3
+int tbpm_ham_lattice_info(const tbpm_ham *H, int32_t *kind, size_t *bytes_per_term);
+
 /* TBPM_EBOUND if gershgorin > rescale (test is '>' : config 4 sits exactly at equality), else TBPM_OK. */
 int tbpm_check_bound(const tbpm_ham *H, double rescale);
 

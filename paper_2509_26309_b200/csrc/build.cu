@@ -756,6 +756,28 @@ extern "C" int tbpm_ham_info(const tbpm_ham *H, int64_t *n_orb, int64_t *nnz, in
     return TBPM_OK;
 }
 
+// Which lattice kernel tiles of 8 states run on, and the bytes of H that kernel reads per Chebyshev term.
+extern "C" int tbpm_ham_lattice_info(const tbpm_ham *H, int32_t *kind, size_t *bytes_per_term)
+{
+    if (!H) return TBPM_EINVAL;
+    int k = 0;
+    size_t b = 0;
+    const int n_off = H->max_row_nnz - (H->has_onsite ? 1 : 0);
+    const bool uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
+    if (H->n_table > 0 && uniform && H->lat_periodic3 && H->single_real && n_off == 6 && H->lat_delta[4] % 32 == 0 &&
+        H->lat_delta[5] % (H->lat_delta[4] * 4) == 0 && H->n_orb / H->lat_delta[5] >= 4 && H->n_regular * 2 >= H->n_orb) {
+        k = TBPM_LATTICE_CUBIC;                               // term_l3.cu: real diagonal + one bit per row (+ the column words of the
+        b = (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0) + (size_t)H->n_orb / 8 + sizeof(double2) +   // rows off the lattice)
+            (size_t)(H->n_orb - H->n_regular) * n_off * sizeof(int32_t);
+    } else if (H->sq8_line > 0 && H->sq8_line % 128 == 0) {
+        k = TBPM_LATTICE_SQUARE8;                             // term_sq.cu: value indices by direction of one line + the value table
+        b = sizeof(uint16_t) * 8 * (size_t)H->sq8_line + sizeof(double2) * (size_t)H->n_table + (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0);
+    }
+    if (kind) *kind = k;
+    if (bytes_per_term) *bytes_per_term = b;
+    return TBPM_OK;
+}
+
 extern "C" int tbpm_check_bound(const tbpm_ham *H, double rescale)
 {
     if (!H || !(rescale > 0.0)) return TBPM_EINVAL;
@@ -775,4 +797,9 @@ extern "C" int tbpm_export_csr(const tbpm_ham *H, int64_t *rowptr, int32_t *col,
     return TBPM_OK;
 }
 
-extern "C" void tbpm_free(tbpm_ham *H) { delete H; }
+extern "C" void tbpm_free(tbpm_ham *H)
+{
+    if (!H) return;
+    for (cudaGraphExec_t g : H->graph_execs) cudaGraphExecDestroy(g);
+    delete H;
+}

@@ -181,7 +181,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_term_ph(const TermParams p
         // Lane 0 stages the matrix slices.  All 32 lanes then PREFETCH INTO L2 the vector rows that a tile `pf_dist` steps
         // further along this block's walk will stream (y, psi', psi0) or touch first (x at the leading edge of the gather
         // window): the consumers hold one row group per warp in registers, which keeps only ~30 KB of DRAM-bound loads
-        // in flight per SM where the HBM needs ~64 KB (microbenchmark, profiles/r2_probe.md); prefetches hold no
+        // in flight per SM where the HBM needs ~64 KB (microbenchmark, profiles/r2_microbench.md); prefetches hold no
         // registers, so they carry the DRAM latency and the consumers' loads become L2 hits.
         const int lane = tid - kConsumers;
         uint32_t q_lo = 0, q_hi = 0;                        // offsets bounding the next tile to issue (prefetched)

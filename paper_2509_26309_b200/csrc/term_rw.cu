@@ -4,7 +4,7 @@
 //   T_k = a*H*T_{k-1} - T_{k-2}  (amxsy) + deferred psi' accumulation (axpy) + last-term
 //   <psi0|psi'>, <psi'|psi'> (calc_corr_dos), exactly as term_ph.cuh; same TermParams, same results.
 //
-// Why (profiles/r2_probe.md, profiles/r1c_final.md): with 8 states a vector row is one 128-byte line, and the phased kernel
+// Why (profiles/r2_ncu_cfg5.md, profiles/r1c_final.md): with 8 states a vector row is one 128-byte line, and the phased kernel
 // asks the L1 for 9-10 lines per row (6-8 gathers, x[row], y, the store).  A line that misses L1 costs the SM 2.2 cycles of
 // its L2 port, one that hits 0.84, and the registers that receive the gathers cap the loads in flight at ~130 KB per SM:
 // 22-30 cycles per row where the HBM needs 15.8.  On a lattice almost all of those requests are redundant.  Let W be the

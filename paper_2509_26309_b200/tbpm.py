@@ -45,6 +45,7 @@ def lib() -> C.CDLL:
         L.tbpm_build.argtypes = [i64, vp, i64, vp, vp, vp, u32, vp, sz, vp, sz, vp, P(vp)]
         L.tbpm_ham_info.argtypes = [vp, P(i64), P(i64), P(i32), P(sz), P(i32), P(dbl)]
         L.tbpm_check_bound.argtypes = [vp, dbl]
+        L.tbpm_ham_lattice_info.argtypes = [vp, P(i32), P(sz)]
         L.tbpm_export_csr.argtypes = [vp, vp, vp, vp, vp]
         L.tbpm_free.argtypes = [vp]
         L.tbpm_free.restype = None
@@ -123,6 +124,9 @@ class Hamiltonian:
         _check(lib().tbpm_ham_info(self.handle, C.byref(n), C.byref(nnz), C.byref(mr), C.byref(mb), C.byref(nt), C.byref(g)), "tbpm_ham_info")
         self.n_orb, self.nnz, self.max_row_nnz = n.value, nnz.value, mr.value
         self.matrix_bytes_per_term, self.n_table, self.gershgorin = mb.value, nt.value, g.value
+        kind, lb = C.c_int32(0), C.c_size_t(0)
+        _check(lib().tbpm_ham_lattice_info(self.handle, C.byref(kind), C.byref(lb)), "tbpm_ham_lattice_info")
+        self.lattice_kind, self.lattice_bytes_per_term = kind.value, lb.value
 
     def __del__(self):
         try:
