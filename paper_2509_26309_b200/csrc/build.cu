@@ -797,9 +797,4 @@ extern "C" int tbpm_export_csr(const tbpm_ham *H, int64_t *rowptr, int32_t *col,
     return TBPM_OK;
 }
 
-extern "C" void tbpm_free(tbpm_ham *H)
-{
-    if (!H) return;
-    for (cudaGraphExec_t g : H->graph_execs) cudaGraphExecDestroy(g);
-    delete H;
-}
+extern "C" void tbpm_free(tbpm_ham *H) { delete H; }

@@ -166,13 +166,11 @@ __global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p
 }
 
 // Sum the block partials in a fixed order: block = state, warp = component, lanes stride over the partials.
-// step_ctr != NULL: the time-step index is read from the device (the launch sits in a CUDA graph that is replayed every third step).
 __global__ void k_reduce_final(const double *__restrict__ partial, int n_blocks, int bt, int n_valid, int state0, int n_step, int step,
-                               double *corr, double *norm2, const int *__restrict__ step_ctr)
+                               double *corr, double *norm2)
 {
     const int bb = blockIdx.x, c = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (bb >= n_valid) return;
-    if (step_ctr) step = *step_ctr;
     double t = 0.0;
     for (int k = lane; k < n_blocks; k += 32) t += partial[((int64_t)k * bt + bb) * 3 + c];
     for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
@@ -182,8 +180,6 @@ __global__ void k_reduce_final(const double *__restrict__ partial, int n_blocks,
         else if (norm2) norm2[at] = t;
     }
 }
-
-__global__ void k_step_ctr(int *ctr, int set, int add) { *ctr = (set >= 0 ? set : *ctr) + add; }
 
 // a2: state-major psi0 -> interleaved tile buffers (psi and the bra); states beyond n_valid are zero padding.
 __global__ void k_interleave(const double2 *__restrict__ psi0, int64_t n_orb, int state0, int n_valid, int bt, double2 *psi, double2 *bra)
@@ -534,13 +530,7 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
             count_launches(1);
         };
         if (qe && n_el > 0) qe_add(buf[start_slot], 0);
-        // Small models are launch-bound (cfg1: 4.6 us per launch for microseconds of work): after three directly launched steps
-        // (one per phase of the buffer rotation; they also configure the kernels) a time step -- K - 1 terms, the final reduction,
-        // the step counter -- is captured once per phase into a CUDA graph and replayed; the step index lives on the device.
-        bool use_graph = !qe && K > 1 && n_step >= 12 && n_el > 0 && n_el <= ((int64_t)1 << 20) && knob("graph", 1);
-        int *step_ctr = reinterpret_cast<int *>(W + 128);
-        cudaGraphExec_t gexec[3] = {nullptr, nullptr, nullptr};
-        auto one_step = [&](int n, cudaStream_t s2, const int *ctr) -> int {
+        auto one_step = [&](int n, cudaStream_t s2) -> int {
             double2 *psi = buf[slot], *t1 = buf[(slot + 1) % 3], *acc = buf[(slot + 2) % 3];
             int grid = 1;
             if (K == 1) {                                 // tau = 0: psi' = c_0 psi, no H application
@@ -552,40 +542,12 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
             step_terms(tp, K, cf, rescale, reverse_odd, psi, t1, acc, term);
             for (int k = 1; k < K; ++k)
                 if ((rc = launch_term(bt, table, H->opt_kernel, term[k], H->num_sms, s2, &grid))) return rc;
-            k_reduce_final<<<bt, 96, 0, s2>>>(partial, grid, bt, n_valid, state0, n_step, n, corr, norm2, ctr);
+            k_reduce_final<<<bt, 96, 0, s2>>>(partial, grid, bt, n_valid, state0, n_step, n, corr, norm2);
             count_launches(1);
             return TBPM_OK;
         };
         for (int n = 0; n < n_step; ++n) {
-            const int phase = n % 3;
-            if (use_graph && n >= 3 && !gexec[phase]) {   // capture this phase's step
-                cudaStream_t cs = nullptr;
-                cudaGraph_t graph = nullptr;
-                const long long before = total_launches();
-                bool ok = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) == cudaSuccess &&
-                          cudaStreamBeginCapture(cs, cudaStreamCaptureModeRelaxed) == cudaSuccess;
-                if (ok) {
-                    ok = one_step(n, cs, step_ctr) == TBPM_OK;
-                    k_step_ctr<<<1, 1, 0, cs>>>(step_ctr, -1, 1);
-                    ok = (cudaStreamEndCapture(cs, &graph) == cudaSuccess) && ok && graph;
-                }
-                if (ok) ok = cudaGraphInstantiate(&gexec[phase], graph, 0) == cudaSuccess;
-                if (graph) cudaGraphDestroy(graph);
-                if (cs) cudaStreamDestroy(cs);
-                count_launches((int)(before - total_launches()));   // the captured launches did not run
-                if (!ok) { (void)cudaGetLastError(); use_graph = false; gexec[phase] = nullptr; }
-                else {
-                    std::lock_guard<std::mutex> lock(H->mu);
-                    H->graph_execs.push_back(gexec[phase]);          // destroyed by tbpm_free (the replays are asynchronous)
-                }
-            }
-            if (use_graph && n >= 3 && gexec[phase]) {
-                TBPM_CUDA_TRY(cudaGraphLaunch(gexec[phase], st));
-                count_launches(K + 1);
-            } else {
-                if ((rc = one_step(n, st, nullptr))) return rc;
-                if (use_graph && n == 2) { k_step_ctr<<<1, 1, 0, st>>>(step_ctr, 3, 0); count_launches(1); }
-            }
+            if ((rc = one_step(n, st))) return rc;
             slot = (slot + 2) % 3;                        // psi' (acc) is the next step's psi
             if (qe && n_el > 0) qe_add(buf[slot], n + 1);
         }

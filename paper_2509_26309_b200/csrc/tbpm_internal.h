@@ -100,6 +100,5 @@ struct tbpm_ham {
     // bookkeeping of the propagate calls: written under `mu` (calls on distinct workspaces may run concurrently)
     mutable std::mutex mu;
     std::vector<tbpm_detail::RunRecord> runs;
-    std::vector<cudaGraphExec_t> graph_execs;   // time-step graphs of small models (propagate.cu), destroyed by tbpm_free
     std::atomic<long long> last_launches{0};
 };
