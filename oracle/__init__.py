@@ -237,3 +237,70 @@ def haydock_ldos(a, b, energies, eta):
         tail = (b[n] ** 2) * g if n < a.size - 1 else 0.0
         g = 1.0 / (z - a[n] - tail)
     return -g.imag / np.pi
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# NEXT-4: AC-conductivity correlation function (Fermi-operator Chebyshev filter + current-operator matrix-vector products)
+# ---------------------------------------------------------------------------------------------------------------------
+def fermi_cheb_coeff(beta: float, mu: float, rescale: float, tol: float = 1e-13, n_quad: int = 8192, one_minus: bool = False) -> np.ndarray:
+    """Chebyshev coefficients of the Fermi operator on [-s, s]: f(E) = 1 / (exp(beta (E - mu)) + 1) = sum_k c_k T_k(E / s),
+    c_k = (2 - delta_k0) / M * sum_m f(s cos theta_m) cos(k theta_m), theta_m = pi (m + 1/2) / M (Gauss-Chebyshev quadrature, M =
+    n_quad), kept up to the LAST k with |c_k| >= tol.  one_minus: the coefficients of 1 - f.  [paper silent; reading #30]"""
+    m = np.arange(n_quad)
+    th = np.pi * (m + 0.5) / n_quad
+    x = beta * (rescale * np.cos(th) - mu)
+    f = np.where(x > 0, np.exp(-np.abs(x)) / (1.0 + np.exp(-np.abs(x))), 1.0 / (1.0 + np.exp(-np.abs(x))))
+    kmax = n_quad // 4
+    c = np.array([(1.0 if k == 0 else 2.0) / n_quad * np.sum(f * np.cos(k * th)) for k in range(kmax)])
+    big = np.nonzero(np.abs(c) >= tol)[0]
+    K = int(big[-1]) + 1 if big.size else 1
+    c = c[:K].copy()
+    if one_minus:
+        c = -c
+        c[0] += 1.0
+    return c
+
+
+def apply_cheb_series(n_orb, onsite, hop_i, hop_j, hop_val, coeff, rescale, x, hops_full=False):
+    """y = sum_k coeff[k] T_k(H / s) x by the forward recurrence T_0 = x, T_1 = H' x, T_{k+1} = 2 H' T_k - T_{k-1} (the loop of
+    PAPER.md:437-443 with other coefficients), H applied by the oracle's hop-list routine."""
+    coeff = np.asarray(coeff)
+    t0 = _c128(x).copy()
+    y = coeff[0] * t0
+    if coeff.size > 1:
+        t1 = apply_h(n_orb, onsite, hop_i, hop_j, hop_val, t0, hops_full) / rescale
+        y = y + coeff[1] * t1
+        for k in range(2, coeff.size):
+            t2 = (2.0 / rescale) * apply_h(n_orb, onsite, hop_i, hop_j, hop_val, t1, hops_full) - t0
+            y = y + coeff[k] * t2
+            t0, t1 = t1, t2
+    return y
+
+
+def corr_ac(n_orb, onsite, hop_i, hop_j, hop_val, ja_hops, jb_hops, psi0, n_step, dt, rescale, beta, mu):
+    """AC-conductivity correlation of TBPM ("AC conductivity (AC)" is a solver function of the paper, Table 7
+    PAPER.md:1744; the current operator acts through a sparse matrix-vector product; no formula is printed).
+    DESIGN.md reading #30, with f the Fermi operator and J_a, J_b the current-operator matrices (given as hop lists, Hermitian):
+
+        psi1(0) = [1 - f(H)] J_b psi0,   psi2(0) = f(H) psi0,   psi_i(t) = exp(-i H t) psi_i(0)
+        corr[b][n] = < psi2(n dt) | J_a | psi1(n dt) >,   n = 0 .. n_step
+
+    f(H) and 1 - f(H) by their Chebyshev series (fermi_cheb_coeff), the time evolution by the oracle's own propagation one step at a
+    time.  ja_hops / jb_hops = (hop_i, hop_j, hop_val) of the two current operators (each conjugate pair once).  Returns complex128
+    [B][n_step + 1]."""
+    psi0 = np.atleast_2d(_c128(psi0))
+    cf = fermi_cheb_coeff(beta, mu, rescale)
+    cg = fermi_cheb_coeff(beta, mu, rescale, one_minus=True)
+    out = np.zeros((psi0.shape[0], n_step + 1), dtype=np.complex128)
+    for b in range(psi0.shape[0]):
+        phi = apply_h(n_orb, None, *jb_hops, psi0[b])
+        p1 = apply_cheb_series(n_orb, onsite, hop_i, hop_j, hop_val, cg, rescale, phi)
+        p2 = apply_cheb_series(n_orb, onsite, hop_i, hop_j, hop_val, cf, rescale, psi0[b])
+        for n in range(n_step + 1):
+            if n > 0:
+                _, _, fin = propagate(n_orb, onsite, hop_i, hop_j, hop_val, p1, 1, dt, rescale, psi_start=p1, return_state=True)
+                p1 = fin[0]
+                _, _, fin = propagate(n_orb, onsite, hop_i, hop_j, hop_val, p2, 1, dt, rescale, psi_start=p2, return_state=True)
+                p2 = fin[0]
+            out[b, n] = np.vdot(p2, apply_h(n_orb, None, *ja_hops, p1))
+    return out

@@ -189,6 +189,21 @@ def square_peierls_hops(Lx: int, Ly: int, t: float = -1.0, t2: float = 0.2, phi_
     return Lx * Ly, hop_i, hop_j, hop_val
 
 
+def square_current_hops(Lx: int, Ly: int, axis: int, t: float = -1.0, t2: float = 0.2, phi_num: int = 1, phi_den: int = 1024, device="cpu"):
+    """Hop list of the current operator J_axis = i [H, r_axis] of square_peierls_hops' lattice (hbar = e = 1; NEXT-4): the entry
+    <r'|J|r> = i * <r'|H|r> * (r' - r)_axis with the UNWRAPPED displacement of the hop; hops without a component along the axis are
+    left out.  Hermitian like H, so the list holds each conjugate pair once and goes through tbpm_build / the oracle as it is."""
+    n, hi, hj, hv = square_peierls_hops(Lx, Ly, t, t2, phi_num, phi_den, device)
+    per = Lx * Ly
+    disp = []
+    for dx, dy in ((1, 0), (0, 1), (1, 1), (-1, 1)):               # the four hop families, in square_peierls_hops' order
+        disp.append(torch.full((per,), float((dx, dy)[axis]), dtype=torch.float64, device=device))
+    d = torch.cat(disp)
+    keep = d != 0
+    val = torch.complex(-hv.imag * d, hv.real * d)                 # i * v * d
+    return n, hi[keep].contiguous(), hj[keep].contiguous(), val[keep].contiguous()
+
+
 def cubic_hops(L: int, t: float = -1.0, device="cpu"):
     """Simple-cubic L^3 periodic, idx = (z*L + y)*L + x, hops to +x, +y, +z (reading #24)."""
     if L < 3:

@@ -133,3 +133,60 @@ def test_haydock_agrees_with_time_domain_ldos(oracle_mod):
     m1d, m1h = np.trapezoid(E * D, E) / np.trapezoid(D, E), np.trapezoid(E * Hd, E) / np.trapezoid(Hd, E)
     assert abs(m1d - m1h) < 0.05 * w.rescale
     assert abs(m1d - on[site]) < 0.05 * w.rescale                   # <i|H|i> = onsite_i
+
+
+# ---- NEXT-4: AC-conductivity correlation ----------------------------------------------------------------------------
+@pytest.mark.parametrize("beta,mu,s", [(2.0, 0.3, 4.8), (11.0, -1.0, 4.8), (0.5, 0.0, 9.0)])
+def test_fermi_chebyshev_closed_form(oracle_mod, beta, mu, s):
+    """sum_k c_k T_k(x) = 1 / (exp(beta (s x - mu)) + 1) on [-1, 1]; the complement sums to 1 - f; |c_k| decays."""
+    c = oracle_mod.fermi_cheb_coeff(beta, mu, s)
+    g = oracle_mod.fermi_cheb_coeff(beta, mu, s, one_minus=True)
+    x = np.linspace(-1, 1, 201)
+    T = np.cos(np.outer(np.arange(c.size), np.arccos(x)))
+    f = 1.0 / (np.exp(beta * (s * x - mu)) + 1.0)
+    assert np.abs(c @ T - f).max() < 1e-11
+    assert np.abs(g @ T - (1 - f)).max() < 1e-11
+    assert abs(c[-1]) >= 1e-13 and c.size < 2048
+
+
+def test_current_operator_generator():
+    """W.square_current_hops: J = i * H_ij * (r_i - r_j) with the minimum-image displacement, Hermitian (brute force on 7 x 5)."""
+    Lx, Ly = 7, 5
+    n, hi, hj, hv = W.square_peierls_hops(Lx, Ly, -1.0, 0.2, 1, 7)
+    H = dense_h(n, hi.numpy(), hj.numpy(), hv.numpy())
+    xs, ys = np.arange(n) % Lx, np.arange(n) // Lx
+    for axis, (c, L) in enumerate(((xs, Lx), (ys, Ly))):
+        n2, ji, jj, jv = W.square_current_hops(Lx, Ly, axis, -1.0, 0.2, 1, 7)
+        J = dense_h(n2, ji.numpy(), jj.numpy(), jv.numpy())
+        d = c[:, None] - c[None, :]
+        d = (d + L // 2) % L - L // 2                                # minimum image (L odd: unique)
+        assert np.abs(J - 1j * H * d).max() < 1e-14
+        assert np.abs(J - J.conj().T).max() < 1e-14
+
+
+@pytest.mark.parametrize("beta,mu", [(1.5, 0.4), (6.0, -0.8)])
+def test_corr_ac_exact_diagonalisation(oracle_mod, beta, mu):
+    """corr_n = psi0^+ f(H) e^{+iHt} J_a e^{-iHt} (1 - f(H)) J_b psi0 by full diagonalisation (numpy.linalg.eigh) on a 10 x 8 square
+    lattice with flux: a swapped pair of operators, a missing 1 - f, the sign of the time phase or an off-by-one in n each fail."""
+    Lx, Ly, s = 10, 8, 4.8
+    w = W.make_workload(4, Lx=Lx, Ly=Ly, phi_den=5)
+    hi, hj, hv, on = np_hops(w)
+    psi0 = w.psi0(n_state=2).numpy()
+    ja = tuple(t.numpy() for t in W.square_current_hops(Lx, Ly, 0, phi_den=5)[1:])
+    jb = tuple(t.numpy() for t in W.square_current_hops(Lx, Ly, 1, phi_den=5)[1:])
+    n_step = 12
+    corr = oracle_mod.corr_ac(w.n_orb, on, hi, hj, hv, ja, jb, psi0, n_step, w.dt, s, beta, mu)
+    H = dense_h(w.n_orb, hi, hj, hv, on)
+    Ja, Jb = dense_h(w.n_orb, *ja), dense_h(w.n_orb, *jb)
+    E, V = np.linalg.eigh(H)
+    f = 1.0 / (np.exp(beta * (E - mu)) + 1.0)
+    for b in range(2):
+        p1 = V @ ((1 - f) * (V.conj().T @ (Jb @ psi0[b])))
+        p2 = V @ (f * (V.conj().T @ psi0[b]))
+        for n in range(n_step + 1):
+            U = (V * np.exp(-1j * E * n * w.dt)) @ V.conj().T
+            ref = np.vdot(U @ p2, Ja @ (U @ p1))
+            assert abs(corr[b, n] - ref) < 1e-11, (b, n)
+    # a full band (mu far above the spectrum): 1 - f = 0, nothing to excite
+    z = oracle_mod.corr_ac(w.n_orb, on, hi, hj, hv, ja, jb, psi0[:1], 2, w.dt, s, 40.0, 3 * s)
+    assert np.abs(z).max() < 1e-10
