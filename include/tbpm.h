@@ -180,6 +180,21 @@ int tbpm_propagate_qe(tbpm_ham *H, const double *psi0, int n_state, int n_step, 
 int tbpm_haydock(tbpm_ham *H, const int64_t *sites /* host */, int n_site, int n_iter, double *a /* device out */,
                  double *b /* device out */, void *workspace, size_t workspace_bytes, void *stream);
 
+/* ---- NEXT-4: AC-conductivity correlation function ("AC conductivity (AC)"; Table 7; the current
+ * operator acts through a sparse matrix-vector product, and has a CSR of its own) ------------------
+ * The paper prints no formula; reading #30 (hbar = e = 1):
+ *     psi1(0) = [1 - f(H)] J_b psi0,   psi2(0) = f(H) psi0,   f(E) = 1 / (exp(beta (E - mu)) + 1),   psi_i(t) = exp(-i H t) psi_i(0),
+ *     corr[b][n] = < psi2(n dt) | J_a | psi1(n dt) >,   n = 0 .. n_step      (device out [n_state][n_step + 1][2]).
+ * Ja, Jb: handles built with tbpm_build from the hop lists of the current operators J = i [H, r] (entry <i|J|j> = i <i|H|j>
+ * (r_i - r_j), Hermitian, so each conjugate pair once; no onsite), same n_orb and device as H.  f(H) and 1 - f(H) are applied by
+ * their Chebyshev series on [-rescale, rescale] (tbpm_fermi_coeff: host only, real coefficients as (re, 0) pairs, truncated after
+ * the last |c_k| >= tol; the library uses tol = 1e-13).  Workspace: tbpm_corr_ac_bytes (six vectors of one tile). */
+int tbpm_fermi_coeff(double beta, double mu, double rescale, int one_minus, double tol, int kcap, int *K, double *coeff /* host [kcap][2] */);
+int tbpm_corr_ac_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes);
+int tbpm_corr_ac(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const double *psi0 /* device [n_state][n_orb][2] */, int n_state, int n_step,
+                 double dt, double rescale, double beta, double mu, double *corr /* device out */, void *workspace,
+                 size_t workspace_bytes, void *stream);
+
 /* ---- end to end with HOST buffers ------------------------------------------------------------------------------------
  * Whole path for host-resident inputs: H2D of the list and psi0, tbpm_build, tbpm_propagate, D2H of corr/norm2, then a
  * stream synchronise.  `arena` is caller-owned device memory of at least tbpm_corr_host_bytes(); host buffers should be

@@ -78,3 +78,39 @@ extern "C" int tbpm_cheb_coeff(double tau, double tol, int kcap, int *K, double 
     }
     return TBPM_OK;
 }
+
+// NEXT-4: Chebyshev coefficients of the Fermi operator f(E) = 1 / (exp(beta (E - mu)) + 1) on [-s, s] (or of 1 - f):
+//     c_k = (2 - delta_k0) / pi * integral_0^pi f(s cos t) cos(k t) dt,
+// evaluated by the midpoint rule on M = 16384 points (exact for the truncated series: Gauss-Chebyshev), k ascending until 64
+// consecutive coefficients are below tol; the coefficients after the last one >= tol are dropped.  Real coefficients, written as
+// (re, 0) pairs so that the series goes through the same fused kernels as the time step.  DESIGN.md reading #30.
+extern "C" int tbpm_fermi_coeff(double beta, double mu, double rescale, int one_minus, double tol, int kcap, int *K, double *coeff)
+{
+    if (!K || !coeff || kcap < 1 || !(beta >= 0.0) || !std::isfinite(beta) || !std::isfinite(mu) || !(rescale > 0.0) || !(tol > 0.0)) return TBPM_EINVAL;
+    constexpr int M = 16384;
+    const double pi = 3.14159265358979323846;
+    std::vector<double> f(M), th(M);
+    for (int m = 0; m < M; ++m) {
+        th[m] = pi * (m + 0.5) / M;
+        const double x = beta * (rescale * std::cos(th[m]) - mu);
+        const double e = std::exp(-std::fabs(x));
+        f[m] = x > 0.0 ? e / (1.0 + e) : 1.0 / (1.0 + e);
+    }
+    std::vector<double> c;
+    int last_big = 0, quiet = 0;
+    for (int k = 0; k < M / 4 && quiet < 64; ++k) {
+        long double acc = 0.0L;
+        for (int m = 0; m < M; ++m) acc += (long double)f[m] * (long double)std::cos(k * th[m]);
+        const double ck = (double)((k == 0 ? 1.0L : 2.0L) * acc / M);
+        c.push_back(ck);
+        if (std::fabs(ck) >= tol) { last_big = k; quiet = 0; } else ++quiet;
+    }
+    const int Kf = last_big + 1;
+    *K = Kf;
+    if (Kf > kcap) return TBPM_ENOMEM;
+    for (int k = 0; k < Kf; ++k) {
+        coeff[2 * k] = one_minus ? (k == 0 ? 1.0 - c[k] : -c[k]) : c[k];
+        coeff[2 * k + 1] = 0.0;
+    }
+    return TBPM_OK;
+}

@@ -430,6 +430,36 @@ void step_terms(const TermParams &base, int K, const std::vector<double> &cf, do
     }
 }
 
+// The matrix side of a term launch: everything of TermParams that comes from the handle.
+TermParams matrix_params(const tbpm_ham *H, double *partial)
+{
+    TermParams mp{};
+    mp.orp = H->orp; mp.ocol = H->ocol; mp.oidx = H->oidx; mp.vtab = H->vtab; mp.diag = H->diag;
+    mp.rowptr = H->rowptr; mp.col = H->col; mp.val = H->val;
+    mp.n_orb = H->n_orb;
+    mp.partial = partial;
+    mp.n_table = H->n_table;
+    mp.packed = H->packed;
+    mp.single_real = H->single_real;
+    mp.device = H->device;
+    mp.walk_stride = 0; mp.walk_run = 1;
+    mp.n_lat_off = H->n_lat_off;
+    for (int j = 0; j < H->n_lat_off; ++j) { mp.lat_off[j] = H->lat_off[j]; mp.lat_delta[j] = H->lat_delta[j]; }
+    mp.lat_flags = H->lat_flags;
+    mp.n_regular = H->n_regular;
+    mp.lat_periodic3 = H->lat_periodic3;
+    mp.sq8_line = H->sq8_line; mp.dline = H->dline;
+    mp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
+    mp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
+    // L2 prefetch of the vector rows a few tiles ahead (term_ph.cuh, producer warp).  The leading edge of the gather
+    // window is the farthest neighbour: the largest lattice stride on uniform lattices, else the widest |col - row|.
+    mp.pf_dist = knob("pf", 0);
+    mp.pf_mask = knob("pf_mask", 3);
+    mp.pf_lead = H->n_lat_off > 0 ? H->lat_off[H->n_lat_off - 1] : H->halo_rows;
+    if (knob("pf_lead", -1) >= 0) mp.pf_lead = knob("pf_lead", -1);
+    return mp;
+}
+
 // Shared body of tbpm_propagate (psi0 != NULL) and tbpm_ldos (sites != NULL).
 struct QeSpec { const double *energies; int n_energy; double *out; };   // NEXT-3: energies on the host, out on the device
 
@@ -466,30 +496,7 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
     const int start_slot = n_step % 3;
 
     const bool table = H->n_table > 0;
-        TermParams tp{};
-    tp.orp = H->orp; tp.ocol = H->ocol; tp.oidx = H->oidx; tp.vtab = H->vtab; tp.diag = H->diag;
-    tp.rowptr = H->rowptr; tp.col = H->col; tp.val = H->val;
-    tp.n_orb = H->n_orb;
-    tp.partial = partial;
-    tp.n_table = H->n_table;
-    tp.packed = H->packed;
-    tp.single_real = H->single_real;
-    tp.device = H->device;
-    tp.walk_stride = 0; tp.walk_run = 1;
-    tp.n_lat_off = H->n_lat_off;
-    for (int j = 0; j < H->n_lat_off; ++j) { tp.lat_off[j] = H->lat_off[j]; tp.lat_delta[j] = H->lat_delta[j]; }
-    tp.lat_flags = H->lat_flags;
-    tp.n_regular = H->n_regular;
-    tp.lat_periodic3 = H->lat_periodic3;
-    tp.sq8_line = H->sq8_line; tp.dline = H->dline;
-    tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
-    tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
-    // L2 prefetch of the vector rows a few tiles ahead (term_ph.cuh, producer warp).  The leading edge of the gather
-    // window is the farthest neighbour: the largest lattice stride on uniform lattices, else the widest |col - row|.
-    tp.pf_dist = knob("pf", 0);
-    tp.pf_mask = knob("pf_mask", 3);
-    tp.pf_lead = H->n_lat_off > 0 ? H->lat_off[H->n_lat_off - 1] : H->halo_rows;
-    if (knob("pf_lead", -1) >= 0) tp.pf_lead = knob("pf_lead", -1);
+    TermParams tp = matrix_params(H, partial);
     const bool reverse_odd = knob("rev", 1) != 0;         // odd terms sweep backwards (term_ph.cuh)
 
     std::vector<TermParams> term;
@@ -634,20 +641,7 @@ extern "C" int tbpm_haydock(tbpm_ham *H, const int64_t *sites, int n_site, int n
     int64_t *d_sites = reinterpret_cast<int64_t *>(W + P.sites_off);
     TBPM_CUDA_TRY(cudaMemcpyAsync(d_sites, sites, sizeof(int64_t) * (size_t)n_site, cudaMemcpyHostToDevice, st));
     const bool table = H->n_table > 0;
-    TermParams tp{};
-    tp.orp = H->orp; tp.ocol = H->ocol; tp.oidx = H->oidx; tp.vtab = H->vtab; tp.diag = H->diag;
-    tp.rowptr = H->rowptr; tp.col = H->col; tp.val = H->val;
-    tp.n_orb = H->n_orb;
-    tp.partial = partial;
-    tp.n_table = H->n_table; tp.packed = H->packed; tp.single_real = H->single_real; tp.device = H->device;
-    tp.walk_stride = 0; tp.walk_run = 1;
-    tp.n_lat_off = H->n_lat_off;
-    for (int j = 0; j < H->n_lat_off; ++j) { tp.lat_off[j] = H->lat_off[j]; tp.lat_delta[j] = H->lat_delta[j]; }
-    tp.lat_flags = H->lat_flags; tp.n_regular = H->n_regular; tp.lat_periodic3 = H->lat_periodic3;
-    tp.sq8_line = H->sq8_line; tp.dline = H->dline;
-    tp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
-    tp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
-    tp.pf_lead = H->n_lat_off > 0 ? H->lat_off[H->n_lat_off - 1] : H->halo_rows;
+    TermParams tp = matrix_params(H, partial);
     // t = H u_n and <u_n|t> in one sweep: the last-term shape of the fused kernel with psi' := 1 * T_k, first flush, bra = u_n
     tp.a = 1.0; tp.ca = make_double2(1.0, 0.0); tp.n_acc = 1; tp.flags = F_ACC_INIT | F_REDUCE;
     const int nn_grid = std::min(H->num_sms * 4, 64);
@@ -678,6 +672,111 @@ extern "C" int tbpm_haydock(tbpm_ham *H, const int64_t *sites, int n_site, int n
         }
     }
     TBPM_CUDA_TRY(cudaGetLastError());
+    return TBPM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// NEXT-4: AC-conductivity correlation  corr[b][n] = < psi2(n dt) | J_a | psi1(n dt) >,  psi1(0) = [1 - f(H)] J_b psi0,
+// psi2(0) = f(H) psi0  (reading #30).  Everything runs on the fused term kernels: a Chebyshev series (Fermi operator or
+// time step) is K - 1 term launches with the series' coefficients, J x is the first-term shape with J's matrix, and
+// <psi2|J_a psi1> is the last-term shape (first flush of 1 * T, bra = psi2) with J_a's matrix.  One tile of states at a time:
+// two sets of three rotating vectors.
+// ---------------------------------------------------------------------------------------------------------------------
+extern "C" int tbpm_corr_ac_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes)
+{
+    if (!H || n_state < 0 || !workspace_bytes) return TBPM_EINVAL;
+    const Plan P = make_plan(H->n_orb, n_state, H->opt_tile);
+    *workspace_bytes = P.vec0_off + 6 * P.full_vec;
+    return TBPM_OK;
+}
+
+extern "C" int tbpm_corr_ac(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const double *psi0, int n_state, int n_step, double dt, double rescale,
+                            double beta, double mu, double *corr, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!H || !Ja || !Jb || n_state < 0 || n_step < 0 || !(rescale > 0.0) || !(dt >= 0.0) || !std::isfinite(dt) || !std::isfinite(rescale))
+        return TBPM_EINVAL;
+    if (Ja->n_orb != H->n_orb || Jb->n_orb != H->n_orb || Ja->device != H->device || Jb->device != H->device) return TBPM_EINVAL;
+    if (n_state == 0) return TBPM_OK;
+    if (!psi0 || !corr || !workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || (reinterpret_cast<uintptr_t>(psi0) & 15u)) return TBPM_EINVAL;
+    const Plan P = make_plan(H->n_orb, n_state, H->opt_tile);
+    if (workspace_bytes < P.vec0_off + 6 * P.full_vec) return TBPM_ENOMEM;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const long long launches0 = total_launches();
+
+    std::vector<double> ct(2 * 8192), cf(2 * 8192), cg(2 * 8192);   // time step, f, 1 - f
+    int Kt = 0, Kf = 0, Kg = 0, rc;
+    if ((rc = tbpm_cheb_coeff(rescale * dt, 1e-15, 8192, &Kt, ct.data()))) return rc;
+    if ((rc = tbpm_fermi_coeff(beta, mu, rescale, 0, 1e-13, 8192, &Kf, cf.data()))) return rc;
+    if ((rc = tbpm_fermi_coeff(beta, mu, rescale, 1, 1e-13, 8192, &Kg, cg.data()))) return rc;
+
+    char *W = static_cast<char *>(workspace);
+    double *partial = reinterpret_cast<double *>(W + P.partial_off);
+    const TermParams mh = matrix_params(H, partial), ma = matrix_params(Ja, partial), mb = matrix_params(Jb, partial);
+    const bool reverse_odd = knob("rev", 1) != 0;
+    std::vector<TermParams> term;
+    const int n_out = n_step + 1;
+
+    for (int t = 0; t < P.n_tile; ++t) {
+        const int state0 = t * P.tile;
+        const int n_valid = std::min(P.tile, n_state - state0);
+        const int bt = (t == P.n_tile - 1) ? P.last_bt : P.tile;
+        const size_t vec = align_up((size_t)H->n_orb * bt * sizeof(double2));
+        char *base = W + P.vec0_off;
+        double2 *A[3], *B[3];
+        for (int i = 0; i < 3; ++i) { A[i] = reinterpret_cast<double2 *>(base + i * vec); B[i] = reinterpret_cast<double2 *>(base + (3 + i) * vec); }
+        const int64_t n_el = H->n_orb * bt;
+        if (n_el == 0) continue;
+        k_interleave<<<(unsigned)((n_el + kThreads - 1) / kThreads), kThreads, 0, st>>>(reinterpret_cast<const double2 *>(psi0), H->n_orb, state0,
+                                                                                       n_valid, bt, A[0], B[0]);
+        count_launches(1);
+        int grid = 1;
+        // a Chebyshev series sum_k c_k T_k(H / s) applied to buf[slot]; returns the slot that holds the result
+        auto series = [&](double2 **buf, int slot, int K, const std::vector<double> &c) -> int {
+            double2 *psi = buf[slot], *t1 = buf[(slot + 1) % 3], *acc = buf[(slot + 2) % 3];
+            TermParams tp = mh;
+            tp.psi0 = psi;                                // the last term's dot products are not used here
+            if (K == 1) {
+                TermParams t0 = tp;
+                t0.x = psi; t0.y = t1; t0.acc = acc; t0.a = 0.0;
+                t0.ca = make_double2(c[0], c[1]); t0.n_acc = 1; t0.flags = F_SKIP_H | F_ACC_INIT | F_REDUCE;
+                rc = launch_term(bt, H->n_table > 0, 1, t0, H->num_sms, st, &grid);
+            } else {
+                step_terms(tp, K, c, rescale, reverse_odd, psi, t1, acc, term);
+                for (int k = 1; k < K && !rc; ++k) rc = launch_term(bt, H->n_table > 0, H->opt_kernel, term[k], H->num_sms, st, &grid);
+            }
+            return (slot + 2) % 3;
+        };
+        // corr[.][n] = <psi2|J_a psi1>: J_a psi1 goes to a free buffer of set A
+        auto cross = [&](int sa, int sb, int n) {
+            TermParams tp = ma;
+            tp.x = A[sa]; tp.psi0 = B[sb]; tp.acc = A[(sa + 1) % 3]; tp.y = A[(sa + 2) % 3];
+            tp.a = 1.0; tp.ca = make_double2(1.0, 0.0); tp.n_acc = 1; tp.flags = F_ACC_INIT | F_REDUCE;
+            rc = launch_term(bt, Ja->n_table > 0, Ja->opt_kernel, tp, Ja->num_sms, st, &grid);
+            k_reduce_final<<<bt, 96, 0, st>>>(partial, grid, bt, n_valid, state0, n_out, n, corr, nullptr);
+            count_launches(1);
+        };
+        rc = TBPM_OK;
+        {   // A[1] = J_b psi0 (first-term shape: y = a J x)
+            TermParams tp = mb;
+            tp.x = A[0]; tp.y = A[1]; tp.acc = A[2]; tp.psi0 = A[0];
+            tp.a = 1.0; tp.n_acc = 0; tp.flags = F_WRITE_Y;
+            rc = launch_term(bt, Jb->n_table > 0, Jb->opt_kernel, tp, Jb->num_sms, st, &grid);
+        }
+        if (rc) return rc;
+        int sa = series(A, 1, Kg, cg);                    // psi1 = [1 - f(H)] J_b psi0
+        if (rc) return rc;
+        int sb = series(B, 0, Kf, cf);                    // psi2 = f(H) psi0
+        if (rc) return rc;
+        cross(sa, sb, 0);
+        for (int n = 1; n <= n_step && !rc; ++n) {
+            sa = series(A, sa, Kt, ct);
+            if (!rc) sb = series(B, sb, Kt, ct);
+            if (!rc) cross(sa, sb, n);
+        }
+        if (rc) return rc;
+    }
+    TBPM_CUDA_TRY(cudaGetLastError());
+    H->last_launches = total_launches() - launches0;
     return TBPM_OK;
 }
 

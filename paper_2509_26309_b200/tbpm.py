@@ -57,6 +57,9 @@ def lib() -> C.CDLL:
         L.tbpm_propagate_qe_bytes.argtypes = [vp, C.c_int, C.c_int, P(sz)]
         L.tbpm_propagate_qe.argtypes = [vp, vp, C.c_int, C.c_int, dbl, dbl, vp, C.c_int, vp, vp, vp, vp, sz, vp]
         L.tbpm_haydock.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp, sz, vp]
+        L.tbpm_fermi_coeff.argtypes = [dbl, dbl, dbl, C.c_int, dbl, C.c_int, P(C.c_int), vp]
+        L.tbpm_corr_ac_bytes.argtypes = [vp, C.c_int, P(sz)]
+        L.tbpm_corr_ac.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, dbl, dbl, dbl, dbl, vp, vp, sz, vp]
         L.tbpm_last_launch_count.restype = i64
         L.tbpm_last_launch_count.argtypes = [vp]
         L.tbpm_set_option.argtypes = [vp, C.c_int, i64]
@@ -253,6 +256,32 @@ def tbpm_haydock(H: Hamiltonian, sites, n_iter: int, workspace: Optional[torch.T
                                 workspace.numel(), _stream(dev))
     _check(rc, "tbpm_haydock")
     return a, b
+
+
+def tbpm_fermi_coeff(beta: float, mu: float, rescale: float, one_minus: bool = False, tol: float = 1e-13, kcap: int = 8192) -> torch.Tensor:
+    """Host only: real Chebyshev coefficients [K] of the Fermi operator (or of 1 - f) on [-rescale, rescale]."""
+    buf = torch.empty(kcap, dtype=torch.complex128)
+    K = C.c_int(0)
+    _check(lib().tbpm_fermi_coeff(beta, mu, rescale, int(one_minus), tol, kcap, C.byref(K), C.c_void_p(buf.data_ptr())), "tbpm_fermi_coeff")
+    return buf[: K.value].real.clone()
+
+
+def tbpm_corr_ac(H: Hamiltonian, Ja: Hamiltonian, Jb: Hamiltonian, psi0: torch.Tensor, n_step: int, dt: float, rescale: float, beta: float,
+                 mu: float) -> torch.Tensor:
+    """NEXT-4: corr complex128 [n_state][n_step + 1], entry n = <psi2(n dt)|J_a|psi1(n dt)>."""
+    _need_cuda(psi0)
+    dev = H.device
+    psi0 = psi0.contiguous()
+    n_state = psi0.shape[0]
+    wb = C.c_size_t(0)
+    _check(lib().tbpm_corr_ac_bytes(H.handle, n_state, C.byref(wb)), "tbpm_corr_ac_bytes")
+    ws = _bytes(wb.value, dev)
+    corr = torch.zeros((n_state, n_step + 1), dtype=torch.complex128, device=dev)
+    with torch.cuda.device(dev):
+        rc = lib().tbpm_corr_ac(H.handle, Ja.handle, Jb.handle, _ptr(psi0), n_state, n_step, dt, rescale, beta, mu, _ptr(corr), _ptr(ws),
+                                ws.numel(), _stream(dev))
+    _check(rc, "tbpm_corr_ac")
+    return corr
 
 
 def tbpm_dos(corr: torch.Tensor, dt: float, rescale: float):

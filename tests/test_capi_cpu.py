@@ -54,6 +54,27 @@ def test_cheb_coeff_host_logic():
     assert tbpm.lib().tbpm_cheb_coeff(-1.0, 1e-15, 4, C.byref(K), buf) == tbpm.TBPM_EINVAL
 
 
+def test_fermi_coeff_host_logic():
+    """NEXT-4: sum_k c_k T_k(x) = 1 / (exp(beta (s x - mu)) + 1) on [-1, 1] (closed form), the complement, beta = 0, bad arguments."""
+    for beta, mu, s in ((2.0, 0.3, 4.8), (11.0, -1.0, 4.8), (0.5, 0.0, 9.0)):
+        c = tbpm.tbpm_fermi_coeff(beta, mu, s).numpy()
+        g = tbpm.tbpm_fermi_coeff(beta, mu, s, one_minus=True).numpy()
+        x = np.linspace(-1, 1, 201)
+        Tk = np.cos(np.outer(np.arange(len(c)), np.arccos(x)))
+        f = 1.0 / (np.exp(beta * (s * x - mu)) + 1.0)
+        assert np.abs(c @ Tk - f).max() < 1e-11 and np.abs(g @ Tk - (1 - f)).max() < 1e-11
+        assert abs(c[-1]) >= 1e-13
+    assert tbpm.tbpm_fermi_coeff(0.0, 0.0, 3.0).tolist() == [0.5]
+    K = C.c_int(0)
+    buf = (C.c_double * 8)()
+    L = tbpm.lib()
+    assert L.tbpm_fermi_coeff(11.0, 0.0, 4.8, 0, 1e-13, 4, C.byref(K), buf) == tbpm.TBPM_ENOMEM and K.value > 4
+    assert L.tbpm_fermi_coeff(-1.0, 0.0, 4.8, 0, 1e-13, 4, C.byref(K), buf) == tbpm.TBPM_EINVAL
+    assert L.tbpm_corr_ac(None, None, None, None, 1, 1, 0.1, 1.0, 1.0, 0.0, None, None, 0, None) == tbpm.TBPM_EINVAL
+    assert L.tbpm_haydock(None, None, 1, 1, None, None, None, 0, None) == tbpm.TBPM_EINVAL
+    assert L.tbpm_propagate_qe(None, None, 1, 1, 0.1, 1.0, None, 0, None, None, None, None, 0, None) == tbpm.TBPM_EINVAL
+
+
 def test_sizes_and_argument_checks():
     p, s = tbpm.tbpm_build_bytes(8192, 12288, False)
     assert p >= 24576 * 20 + 8193 * 8 and s > 0

@@ -1,5 +1,5 @@
-"""Parity of the NEXT rows of SURVEY.md 8(f) on the GPU (`-m gpu`): quasi-eigenstates (NEXT-3, tbpm_propagate_qe) and the Haydock
-recursion (NEXT-2, tbpm_haydock) against the oracle's plain statements (oracle.quasi_eigenstates / oracle.haydock, themselves
+"""Parity of the NEXT rows of SURVEY.md 8(f) on the GPU (`-m gpu`): quasi-eigenstates (NEXT-3, tbpm_propagate_qe), the Haydock
+recursion (NEXT-2, tbpm_haydock) and the AC-conductivity correlation (NEXT-4, tbpm_corr_ac) against the oracle's plain statements (oracle.quasi_eigenstates / oracle.haydock, themselves
 pinned in tests/test_oracle_next_pins.py), element by element on the same seeded inputs."""
 import math
 
@@ -114,3 +114,27 @@ def test_haydock_chain_closed_form_and_ldos(dev, oracle_mod):
     assert tbpm.lib().tbpm_haydock(Hs.handle, None, 0, 5, None, None, None, 0, None) == tbpm.TBPM_OK   # n_site = 0
     with pytest.raises(tbpm.TbpmError):
         tbpm.tbpm_haydock(Hs, [64], 3)
+
+
+@pytest.mark.parametrize("Lx,Ly,phi_den,n_state,n_step,beta,mu,axes", [
+    (64, 24, 16, 3, 10, 2.0, 0.4, (0, 1)),                           # padded tile of 4; sigma_xy-type correlation
+    (128, 16, 32, 8, 6, 6.0, -0.8, (0, 0)),                          # W = 128: H runs on the square-lattice kernel; sigma_xx
+    (48, 40, 8, 9, 5, 1.0, 0.0, (1, 1)),                             # tile of 8 + padded tile of 1; sigma_yy
+])
+def test_corr_ac(dev, oracle_mod, Lx, Ly, phi_den, n_state, n_step, beta, mu, axes):
+    """NEXT-4: <psi2(t)|J_a|psi1(t)> with psi1 = [1 - f(H)] J_b psi0, psi2 = f(H) psi0, every entry against the oracle."""
+    w = W.make_workload(4, device=dev, Lx=Lx, Ly=Ly, phi_den=phi_den)
+    psi0 = w.psi0(device=dev, n_state=n_state)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    J, jn = [], []
+    for ax in axes:
+        n, ji, jj, jv = W.square_current_hops(Lx, Ly, ax, phi_den=phi_den, device=dev)
+        J.append(tbpm.tbpm_build(n, None, ji, jj, jv))
+        jn.append((ji.cpu().numpy(), jj.cpu().numpy(), jv.cpu().numpy()))
+    corr = tbpm.tbpm_corr_ac(H, J[0], J[1], psi0, n_step, w.dt, w.rescale, beta, mu)
+    hi, hj, hv, on = to_np(w)
+    ref = oracle_mod.corr_ac(w.n_orb, on, hi, hj, hv, jn[0], jn[1], psi0.cpu().numpy(), n_step, w.dt, w.rescale, beta, mu)
+    assert corr.shape == (n_state, n_step + 1)
+    assert np.abs(corr.cpu().numpy() - ref).max() <= 1e-10 * max(1.0, np.abs(ref).max())
+    again = tbpm.tbpm_corr_ac(H, J[0], J[1], psi0, n_step, w.dt, w.rescale, beta, mu)
+    assert torch.equal(corr, again)                                  # deterministic
