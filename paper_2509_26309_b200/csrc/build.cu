@@ -202,7 +202,7 @@ __global__ void k_fill(int64_t n_hop, const int32_t *__restrict__ hop_i, const i
     }
 }
 
-// 4. per-row insertion sort by column + checks
+// 4. per-row sort by column (one thread per row) + checks
 __global__ void k_sort_rows(int64_t n_orb, const int64_t *__restrict__ rowptr, int32_t *col, double2 *val, int32_t *status)
 {
     int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -213,17 +213,39 @@ __global__ void k_sort_rows(int64_t n_orb, const int64_t *__restrict__ rowptr, i
         int64_t b = rowptr[r], e = rowptr[r + 1];
         len = (int)(e - b);
         nlen = -len;
-        for (int64_t p = b + 1; p < e; ++p) {
-            int32_t c = col[p];
-            double2 v = val[p];
-            int64_t q = p - 1;
-            while (q >= b && col[q] > c) {
-                col[q + 1] = col[q];
-                val[q + 1] = val[q];
-                --q;
+        if (len <= 32) {                                    // lattice rows: insertion sort
+            for (int64_t p = b + 1; p < e; ++p) {
+                int32_t c = col[p];
+                double2 v = val[p];
+                int64_t q = p - 1;
+                while (q >= b && col[q] > c) {
+                    col[q + 1] = col[q];
+                    val[q + 1] = val[q];
+                    --q;
+                }
+                col[q + 1] = c;
+                val[q + 1] = v;
             }
-            col[q + 1] = c;
-            val[q + 1] = v;
+        } else {                                            // hub rows: in-place heap sort, O(len log len) (columns are unique)
+            int32_t *c = col + b;
+            double2 *v = val + b;
+            auto sift = [&](int root, int end) {
+                for (;;) {
+                    int child = 2 * root + 1;
+                    if (child >= end) break;
+                    if (child + 1 < end && c[child + 1] > c[child]) ++child;
+                    if (c[root] >= c[child]) break;
+                    const int32_t tc = c[root]; c[root] = c[child]; c[child] = tc;
+                    const double2 tv = v[root]; v[root] = v[child]; v[child] = tv;
+                    root = child;
+                }
+            };
+            for (int i = len / 2 - 1; i >= 0; --i) sift(i, len);
+            for (int end = len - 1; end > 0; --end) {
+                const int32_t tc = c[0]; c[0] = c[end]; c[end] = tc;
+                const double2 tv = v[0]; v[0] = v[end]; v[end] = tv;
+                sift(0, end);
+            }
         }
         for (int64_t p = b; p < e; ++p) {
             double2 v = val[p];

@@ -102,6 +102,11 @@ def test_build_edge_cases(dev, oracle_mod):
     H = tbpm.tbpm_build(n, None, star.hop_i, star.hop_j, star.hop_val)
     assert H.max_row_nnz == n - 1
     assert_csr_bit_exact(H, oracle_mod, star)
+    sp0 = star.psi0(device=dev, n_state=2)                            # a row of 2,999 entries on the general kernel
+    sc, sn, _ = tbpm.tbpm_propagate(H, sp0, 4, star.dt, star.rescale)
+    shi, shj, shv, _ = to_np(star)
+    sref, _ = oracle_mod.propagate(n, None, shi, shj, shv, sp0.cpu().numpy(), 4, star.dt, star.rescale)
+    assert np.abs(sc.cpu().numpy() - sref).max() <= CORR_TOL and np.abs(sn.cpu().numpy() - 1).max() <= NORM_TOL
     # errors
     for hi, hj, code in (([1], [1], tbpm.TBPM_EDIAG), ([0, 1], [1, 0], tbpm.TBPM_EDUP), ([0, 0], [1, 1], tbpm.TBPM_EDUP),
                          ([0], [3], tbpm.TBPM_EINDEX), ([-1], [2], tbpm.TBPM_EINDEX)):
