@@ -7,7 +7,7 @@ tbpm_build (hop list -> CSR + kernel layout) followed by tbpm_propagate of ALL t
 tile, per-step correlation + norm).  Inputs are resident in HBM when the timed region starts.
 `value` = n_state * n_block * (K-1) * nnz / step time, summed over ranks.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5|5ldos] [--block B] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5|5ldos|3qe|5haydock] [--block B] [--impl reference]
 
 Default workload: BASELINE.json:configs[4] (cubic 256^3 + Anderson disorder, 16,777,216 orbitals x 32 states): the largest
 single-GPU configuration, one of the >= 16 M-orbital configs `north_star` sets its target on.  The full run length of a
@@ -17,6 +17,8 @@ the line also carries `per_workload`: cfg3, cfg4 and cfg5's 64-site LDOS leg mea
 Multi-GPU: states are independent, so every rank propagates its own batch of seeded states on a replica of
 H (paper_2509_26309_b200/replicas.py); no data-path collective; scaling is weak.
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+`--workload 3qe` (cfg3 + quasi-eigenstates at 2 energies, NEXT-3) and `--workload 5haydock` (Haydock recursion from cfg5's 64
+sites, NEXT-2) time the two NEXT rows that have kernels of their own (one GPU, one JSON line with `roofline`).
 """
 from __future__ import annotations
 
@@ -428,6 +430,82 @@ def main_ours(args):
     return 0
 
 
+# ---------------------------------------------------------------------------------------------------------------------
+# the NEXT rows with kernels of their own: quasi-eigenstates (3qe) and the Haydock recursion (5haydock); one GPU
+# ---------------------------------------------------------------------------------------------------------------------
+def main_next(args):
+    import torch
+    from paper_2509_26309_b200 import tbpm, workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the TBPM path has no CPU fallback")
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, peak_src = load_peaks()
+    cfg = int(args.workload[0])
+    haydock = args.workload.endswith("haydock")
+    w = W.make_workload(cfg, device=dev)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val, 0)
+    block = args.block or 8
+    K = len(tbpm.tbpm_cheb_coeff(w.rescale * w.dt))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    if haydock:
+        n_state = w.ldos_n_site
+        sites = W.ldos_sites(w.n_orb, n_state)
+        ws = torch.empty(tbpm.tbpm_propagate_bytes(H, n_state), dtype=torch.uint8, device=dev)
+        run = lambda: tbpm.tbpm_haydock(H, sites, block, workspace=ws)
+        units = n_state * block * H.nnz                              # H applications x nnz
+        tile = 8
+        mat = H.lattice_bytes_per_term if H.lattice_kind else H.matrix_bytes_per_term
+        # per recursion level and tile: H u (matrix, gather u, write t) + update (read t, u, u_prev, write u_next): matrix + 6 vectors
+        bytes_step = (n_state // tile) * block * (mat + 6 * 16 * w.n_orb * tile)
+        what = "Haydock recursion: H u fused with <u|H u> (k_term_l3, last-term shape) + three-vector update fused with the norm (k_haydock_update)"
+        count = "per level and tile of 8 sites: matrix bytes of the running kernel's layout + 6 vectors (gather u, write t; read t, u, u_prev, write u_next)"
+    else:
+        n_state = w.n_state
+        psi0 = w.psi0(device=dev, n_state=n_state)
+        energies = [0.0, 0.5 * w.rescale]
+        run = lambda: tbpm.tbpm_propagate_qe(H, psi0, energies, block, w.dt, w.rescale)
+        units = n_state * block * (K - 1) * H.nnz
+        # per time step: the K - 1 terms (matrix + 3 vectors each) + the accumulation sweep (read psi', read + write n_E vectors)
+        bytes_step = block * ((K - 1) * (H.matrix_bytes_per_term + 48 * w.n_orb * n_state) + (1 + 2 * len(energies)) * 16 * w.n_orb * n_state)
+        what = "propagation + quasi-eigenstates at 2 energies: k_term_ph per term, k_qe_axpy once per time step"
+        count = "per time step: (K - 1) x (matrix + 3 vectors) + (1 + 2 n_E) vectors of the accumulation sweep (workspace allocation and export included in the time)"
+    for _ in range(max(args.warmup, 1)):
+        run()
+    torch.cuda.synchronize()
+    launches0 = tbpm.tbpm_total_launch_count()
+    sampler = ClockSampler(0)
+    evs = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); out = run(); e1.record()
+        evs.append((e0, e1))
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = sum(a.elapsed_time(b) for a, b in evs)
+    achieved = args.steps * bytes_step / (ms * 1e-3) / 1e9
+    line = {"metric": "Hamiltonian applications*nnz/sec (complex128)" if haydock else METRIC, "value": args.steps * units / (ms * 1e-3), "unit": UNIT,
+            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "complex128", "data": "synthetic",
+            "config": {"workload": w.name + ("-haydock" if haydock else "-qe"), "n_orb": w.n_orb, "nnz": H.nnz, "n_state": n_state,
+                       "n_step_per_bench_step": block, "what": what, "l2": "256 MB flush between iterations; working set > L2"},
+            "gpu_launches": int(tbpm.tbpm_total_launch_count() - launches0), "clocks": clocks,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                         "peak_source": peak_src, "count": count}}
+    if haydock:
+        a, b = out
+        line["finite"] = bool(torch.isfinite(a).all() and torch.isfinite(b).all() and (b > 0).all())
+    else:
+        line["max_norm_dev"] = float((out[1] - 1).abs().max())
+    print(json.dumps(line))
+    return 0
+
+
 if __name__ == "__main__":
     a = parse_args()
+    if a.workload.endswith("qe") or a.workload.endswith("haydock"):
+        sys.exit(main_next(a))
     sys.exit(main_reference(a) if a.impl == "reference" else main_ours(a))

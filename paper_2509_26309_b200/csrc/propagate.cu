@@ -644,7 +644,7 @@ extern "C" int tbpm_haydock(tbpm_ham *H, const int64_t *sites, int n_site, int n
     TermParams tp = matrix_params(H, partial);
     // t = H u_n and <u_n|t> in one sweep: the last-term shape of the fused kernel with psi' := 1 * T_k, first flush, bra = u_n
     tp.a = 1.0; tp.ca = make_double2(1.0, 0.0); tp.n_acc = 1; tp.flags = F_ACC_INIT | F_REDUCE;
-    const int nn_grid = std::min(H->num_sms * 4, 64);
+    const int nn_grid = std::max(1, std::min(H->num_sms * 8, (int)((kAuxBytes / sizeof(double) - 4 * kMaxBT) / kMaxBT)));   // norm partials: [nn_grid][bt] doubles in the aux area
     int rc = TBPM_OK;
     for (int t = 0; t < P.n_tile; ++t) {
         const int state0 = t * P.tile;
