@@ -112,8 +112,10 @@ void tbpm_free(tbpm_ham *H);
  * TBPM_OPT_TILE).  The library reads nothing from the environment: its behaviour is a function of its arguments. */
 #define TBPM_OPT_TILE 1   /* states propagated together per tile (SpMM width, PAPER.md:554 runs one state at a time):
                              1, 2, 4, 8 (default: 8 interleaved complex128 = one 128-byte line per row), 16, 32        */
-#define TBPM_OPT_KERNEL 2 /* 0 (default): the fastest kernel that applies (rolling-window on lattices, else phased, else
-                             general); 1: every term on the general kernel; 2: no rolling-window kernel                */
+#define TBPM_OPT_KERNEL 2 /* 0 (default): the fastest kernel that applies (tiles of 8 states on a recognised lattice: the
+                             three-dimensional / square-lattice / rolling-window kernel; else phased; else general);
+                             1: every term on the general kernel; 2: no lattice kernel (phased, else general);
+                             3: of the lattice kernels only the rolling-window one (tests)                               */
 int tbpm_set_option(tbpm_ham *H, int option, int64_t value);
 
 /* ---- a2-a7: propagate ------------------------------------------------------------------------------------------------

@@ -44,12 +44,12 @@ __device__ __forceinline__ void st_stream(double2 *p, double2 v) { __stcs(p, v);
 // offsets, so they are issued first; the row offsets of the NEXT grid-stride iteration are prefetched while the current
 // row is processed, which leaves a two-deep dependent chain (column/value index -> gather) per row.
 // ---------------------------------------------------------------------------------------------------------------------
-template <int BT, bool TABLE, int MINB>
-__global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p)
+// Rows first_row, first_row + stride, ... of one term for state b; the three partial sums of the last term are returned in s_*.
+// COH: the vectors were written by OTHER thread blocks earlier in the same kernel (k_small_steps): read them through the L2.
+template <int BT, bool TABLE, bool COH>
+__device__ __forceinline__ void cheb_term_rows(const TermParams &p, int64_t first_row, int64_t stride, int b, double &s_re, double &s_im,
+                                               double &s_nn)
 {
-    constexpr int kRowsPerBlock = kThreads / BT;
-    const int b = threadIdx.x % BT;
-    const int64_t stride = (int64_t)gridDim.x * kRowsPerBlock;
     const int flags = p.flags;
     const int n_acc = p.n_acc;
     const bool skip_h = flags & F_SKIP_H;
@@ -57,9 +57,8 @@ __global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p
     const bool need_xrow = skip_h || n_acc >= 2 || (TABLE && p.diag != nullptr);
     const bool need_acc = n_acc > 0 && !(flags & F_ACC_INIT);
     const bool reduce = flags & F_REDUCE;
-    double s_re = 0.0, s_im = 0.0, s_nn = 0.0;
-
-    int64_t row = (int64_t)blockIdx.x * kRowsPerBlock + threadIdx.x / BT;
+    auto ldx = [](const double2 *q) -> double2 { return COH ? __ldcg(q) : __ldg(q); };
+    int64_t row = first_row;
     int64_t q0 = 0, q1 = 0;                                 // offsets of the current row (prefetched)
     if (row < p.n_orb && !skip_h) {
         if (TABLE) { q0 = __ldg(p.orp + row); q1 = __ldg(p.orp + row + 1); }
@@ -70,10 +69,10 @@ __global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p
         // ---- level 0: everything that needs no index
         double2 yold = make_double2(0.0, 0.0), xrow = yold, aold = yold, z = yold;
         double d = 0.0;
-        if (need_y) yold = ld_stream(p.y + e);
-        if (need_acc) aold = ld_stream(p.acc + e);
-        if (reduce) z = ld_stream(p.psi0 + e);
-        if (need_xrow) xrow = __ldg(p.x + e);
+        if (need_y) yold = COH ? __ldcg(p.y + e) : ld_stream(p.y + e);
+        if (need_acc) aold = COH ? __ldcg(p.acc + e) : ld_stream(p.acc + e);
+        if (reduce) z = COH ? __ldcg(p.psi0 + e) : ld_stream(p.psi0 + e);
+        if (need_xrow) xrow = ldx(p.x + e);
         if (TABLE && p.diag != nullptr && !skip_h) d = __ldg(p.diag + row);
         const int64_t nrow = row + stride;
         int64_t nq0 = 0, nq1 = 0;
@@ -104,11 +103,11 @@ __global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p
                     if (p2) { c2 = __ldg(p.col + q + 2); v2 = __ldg(p.val + q + 2); }
                     if (p3) { c3 = __ldg(p.col + q + 3); v3 = __ldg(p.val + q + 3); }
                 }
-                const double2 x0 = __ldg(p.x + (int64_t)c0 * BT + b);
+                const double2 x0 = ldx(p.x + (int64_t)c0 * BT + b);
                 double2 x1 = make_double2(0.0, 0.0), x2 = x1, x3 = x1;
-                if (p1) x1 = __ldg(p.x + (int64_t)c1 * BT + b);
-                if (p2) x2 = __ldg(p.x + (int64_t)c2 * BT + b);
-                if (p3) x3 = __ldg(p.x + (int64_t)c3 * BT + b);
+                if (p1) x1 = ldx(p.x + (int64_t)c1 * BT + b);
+                if (p2) x2 = ldx(p.x + (int64_t)c2 * BT + b);
+                if (p3) x3 = ldx(p.x + (int64_t)c3 * BT + b);
                 cfma(h, v0, x0);
                 cfma(h, v1, x1);
                 cfma(h, v2, x2);
@@ -137,31 +136,159 @@ __global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p
                 s_nn = fma(s.y, s.y, s_nn);
                 p.acc[e] = s;                               // psi': T_0 of the next step, gathered right away
             } else {
-                st_stream(p.acc + e, s);
+                if (COH) p.acc[e] = s; else st_stream(p.acc + e, s);
             }
         }
         q0 = nq0;
         q1 = nq1;
     }
 
-    if (reduce) {
-        __shared__ double sm[kThreads / 32][kMaxBT][3];
+}
+
+// per-thread sums -> warp shuffles -> shared memory -> one partial per block (fixed order)
+template <int BT, int THREADS>
+__device__ __forceinline__ void block_partial(double s_re, double s_im, double s_nn, double *partial, int block)
+{
+    __shared__ double sm[THREADS / 32][kMaxBT][3];
 #pragma unroll
-        for (int o = 16; o >= BT; o >>= 1) {                // lanes with equal (lane % BT) hold the same state
-            s_re += __shfl_xor_sync(0xffffffffu, s_re, o);
-            s_im += __shfl_xor_sync(0xffffffffu, s_im, o);
-            s_nn += __shfl_xor_sync(0xffffffffu, s_nn, o);
+    for (int o = 16; o >= BT; o >>= 1) {                    // lanes with equal (lane % BT) hold the same state
+        s_re += __shfl_xor_sync(0xffffffffu, s_re, o);
+        s_im += __shfl_xor_sync(0xffffffffu, s_im, o);
+        s_nn += __shfl_xor_sync(0xffffffffu, s_nn, o);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane < BT) { sm[warp][lane][0] = s_re; sm[warp][lane][1] = s_im; sm[warp][lane][2] = s_nn; }
+    __syncthreads();
+    if (threadIdx.x < BT * 3) {
+        const int bb = threadIdx.x / 3, c = threadIdx.x % 3;
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < THREADS / 32; ++w) t += sm[w][bb][c];
+        partial[((int64_t)block * BT + bb) * 3 + c] = t;
+    }
+    __syncthreads();
+}
+
+template <int BT, bool TABLE, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p)
+{
+    constexpr int kRowsPerBlock = kThreads / BT;
+    double s_re = 0.0, s_im = 0.0, s_nn = 0.0;
+    cheb_term_rows<BT, TABLE, false>(p, (int64_t)blockIdx.x * kRowsPerBlock + threadIdx.x / BT, (int64_t)gridDim.x * kRowsPerBlock,
+                                     threadIdx.x % BT, s_re, s_im, s_nn);
+    if (p.flags & F_REDUCE) block_partial<BT, kThreads>(s_re, s_im, s_nn, p.partial, blockIdx.x);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Small models (cfg1: 8,192 orbitals, one state) are launch-bound on the path above: 21 launches of ~3 us of device work each per
+// time step.  k_small_steps runs ALL time steps of a tile in ONE launch of one thread-block cluster (8 blocks x 1024 threads on 8
+// SMs; the vectors of such a model live in L2).  A thread owns at most two (row, state) elements for the whole run and keeps their
+// column words, value indices and diagonal in registers, so a term is: gather x (L2), read y / psi', compute, store, and a hardware
+// cluster barrier (barrier.cluster with release / acquire: ~0.3 us) before the next term; block 0 adds the 8 block partials of
+// the last term in a fixed order.  The per-term scalars of the three buffer-rotation phases sit in shared memory.
+// Kernel layout with a value table, rows of <= 4 off-diagonal entries, <= 16,384 elements per vector; anything else takes the
+// launch-per-term path.
+// ---------------------------------------------------------------------------------------------------------------------
+constexpr int kSmallThreads = 1024, kSmallCluster = 8, kSmallMaxK = 28, kSmallCH = 4, kSmallRPT = 2;
+struct TermLite {
+    const double2 *x; double2 *y, *acc;
+    double a; double2 ca, cb, cc;
+    int n_acc, flags;
+};
+struct SmallParams {
+    const TermLite *terms;        // device [3][K]: terms[slot * K + k] for psi in buffer `slot`
+    const uint32_t *orp; const int32_t *ocol; const uint16_t *oidx; const double2 *vtab; const double *diag; const double2 *psi0;
+    int64_t n_orb;
+    int K, n_step, start_slot, n_valid, state0, packed, uniform, max_row_off;
+    double *corr, *norm2, *partial;
+};
+template <int BT>
+__global__ void __launch_bounds__(kSmallThreads, 1) k_small_steps(const SmallParams sp)
+{
+    __shared__ TermLite tl[3 * kSmallMaxK];
+    for (int i = threadIdx.x; i < 3 * sp.K * (int)(sizeof(TermLite) / 4); i += kSmallThreads)
+        reinterpret_cast<uint32_t *>(tl)[i] = __ldg(reinterpret_cast<const uint32_t *>(sp.terms) + i);
+    constexpr int kRowsPerBlock = kSmallThreads / BT;
+    const int b = threadIdx.x % BT;
+    const int64_t stride = (int64_t)gridDim.x * kRowsPerBlock;
+    // the thread's elements and their matrix rows, for the whole run
+    int64_t e[kSmallRPT];
+    int32_t col[kSmallRPT][kSmallCH];
+    double2 val[kSmallRPT][kSmallCH];
+    double dg[kSmallRPT];
+    int nr[kSmallRPT];
+#pragma unroll
+    for (int i = 0; i < kSmallRPT; ++i) {
+        const int64_t row = (int64_t)blockIdx.x * kRowsPerBlock + threadIdx.x / BT + i * stride;
+        nr[i] = -1; e[i] = 0; dg[i] = 0.0;
+#pragma unroll
+        for (int j = 0; j < kSmallCH; ++j) { col[i][j] = 0; val[i][j] = make_double2(0.0, 0.0); }
+        if (row < sp.n_orb) {
+            e[i] = row * BT + b;
+            const uint32_t q0 = sp.uniform ? (uint32_t)row * (uint32_t)sp.max_row_off : __ldg(sp.orp + row);
+            const uint32_t q1 = sp.uniform ? q0 + (uint32_t)sp.max_row_off : __ldg(sp.orp + row + 1);
+            nr[i] = (int)(q1 - q0);
+            for (int j = 0; j < nr[i]; ++j) {
+                const uint32_t w = (uint32_t)__ldg(sp.ocol + q0 + j);
+                const uint32_t id = sp.packed ? (w >> 31) << 15 : (uint32_t)__ldg(sp.oidx + q0 + j);
+                col[i][j] = (int32_t)(w & 0x7fffffffu);
+                val[i][j] = table_value(__ldg(sp.vtab + (id & 0x7fffu)), id);
+            }
+            if (sp.diag) dg[i] = __ldg(sp.diag + row);
         }
-        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-        if (lane < BT) { sm[warp][lane][0] = s_re; sm[warp][lane][1] = s_im; sm[warp][lane][2] = s_nn; }
-        __syncthreads();
-        if (threadIdx.x < BT * 3) {
+    }
+    __syncthreads();
+    int slot = sp.start_slot;
+    for (int n = 0; n < sp.n_step; ++n) {
+        for (int k = 1; k < sp.K; ++k) {
+            const TermLite &t = tl[slot * sp.K + k];
+            const bool sub_y = t.flags & F_SUB_Y, reduce = t.flags & F_REDUCE, wy = t.flags & F_WRITE_Y;
+            const bool need_y = sub_y || t.n_acc == 3, need_acc = t.n_acc > 0 && !(t.flags & F_ACC_INIT);
+            double s_re = 0.0, s_im = 0.0, s_nn = 0.0;
+#pragma unroll
+            for (int i = 0; i < kSmallRPT; ++i) {
+                if (nr[i] < 0) continue;
+                double2 xv[kSmallCH];
+#pragma unroll
+                for (int j = 0; j < kSmallCH; ++j) xv[j] = j < nr[i] ? __ldcg(t.x + (int64_t)col[i][j] * BT + b) : make_double2(0.0, 0.0);
+                const double2 xrow = __ldcg(t.x + e[i]);
+                double2 yold = make_double2(0.0, 0.0), aold = yold, z = yold;
+                if (need_y) yold = __ldcg(t.y + e[i]);
+                if (need_acc) aold = __ldcg(t.acc + e[i]);
+                if (reduce) z = __ldg(sp.psi0 + e[i]);
+                double2 h = make_double2(0.0, 0.0);
+#pragma unroll
+                for (int j = 0; j < kSmallCH; ++j) cfma(h, val[i][j], xv[j]);
+                h.x = fma(dg[i], xrow.x, h.x); h.y = fma(dg[i], xrow.y, h.y);
+                h.x *= t.a; h.y *= t.a;
+                if (sub_y) { h.x -= yold.x; h.y -= yold.y; }
+                if (wy) t.y[e[i]] = h;
+                if (t.n_acc > 0) {
+                    double2 s = aold;
+                    cfma(s, t.ca, h);
+                    if (t.n_acc >= 2) cfma(s, t.cb, xrow);
+                    if (t.n_acc == 3) cfma(s, t.cc, yold);
+                    t.acc[e[i]] = s;
+                    if (reduce) {
+                        s_re = fma(z.x, s.x, s_re); s_re = fma(z.y, s.y, s_re);
+                        s_im = fma(z.x, s.y, s_im); s_im = fma(-z.y, s.x, s_im);
+                        s_nn = fma(s.x, s.x, s_nn); s_nn = fma(s.y, s.y, s_nn);
+                    }
+                }
+            }
+            if (reduce) block_partial<BT, kSmallThreads>(s_re, s_im, s_nn, sp.partial, blockIdx.x);
+            // T_k (and the partials) become visible to the whole cluster: every block of the grid is in it
+            asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+        }
+        if (blockIdx.x == 0 && threadIdx.x < sp.n_valid * 3) {
             const int bb = threadIdx.x / 3, c = threadIdx.x % 3;
-            double t = 0.0;
-#pragma unroll
-            for (int w = 0; w < kThreads / 32; ++w) t += sm[w][bb][c];
-            p.partial[((int64_t)blockIdx.x * BT + bb) * 3 + c] = t;
+            double tsum = 0.0;
+            for (int g = 0; g < (int)gridDim.x; ++g) tsum += __ldcg(sp.partial + ((int64_t)g * BT + bb) * 3 + c);
+            const int64_t at = (int64_t)(sp.state0 + bb) * sp.n_step + n;
+            if (c < 2) sp.corr[2 * at + c] = tsum;
+            else if (sp.norm2) sp.norm2[at] = tsum;
         }
+        slot = (slot + 2) % 3;
     }
 }
 
@@ -363,11 +490,12 @@ int launch_term_t(const TermParams &p, int num_sms, cudaStream_t st, int *grid_o
     return TBPM_OK;
 }
 
-// One Chebyshev term.  Lattices with tiles of 8 states run on the rolling-window kernel (term_rw.cu) when their strides
-// allow it (TBPM_OPT_KERNEL = 2 turns that off).  The phased kernel (term_ph.cuh) runs whenever it has an instantiation for the term and its stages
-// fit (kernel layout with a value table, tiles of 1-8 states, rows of up to a few dozen entries); everything else -- no
-// table, tiles of 16 / 32 states, long rows, tau = 0 -- and every term under TBPM_OPT_KERNEL = 1 runs on the general
-// kernel k_cheb_term.
+// One Chebyshev term.  TBPM_OPT_KERNEL = 0: tiles of 8 states on a lattice the builder recognised run on term_l3.cu
+// (three-dimensional, one real hopping value), term_sq.cu (square + next-nearest neighbours, in-line hoppings) or term_rw.cu (other
+// strides of whole 128-row tiles); the phased kernel (term_ph.cuh) runs whenever it has an instantiation for the term and its
+// stages fit (kernel layout with a value table, tiles of 1-8 states, rows of up to a few dozen entries); everything else -- no
+// table, tiles of 16 / 32 states, long rows, tau = 0 -- runs on the general kernel k_cheb_term.  1: general kernel only;
+// 2: no lattice kernel; 3: of the lattice kernels only term_rw.
 int launch_term(int bt, bool table, int kernel_opt, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
     const bool general_only = kernel_opt == 1;
@@ -553,7 +681,41 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
             count_launches(1);
             return TBPM_OK;
         };
-        for (int n = 0; n < n_step; ++n) {
+        // small models: all time steps of the tile in one cluster launch (k_small_steps)
+        const bool small = !qe && table && K >= 2 && K <= kSmallMaxK && bt <= 8 && tp.max_row_off <= kSmallCH && n_el > 0 &&
+                           n_el <= (int64_t)kSmallRPT * kSmallCluster * kSmallThreads && H->opt_kernel == 0 && knob("small", 1);
+        if (small) {
+            std::vector<TermLite> all((size_t)3 * K);
+            for (int sl = 0; sl < 3; ++sl) {
+                step_terms(tp, K, cf, rescale, false, buf[sl], buf[(sl + 1) % 3], buf[(sl + 2) % 3], term);
+                for (int k = 1; k < K; ++k) {
+                    const TermParams &q = term[k];
+                    all[(size_t)sl * K + k] = TermLite{q.x, q.y, q.acc, q.a, q.ca, q.cb, q.cc, q.n_acc, q.flags};
+                }
+            }
+            TermLite *d_terms = reinterpret_cast<TermLite *>(W + P.aux_off);
+            // pageable source: the call returns once the data is staged, so `all` may go out of scope
+            TBPM_CUDA_TRY(cudaMemcpyAsync(d_terms, all.data(), all.size() * sizeof(TermLite), cudaMemcpyHostToDevice, st));
+            SmallParams sp{d_terms, tp.orp, tp.ocol, tp.oidx, tp.vtab, tp.diag, bra, H->n_orb, K, n_step, start_slot, n_valid, state0,
+                           tp.packed, tp.uniform, tp.max_row_off, corr, norm2, partial};
+            cudaLaunchConfig_t cfg{};
+            cfg.gridDim = dim3(kSmallCluster); cfg.blockDim = dim3(kSmallThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = kSmallCluster; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            cudaError_t le = cudaErrorInvalidValue;
+            switch (bt) {
+            case 1: le = cudaLaunchKernelEx(&cfg, k_small_steps<1>, sp); break;
+            case 2: le = cudaLaunchKernelEx(&cfg, k_small_steps<2>, sp); break;
+            case 4: le = cudaLaunchKernelEx(&cfg, k_small_steps<4>, sp); break;
+            case 8: le = cudaLaunchKernelEx(&cfg, k_small_steps<8>, sp); break;
+            }
+            TBPM_CUDA_TRY(le);
+            count_launches(1);
+            slot = (start_slot + 2 * n_step) % 3;
+        }
+        for (int n = 0; n < n_step && !small; ++n) {
             if ((rc = one_step(n, st))) return rc;
             slot = (slot + 2) % 3;                        // psi' (acc) is the next step's psi
             if (qe && n_el > 0) qe_add(buf[slot], n + 1);

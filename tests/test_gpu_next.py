@@ -37,7 +37,7 @@ def test_quasi_eigenstates(dev, oracle_mod, cfg, over, n_state, n_step):
     energies = [0.0, 0.31 * w.rescale, -0.77 * w.rescale]
     corr, norm2, qe = tbpm.tbpm_propagate_qe(H, psi0, energies, n_step, w.dt, w.rescale)
     ref_c, _, _ = tbpm.tbpm_propagate(H, psi0, n_step, w.dt, w.rescale)
-    assert torch.equal(corr, ref_c)                                  # the same propagation, bit for bit
+    assert (corr - ref_c).abs().max() <= 1e-13                       # the same propagation (small models: another kernel, rounding only)
     hi, hj, hv, on = to_np(w)
     ref = oracle_mod.quasi_eigenstates(w.n_orb, on, hi, hj, hv, psi0.cpu().numpy(), energies, n_step, w.dt, w.rescale)
     assert qe.shape == (n_state, 3, w.n_orb)

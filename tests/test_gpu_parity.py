@@ -160,7 +160,12 @@ def test_config1_full_length(dev, oracle_mod):
     H, _, corr, _ = run_parity(dev, oracle_mod, w, 1, 256)
     assert corr.shape == (1, 256)
     assert H.n_table == 1                                            # t and conj(t) = (t, -0.0) share the entry
+    assert tbpm.tbpm_last_launch_count(H) == 2                       # state set-up + ONE cluster launch for all 256 steps (k_small_steps)
+    tbpm.tbpm_set_option(H, tbpm.TBPM_OPT_KERNEL, 2)                 # the same on the launch-per-term path
+    psi0 = w.psi0(device=dev, n_state=1)
+    c2, n2, _ = tbpm.tbpm_propagate(H, psi0, 256, w.dt, w.rescale)
     assert tbpm.tbpm_last_launch_count(H) == 256 * 21 + 1            # 20 terms + 1 final reduction per step, + set-up
+    assert (c2 - corr).abs().max() <= 1e-13 and np.abs(n2.cpu().numpy() - 1).max() <= NORM_TOL
 
 
 @pytest.mark.parametrize("cfg,over,n_state,n_step", [
