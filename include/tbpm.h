@@ -197,6 +197,15 @@ int tbpm_corr_ac(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const double *psi0 /* 
                  double dt, double rescale, double beta, double mu, double *corr /* device out */, void *workspace,
                  size_t workspace_bytes, void *stream);
 
+/* Dynamic-polarisation correlation ("dynamic polarizability (DP)"; Table 7; no formula printed).
+ * DESIGN.md reading #31: the scheme of tbpm_corr_ac with DIAGONAL density operators rho(q) = diag(exp(i q.r_i)) in place of the
+ * current operators: psi1(0) = [1 - f(H)] (rho_b * psi0), psi2(0) = f(H) psi0, corr[b][n] = <psi2(n dt)| rho_a * psi1(n dt)>,
+ * n = 0 .. n_step.  rho_a, rho_b: device [n_orb][2] (the caller passes rho_b = rho(-q), rho_a = rho(q)).  Workspace and output
+ * as for tbpm_corr_ac. */
+int tbpm_corr_dp(tbpm_ham *H, const double *rho_a /* device */, const double *rho_b /* device */, const double *psi0 /* device */, int n_state,
+                 int n_step, double dt, double rescale, double beta, double mu, double *corr /* device out */, void *workspace,
+                 size_t workspace_bytes, void *stream);
+
 /* ---- end to end with HOST buffers ------------------------------------------------------------------------------------
  * Whole path for host-resident inputs: H2D of the list and psi0, tbpm_build, tbpm_propagate, D2H of corr/norm2, then a
  * stream synchronise.  `arena` is caller-owned device memory of at least tbpm_corr_host_bytes(); host buffers should be

@@ -304,3 +304,27 @@ def corr_ac(n_orb, onsite, hop_i, hop_j, hop_val, ja_hops, jb_hops, psi0, n_step
                 p2 = fin[0]
             out[b, n] = np.vdot(p2, apply_h(n_orb, None, *ja_hops, p1))
     return out
+
+
+def corr_dp(n_orb, onsite, hop_i, hop_j, hop_val, rho_a, rho_b, psi0, n_step, dt, rescale, beta, mu):
+    """Dynamic-polarisation correlation of TBPM ("dynamic polarizability (DP)", Table 7; no formula
+    printed).  DESIGN.md reading #31: the scheme of corr_ac with the DIAGONAL density operators rho(q) = diag(exp(i q.r_i)) in place
+    of the current operators -- rho_a, rho_b are complex128 [n_orb] (the caller passes rho_b = rho(-q), rho_a = rho(q)):
+
+        psi1(0) = [1 - f(H)] (rho_b * psi0),   psi2(0) = f(H) psi0,   corr[b][n] = < psi2(n dt) | rho_a * psi1(n dt) >,  n = 0 .. n_step."""
+    psi0 = np.atleast_2d(_c128(psi0))
+    ra, rb = _c128(rho_a), _c128(rho_b)
+    cf = fermi_cheb_coeff(beta, mu, rescale)
+    cg = fermi_cheb_coeff(beta, mu, rescale, one_minus=True)
+    out = np.zeros((psi0.shape[0], n_step + 1), dtype=np.complex128)
+    for b in range(psi0.shape[0]):
+        p1 = apply_cheb_series(n_orb, onsite, hop_i, hop_j, hop_val, cg, rescale, rb * psi0[b])
+        p2 = apply_cheb_series(n_orb, onsite, hop_i, hop_j, hop_val, cf, rescale, psi0[b])
+        for n in range(n_step + 1):
+            if n > 0:
+                _, _, fin = propagate(n_orb, onsite, hop_i, hop_j, hop_val, p1, 1, dt, rescale, psi_start=p1, return_state=True)
+                p1 = fin[0]
+                _, _, fin = propagate(n_orb, onsite, hop_i, hop_j, hop_val, p2, 1, dt, rescale, psi_start=p2, return_state=True)
+                p2 = fin[0]
+            out[b, n] = np.vdot(p2, ra * p1)
+    return out

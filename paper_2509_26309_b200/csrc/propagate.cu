@@ -292,6 +292,29 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_small_steps(const SmallPar
     }
 }
 
+// NEXT-4, dynamic polarisation: a DIAGONAL complex operator d (the density operator exp(i q.r)) on one tile of interleaved states.
+__global__ void k_diag_apply(const double2 *__restrict__ d, const double2 *__restrict__ x, double2 *y, int64_t n_orb, int bt)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_orb * bt; i += (int64_t)gridDim.x * blockDim.x) {
+        const double2 dv = d[i / bt], xv = x[i];
+        y[i] = make_double2(dv.x * xv.x - dv.y * xv.y, dv.x * xv.y + dv.y * xv.x);
+    }
+}
+// block partials of <bra| d |x> per state, in the layout k_reduce_final reads ([block][bt][3]; the third component is unused)
+template <int BT>
+__global__ void __launch_bounds__(256) k_diag_dot(const double2 *__restrict__ d, const double2 *__restrict__ x, const double2 *__restrict__ bra,
+                                                  int64_t n_orb, double *partial)
+{
+    double s_re = 0.0, s_im = 0.0, s_nn = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_orb * BT; i += (int64_t)gridDim.x * blockDim.x) {   // stride % BT == 0
+        const double2 dv = d[i / BT], xv = x[i], z = bra[i];
+        const double2 w = make_double2(dv.x * xv.x - dv.y * xv.y, dv.x * xv.y + dv.y * xv.x);
+        s_re = fma(z.x, w.x, s_re); s_re = fma(z.y, w.y, s_re);
+        s_im = fma(z.x, w.y, s_im); s_im = fma(-z.y, w.x, s_im);
+    }
+    block_partial<BT, 256>(s_re, s_im, s_nn, partial, blockIdx.x);
+}
+
 // Sum the block partials in a fixed order: block = state, warp = component, lanes stride over the partials.
 __global__ void k_reduce_final(const double *__restrict__ partial, int n_blocks, int bt, int n_valid, int state0, int n_step, int step,
                                double *corr, double *norm2)
@@ -852,9 +875,13 @@ extern "C" int tbpm_corr_ac_bytes(const tbpm_ham *H, int n_state, size_t *worksp
     return TBPM_OK;
 }
 
-extern "C" int tbpm_corr_ac(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const double *psi0, int n_state, int n_step, double dt, double rescale,
-                            double beta, double mu, double *corr, void *workspace, size_t workspace_bytes, void *stream)
+namespace {
+// The two operators are either matrices (Ja, Jb: current operators) or diagonals (da, db: density operators, device [n_orb][2]).
+int corr_pair(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const double2 *da, const double2 *db, const double *psi0, int n_state, int n_step,
+              double dt, double rescale, double beta, double mu, double *corr, void *workspace, size_t workspace_bytes, void *stream)
 {
+    const bool diag_op = da != nullptr;
+    if (diag_op) { Ja = H; Jb = H; }                     // placeholders: the matrix launches below are not used
     if (!H || !Ja || !Jb || n_state < 0 || n_step < 0 || !(rescale > 0.0) || !(dt >= 0.0) || !std::isfinite(dt) || !std::isfinite(rescale))
         return TBPM_EINVAL;
     if (Ja->n_orb != H->n_orb || Jb->n_orb != H->n_orb || Ja->device != H->device || Jb->device != H->device) return TBPM_EINVAL;
@@ -909,7 +936,21 @@ extern "C" int tbpm_corr_ac(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const doubl
             return (slot + 2) % 3;
         };
         // corr[.][n] = <psi2|J_a psi1>: J_a psi1 goes to a free buffer of set A
+        const int dgrid = (int)std::min<int64_t>((n_el + 255) / 256, (int64_t)H->num_sms * 8);
         auto cross = [&](int sa, int sb, int n) {
+            if (diag_op) {
+                switch (bt) {
+                case 1: k_diag_dot<1><<<dgrid, 256, 0, st>>>(da, A[sa], B[sb], H->n_orb, partial); break;
+                case 2: k_diag_dot<2><<<dgrid, 256, 0, st>>>(da, A[sa], B[sb], H->n_orb, partial); break;
+                case 4: k_diag_dot<4><<<dgrid, 256, 0, st>>>(da, A[sa], B[sb], H->n_orb, partial); break;
+                case 8: k_diag_dot<8><<<dgrid, 256, 0, st>>>(da, A[sa], B[sb], H->n_orb, partial); break;
+                case 16: k_diag_dot<16><<<dgrid, 256, 0, st>>>(da, A[sa], B[sb], H->n_orb, partial); break;
+                default: k_diag_dot<32><<<dgrid, 256, 0, st>>>(da, A[sa], B[sb], H->n_orb, partial); break;
+                }
+                k_reduce_final<<<bt, 96, 0, st>>>(partial, dgrid, bt, n_valid, state0, n_out, n, corr, nullptr);
+                count_launches(2);
+                return;
+            }
             TermParams tp = ma;
             tp.x = A[sa]; tp.psi0 = B[sb]; tp.acc = A[(sa + 1) % 3]; tp.y = A[(sa + 2) % 3];
             tp.a = 1.0; tp.ca = make_double2(1.0, 0.0); tp.n_acc = 1; tp.flags = F_ACC_INIT | F_REDUCE;
@@ -918,7 +959,10 @@ extern "C" int tbpm_corr_ac(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const doubl
             count_launches(1);
         };
         rc = TBPM_OK;
-        {   // A[1] = J_b psi0 (first-term shape: y = a J x)
+        if (diag_op) {                                    // A[1] = d_b psi0
+            k_diag_apply<<<dgrid, 256, 0, st>>>(db, A[0], A[1], H->n_orb, bt);
+            count_launches(1);
+        } else {                                          // A[1] = J_b psi0 (first-term shape: y = a J x)
             TermParams tp = mb;
             tp.x = A[0]; tp.y = A[1]; tp.acc = A[2]; tp.psi0 = A[0];
             tp.a = 1.0; tp.n_acc = 0; tp.flags = F_WRITE_Y;
@@ -940,6 +984,22 @@ extern "C" int tbpm_corr_ac(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const doubl
     TBPM_CUDA_TRY(cudaGetLastError());
     H->last_launches = total_launches() - launches0;
     return TBPM_OK;
+}
+}  // namespace
+
+extern "C" int tbpm_corr_ac(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const double *psi0, int n_state, int n_step, double dt, double rescale,
+                            double beta, double mu, double *corr, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!Ja || !Jb) return TBPM_EINVAL;
+    return corr_pair(H, Ja, Jb, nullptr, nullptr, psi0, n_state, n_step, dt, rescale, beta, mu, corr, workspace, workspace_bytes, stream);
+}
+
+extern "C" int tbpm_corr_dp(tbpm_ham *H, const double *rho_a, const double *rho_b, const double *psi0, int n_state, int n_step, double dt,
+                            double rescale, double beta, double mu, double *corr, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!rho_a || !rho_b || (reinterpret_cast<uintptr_t>(rho_a) & 15u) || (reinterpret_cast<uintptr_t>(rho_b) & 15u)) return TBPM_EINVAL;
+    return corr_pair(H, nullptr, nullptr, reinterpret_cast<const double2 *>(rho_a), reinterpret_cast<const double2 *>(rho_b), psi0, n_state, n_step,
+                     dt, rescale, beta, mu, corr, workspace, workspace_bytes, stream);
 }
 
 extern "C" int tbpm_get_state(const tbpm_ham *H, const void *workspace, int state, double *psi_out, void *stream)

@@ -60,6 +60,7 @@ def lib() -> C.CDLL:
         L.tbpm_fermi_coeff.argtypes = [dbl, dbl, dbl, C.c_int, dbl, C.c_int, P(C.c_int), vp]
         L.tbpm_corr_ac_bytes.argtypes = [vp, C.c_int, P(sz)]
         L.tbpm_corr_ac.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, dbl, dbl, dbl, dbl, vp, vp, sz, vp]
+        L.tbpm_corr_dp.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, dbl, dbl, dbl, dbl, vp, vp, sz, vp]
         L.tbpm_last_launch_count.restype = i64
         L.tbpm_last_launch_count.argtypes = [vp]
         L.tbpm_set_option.argtypes = [vp, C.c_int, i64]
@@ -187,7 +188,7 @@ def tbpm_propagate(H: Hamiltonian, psi0: torch.Tensor, n_step: int, dt: float, r
     _need_cuda(psi0)
     dev = H.device
     assert psi0.dtype == torch.complex128 and psi0.dim() == 2 and psi0.shape[1] == H.n_orb
-    psi0 = psi0.contiguous()
+    psi0 = psi0.resolve_conj().contiguous()
     n_state = psi0.shape[0]
     wb = tbpm_propagate_bytes(H, n_state)
     if workspace is None:
@@ -281,6 +282,26 @@ def tbpm_corr_ac(H: Hamiltonian, Ja: Hamiltonian, Jb: Hamiltonian, psi0: torch.T
         rc = lib().tbpm_corr_ac(H.handle, Ja.handle, Jb.handle, _ptr(psi0), n_state, n_step, dt, rescale, beta, mu, _ptr(corr), _ptr(ws),
                                 ws.numel(), _stream(dev))
     _check(rc, "tbpm_corr_ac")
+    return corr
+
+
+def tbpm_corr_dp(H: Hamiltonian, rho_a: torch.Tensor, rho_b: torch.Tensor, psi0: torch.Tensor, n_step: int, dt: float, rescale: float,
+                 beta: float, mu: float) -> torch.Tensor:
+    """NEXT-4: corr complex128 [n_state][n_step + 1], entry n = <psi2(n dt)| rho_a * psi1(n dt)>; rho_a, rho_b complex128 [n_orb] on the device."""
+    _need_cuda(psi0, rho_a, rho_b)
+    dev = H.device
+    # torch's conj() is lazy: resolve it, the library reads the raw (re, im) pairs
+    psi0, rho_a, rho_b = psi0.resolve_conj().contiguous(), rho_a.resolve_conj().contiguous(), rho_b.resolve_conj().contiguous()
+    assert rho_a.dtype == torch.complex128 and rho_a.numel() == H.n_orb and rho_b.numel() == H.n_orb
+    n_state = psi0.shape[0]
+    wb = C.c_size_t(0)
+    _check(lib().tbpm_corr_ac_bytes(H.handle, n_state, C.byref(wb)), "tbpm_corr_ac_bytes")
+    ws = _bytes(wb.value, dev)
+    corr = torch.zeros((n_state, n_step + 1), dtype=torch.complex128, device=dev)
+    with torch.cuda.device(dev):
+        rc = lib().tbpm_corr_dp(H.handle, _ptr(rho_a), _ptr(rho_b), _ptr(psi0), n_state, n_step, dt, rescale, beta, mu, _ptr(corr), _ptr(ws),
+                                ws.numel(), _stream(dev))
+    _check(rc, "tbpm_corr_dp")
     return corr
 
 

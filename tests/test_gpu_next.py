@@ -138,3 +138,20 @@ def test_corr_ac(dev, oracle_mod, Lx, Ly, phi_den, n_state, n_step, beta, mu, ax
     assert np.abs(corr.cpu().numpy() - ref).max() <= 1e-10 * max(1.0, np.abs(ref).max())
     again = tbpm.tbpm_corr_ac(H, J[0], J[1], psi0, n_step, w.dt, w.rescale, beta, mu)
     assert torch.equal(corr, again)                                  # deterministic
+
+
+@pytest.mark.parametrize("L,n_state,n_step,beta,mu", [(32, 8, 5, 0.4, 1.0), (12, 3, 7, 1.5, -2.0)])
+def test_corr_dp(dev, oracle_mod, L, n_state, n_step, beta, mu):
+    """NEXT-4, dynamic polarisation: <psi2(t)| rho(q) |psi1(t)> with psi1 = [1 - f(H)] rho(-q) psi0 on the disordered cubic lattice
+    (L = 32: H runs on the three-dimensional lattice kernel), every entry against the oracle."""
+    w = W.make_workload(5, device=dev, L=L)
+    psi0 = w.psi0(device=dev, n_state=n_state)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    idx = torch.arange(w.n_orb, device=dev)
+    ph = (2 * math.pi / L) * (1.0 * (idx % L) + 2.0 * (idx // (L * L))).to(torch.float64)
+    rho = torch.complex(torch.cos(ph), torch.sin(ph))
+    corr = tbpm.tbpm_corr_dp(H, rho, rho.conj().contiguous(), psi0, n_step, w.dt, w.rescale, beta, mu)
+    hi, hj, hv, on = to_np(w)
+    ref = oracle_mod.corr_dp(w.n_orb, on, hi, hj, hv, rho.cpu().numpy(), rho.conj().cpu().numpy(), psi0.cpu().numpy(), n_step, w.dt,
+                             w.rescale, beta, mu)
+    assert np.abs(corr.cpu().numpy() - ref).max() <= 1e-10 * max(1.0, np.abs(ref).max())

@@ -190,3 +190,30 @@ def test_corr_ac_exact_diagonalisation(oracle_mod, beta, mu):
     # a full band (mu far above the spectrum): 1 - f = 0, nothing to excite
     z = oracle_mod.corr_ac(w.n_orb, on, hi, hj, hv, ja, jb, psi0[:1], 2, w.dt, s, 40.0, 3 * s)
     assert np.abs(z).max() < 1e-10
+
+
+def test_corr_dp_exact_diagonalisation(oracle_mod):
+    """corr_n = psi0^+ f(H) e^{+iHt} rho(q) e^{-iHt} (1 - f(H)) rho(-q) psi0 by full diagonalisation on the cubic lattice with
+    disorder (N = 216); q = 0 makes rho the identity: corr_n = psi0^+ f (1 - f) psi0, constant in time."""
+    w = W.make_workload(5, L=6)
+    hi, hj, hv, on = np_hops(w)
+    psi0 = w.psi0(n_state=2).numpy()
+    idx = np.arange(w.n_orb)
+    r = np.stack([idx % 6, (idx // 6) % 6, idx // 36], axis=1).astype(np.float64)
+    q = 2 * np.pi / 6 * np.array([1.0, 0.0, 2.0])
+    rho = np.exp(1j * (r @ q))
+    beta, mu, n_step = 0.4, 1.0, 9
+    corr = oracle_mod.corr_dp(w.n_orb, on, hi, hj, hv, rho, rho.conj(), psi0, n_step, w.dt, w.rescale, beta, mu)
+    H = dense_h(w.n_orb, hi, hj, hv, on)
+    E, V = np.linalg.eigh(H)
+    f = 1.0 / (np.exp(beta * (E - mu)) + 1.0)
+    for b in range(2):
+        p1 = V @ ((1 - f) * (V.conj().T @ (rho.conj() * psi0[b])))
+        p2 = V @ (f * (V.conj().T @ psi0[b]))
+        for n in range(n_step + 1):
+            U = (V * np.exp(-1j * E * n * w.dt)) @ V.conj().T
+            assert abs(corr[b, n] - np.vdot(U @ p2, rho * (U @ p1))) < 1e-11
+    one = np.ones(w.n_orb, dtype=np.complex128)
+    c0 = oracle_mod.corr_dp(w.n_orb, on, hi, hj, hv, one, one, psi0[:1], 4, w.dt, w.rescale, beta, mu)
+    cj = V.conj().T @ psi0[0]
+    assert np.abs(c0[0] - np.sum(np.abs(cj) ** 2 * f * (1 - f))).max() < 1e-11
