@@ -207,6 +207,43 @@ def test_lattice_kernels_agree_with_oracle(dev, oracle_mod, cfg, over, n_state, 
     run_parity(dev, oracle_mod, w, n_state, n_step, options={tbpm.TBPM_OPT_KERNEL: kernel})
 
 
+def test_lattice_kernels_rows_off_the_lattice(dev, oracle_mod):
+    """Matrices that only RESEMBLE a lattice.  (i) Cubic 32^3 with two bonds rewired (a-b, c-d -> a-d, c-b): every row still has six
+    entries, four rows are off the lattice -- term_l3 keeps running and gathers the warps that hold them entry by entry through
+    ocol.  (ii) Square lattice with flux where ONE hopping value is changed: the per-line table no longer describes every row, the
+    builder must not certify it (lattice kind 0) and the rolling-window kernel takes over."""
+    w = W.make_workload(5, device=dev, L=32)
+    hi, hj = w.hop_i.clone(), w.hop_j.clone()
+    h1, h2 = 12345, 54321 + 32768                                    # an x-bond and a y-bond far apart
+    hj[h1], hj[h2] = w.hop_j[h2], w.hop_j[h1]
+    w.hop_i, w.hop_j = hi, hj
+    H, _, _, _ = run_parity(dev, oracle_mod, w, 8, 5)
+    assert H.lattice_kind == tbpm.TBPM_LATTICE_CUBIC
+    w = W.make_workload(4, device=dev, Lx=128, Ly=24, phi_den=32)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    assert H.lattice_kind == tbpm.TBPM_LATTICE_SQUARE8
+    w.hop_val = w.hop_val.clone()
+    w.hop_val[777] = w.hop_val[777] * 0.5
+    H, _, _, _ = run_parity(dev, oracle_mod, w, 8, 5)
+    assert H.lattice_kind == 0
+
+
+def test_anisotropic_box_lattice(dev, oracle_mod):
+    """A 64 x 8 x 12 box (line of 64 rows = two tiles, plane of 8 lines = two tile rows, 12 planes: runs shorter than 64) with
+    Anderson disorder: the three-dimensional lattice kernel away from the cube, 16 states = two tiles."""
+    Lx, Ly, Lz = 64, 8, 12
+    z = torch.arange(Lz, device=dev).view(Lz, 1, 1); y = torch.arange(Ly, device=dev).view(1, Ly, 1); x = torch.arange(Lx, device=dev).view(1, 1, Lx)
+    idx = lambda zz, yy, xx: ((zz * Ly + yy) * Lx + xx).expand(Lz, Ly, Lx).reshape(-1)
+    src = idx(z, y, x)
+    hop_i = torch.cat([src, src, src]).to(torch.int32)
+    hop_j = torch.cat([idx(z, y, (x + 1) % Lx), idx(z, (y + 1) % Ly, x), idx((z + 1) % Lz, y, x)]).to(torch.int32)
+    n = Lx * Ly * Lz
+    w = W.Workload("box", n, hop_i, hop_j, torch.full((3 * n,), -1.0, dtype=torch.complex128, device=dev),
+                   W.anderson_onsite(n, 4.0, device=dev), 16, 6, 8.5)
+    H, _, _, _ = run_parity(dev, oracle_mod, w, 16, 6)
+    assert H.lattice_kind == tbpm.TBPM_LATTICE_CUBIC
+
+
 def test_square_nn_lattice_rolling_window(dev, oracle_mod):
     """4 entries per row (t' = 0): the third instantiated shape of term_rw, with one real hopping value and with phases."""
     n, hi, hj, hv = W.square_peierls_hops(128, 20, -1.0, 0.0, 1, 32, dev)
