@@ -261,6 +261,25 @@ def test_row_form_matches_hop_form(oracle_mod, cfg, over):
     assert np.abs(a[2] - b[2]).max() < 1e-13
 
 
+@pytest.mark.parametrize("cfg,over,tau", [(1, dict(Na=16, Nb=16), math.pi), (4, dict(Lx=16, Ly=16, phi_den=16), 2 * math.pi), (5, dict(L=8), 0.7)])
+def test_row_form_exact_diagonalisation_and_window(oracle_mod, cfg, over, tau):
+    """The row form (the one the full-size parity checks and the cpu_baseline use) pinned DIRECTLY, not only through the hop form:
+    exact diagonalisation over 128 steps at three values of tau (other K, other flush patterns), and the windowed restart
+    (psi_start) reproduces the tail of a longer run."""
+    w = W.make_workload(cfg, **over)
+    hi, hj, hv, on = np_hops(w)
+    psi0 = w.psi0(n_state=2).numpy()
+    H = dense_h(w.n_orb, hi, hj, hv, on)
+    dt = tau / w.rescale
+    corr, norm2, fin = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0, 128, dt, w.rescale, form="csr", return_state=True)
+    for b in range(2):
+        assert np.abs(corr[b] - exact_corr(H, psi0[b], 128, tau, w.rescale)).max() < 1e-12
+    assert np.abs(norm2 - 1).max() < 1e-12
+    head, _, mid = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0, 100, dt, w.rescale, form="csr", return_state=True)
+    tail, _ = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0, 28, dt, w.rescale, form="csr", psi_start=mid)
+    assert np.abs(np.concatenate([head, tail], axis=1) - corr).max() < 1e-13
+
+
 # ---- pin 27: closed-form DOS (band edges +-3|t|, van Hove peaks at +-|t|, chain 1/(pi sqrt(4t^2-E^2))) ---------
 def test_dos_honeycomb_features(oracle_mod):
     w = W.make_workload(1, Na=96, Nb=96, n_step=512)
