@@ -49,7 +49,6 @@ struct Geom {
     int slot_shift[kMaxSlot];   // row shift inside the ring slot, in [-kHalo, kHalo]
     int lat;                    // which Lat<> the (src, shift) pattern is, -1: none
     int far_na;                 // far neighbours loaded without L1 allocation
-    int use_flags;              // regular rows are known from the builder's lattice bits: their column words are not read
     int off_y, off_col, off_idx, off_diag, stage_bytes;
 };
 
@@ -188,9 +187,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_rw(const TermParams p, con
                     mbar_wait(b_sempty + 8 * s, sph);
                     const uint32_t full = b_sfull + 8 * s;
                     const uint32_t st = stage0 + (uint32_t)s * (uint32_t)g.stage_bytes;
-                    uint32_t tx = 0;
+                    uint32_t tx = kR * CH * 4;
                     if (need_y) { bulk_g2s(st + g.off_y, p.y + r0 * kBT, kR * kRowBytes, full); tx += kR * kRowBytes; }
-                    if (!g.use_flags) { bulk_g2s(st + g.off_col, p.ocol + r0 * CH, kR * CH * 4, full); tx += kR * CH * 4; }
+                    bulk_g2s(st + g.off_col, p.ocol + r0 * CH, kR * CH * 4, full);
                     if (VK == 0) { bulk_g2s(st + g.off_idx, p.oidx + r0 * CH, kR * CH * 2, full); tx += kR * CH * 2; }
                     if (has_diag) { bulk_g2s(st + g.off_diag, p.diag + r0, kR * 8, full); tx += kR * 8; }
                     mbar_expect_tx(full, tx);
@@ -238,22 +237,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_rw(const TermParams p, con
         const int64_t lb = blockIdx.x / g.d0, pos = blockIdx.x - lb * g.d0;
         far_request(lb * g.len * g.W + pos * kR + rl);
     }
-    // lattice bits of the row (one word per 32 rows), fetched one tile ahead
-    const bool use_flags = g.use_flags != 0;
-    uint32_t fw = 0;
-    if (use_flags && (int64_t)blockIdx.x < n_runs) {
-        const int64_t lb = blockIdx.x / g.d0, pos = blockIdx.x - lb * g.d0;
-        fw = __ldg(p.lat_flags + ((lb * g.len * g.W + pos * kR + rl) >> 5));
-    }
 #pragma unroll 1
     for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
         const int64_t lb = u / g.d0, pos = u - lb * g.d0;
         const int64_t line0 = lb * g.len;
         const int len_u = (int)min((int64_t)g.len, g.n_lines - line0);
         int64_t row = line0 * g.W + pos * kR + rl;
-        // first row of the next run of this block (for the far request / the lattice bits of this run's last tile)
+        // first row of the next run of this block (for the far request of this run's last tile)
         int64_t next_run_row = -1;
-        if ((NG > 0 || use_flags) && u + gridDim.x < n_runs) {
+        if (NG > 0 && u + gridDim.x < n_runs) {
             const int64_t u2 = u + gridDim.x, lb2 = u2 / g.d0, pos2 = u2 - lb2 * g.d0;
             next_run_row = lb2 * g.len * g.W + pos2 * kR + rl;
         }
@@ -264,11 +256,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_rw(const TermParams p, con
             CVec<2> aold, z;
             if (NACC > 0) aold.stream_if(p.acc + e, need_acc);
             if (REDUCE) z.stream_if(p.psi0 + e, true);
-            const bool bit = (fw >> ((uint32_t)row & 31u)) & 1u;
-            if (use_flags) {
-                const int64_t nrow = j + 1 < len_u ? row + g.W : next_run_row;
-                if (nrow >= 0) fw = __ldg(p.lat_flags + (nrow >> 5));
-            }
             // ---- wait: the ring slots of this tile (the first tile of a run waits for all three), then the stage
             if (j == 0) {
                 mbar_wait(b_rfull + 8 * r0p.i, r0p.ph);
@@ -282,22 +269,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_term_rw(const TermParams p, con
             const uint32_t ia = st + g.off_idx + (uint32_t)rl * (CH * 2u);
 #pragma unroll
             for (int jj = 0; jj < CH; jj += 2) {
-                if (!use_flags) lds_v2_u32(ca + 4u * jj, w[jj], w[jj + 1]); else w[jj] = w[jj + 1] = 0u;
+                lds_v2_u32(ca + 4u * jj, w[jj], w[jj + 1]);
                 if (VK == 0) { const uint32_t t = lds_u32(ia + 2u * jj); id[jj] = t & 0xffffu; id[jj + 1] = t >> 16; }
                 else id[jj] = id[jj + 1] = 0u;
             }
             const int row32 = (int)row;
-            bool ok = bit;
-            if (!use_flags) {
-                ok = true;
+            bool ok = true;
 #pragma unroll
-                for (int jj = 0; jj < CH; ++jj) ok = ok && ((int)(w[jj] & 0x7fffffffu) == row32 + g.slot_delta[jj]);
-            }
+            for (int jj = 0; jj < CH; ++jj) ok = ok && ((int)(w[jj] & 0x7fffffffu) == row32 + g.slot_delta[jj]);
             const bool fast = __all_sync(0xffffffffu, ok);
-            if (use_flags && !fast) {                       // a warp with a row off the lattice: its column words, from global memory
-#pragma unroll
-                for (int jj = 0; jj < CH; ++jj) w[jj] = (uint32_t)__ldg(p.ocol + row * CH + jj);
-            }
             const uint32_t bp = ring0 + r0p.i * kSlotBytes + row_off, bo = ring0 + r1p.i * kSlotBytes + row_off,
                            bn = ring0 + r2p.i * kSlotBytes + row_off;
             double2 ha = make_double2(0.0, 0.0), hb = ha;   // slots a / b
@@ -504,7 +484,6 @@ bool make_geom(const TermParams &p, Geom &g)
     g.off_diag = (int)o; o += (size_t)kR * 8;
     g.stage_bytes = (int)((o + 127) & ~size_t(127));
     g.far_na = knob("rw_far_na", 1);
-    g.use_flags = p.lat_flags != nullptr && !p.lat_periodic3 && knob("rw_flags", 0);
     g.n_ring = std::min(kMaxRing, std::max(4, knob("rw_ring", 5)));
     g.n_stage = std::min(kMaxStages, std::max(2, knob("rw_stages", 4)));
     while ((size_t)g.n_ring * kSlotBytes + (size_t)g.n_stage * g.stage_bytes > kSmemMax - 4096) {
