@@ -182,93 +182,117 @@ __global__ void __launch_bounds__(kThreads, MINB) k_cheb_term(const TermParams p
 // ---------------------------------------------------------------------------------------------------------------------
 // Small models (cfg1: 8,192 orbitals, one state) are launch-bound on the path above: 21 launches of ~3 us of device work each per
 // time step.  k_small_steps runs ALL time steps of a tile in ONE launch of one thread-block cluster (8 blocks x 1024 threads on 8
-// SMs; the vectors of such a model live in L2).  A thread owns at most two (row, state) elements for the whole run and keeps their
-// column words, value indices and diagonal in registers, so a term is: gather x (L2), read y / psi', compute, store, and a hardware
-// cluster barrier (barrier.cluster with release / acquire: ~0.3 us) before the next term; block 0 adds the 8 block partials of
-// the last term in a fixed order.  The per-term scalars of the three buffer-rotation phases sit in shared memory.
+// SMs) and keeps the four vectors of the tile (three rotating buffers + the bra) in DISTRIBUTED SHARED MEMORY: block c holds
+// elements [c E, (c + 1) E) of each vector, a gather of x[col] is a ld.shared::cluster from the block that owns it (mapa), and
+// consecutive terms are separated by a hardware cluster barrier with release / acquire semantics.  A thread owns at most two
+// (row, state) elements for the whole run and keeps their column words, hopping values and diagonal in registers; block 0 adds the
+// 8 block partials of the last term in a fixed order.  The per-term scalars of the three buffer-rotation phases sit in shared memory.
 // Kernel layout with a value table, rows of <= 4 off-diagonal entries, <= 16,384 elements per vector; anything else takes the
-// launch-per-term path.
+// launch-per-term path.  psi is written back to its global buffer at the end (tbpm_get_state).
 // ---------------------------------------------------------------------------------------------------------------------
-constexpr int kSmallThreads = 1024, kSmallCluster = 8, kSmallMaxK = 28, kSmallCH = 4, kSmallRPT = 2;
+constexpr int kSmallThreads = 1024, kSmallCluster = 8, kSmallClusterMax = 16, kSmallMaxK = 28, kSmallCH = 4, kSmallRPT = 2;
 struct TermLite {
-    const double2 *x; double2 *y, *acc;
-    double a; double2 ca, cb, cc;
+    int ix, iy, iacc;             // which of the three rotating buffers holds T_{k-1}, T_{k-2} / T_k, psi'
     int n_acc, flags;
+    double a; double2 ca, cb, cc;
 };
 struct SmallParams {
     const TermLite *terms;        // device [3][K]: terms[slot * K + k] for psi in buffer `slot`
-    const uint32_t *orp; const int32_t *ocol; const uint16_t *oidx; const double2 *vtab; const double *diag; const double2 *psi0;
+    const uint32_t *orp; const int32_t *ocol; const uint16_t *oidx; const double2 *vtab; const double *diag;
+    double2 *buf[3];              // global tile buffers: buf[start_slot] holds psi on entry, buf[final slot] psi on exit
+    const double2 *bra;
     int64_t n_orb;
+    int E;                        // elements of a vector per block (a multiple of the tile width)
     int K, n_step, start_slot, n_valid, state0, packed, uniform, max_row_off;
     double *corr, *norm2, *partial;
 };
+__device__ __forceinline__ double2 ld_dsmem(uint32_t local_addr, uint32_t rank)
+{
+    uint32_t ra;
+    double2 v;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(local_addr), "r"(rank));
+    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(ra) : "memory");
+    return v;
+}
 template <int BT>
 __global__ void __launch_bounds__(kSmallThreads, 1) k_small_steps(const SmallParams sp)
 {
+    extern __shared__ __align__(16) unsigned char small_smem[];          // [4][E] complex128: buffers 0..2, bra
     __shared__ TermLite tl[3 * kSmallMaxK];
     for (int i = threadIdx.x; i < 3 * sp.K * (int)(sizeof(TermLite) / 4); i += kSmallThreads)
         reinterpret_cast<uint32_t *>(tl)[i] = __ldg(reinterpret_cast<const uint32_t *>(sp.terms) + i);
-    constexpr int kRowsPerBlock = kSmallThreads / BT;
-    const int b = threadIdx.x % BT;
-    const int64_t stride = (int64_t)gridDim.x * kRowsPerBlock;
-    // the thread's elements and their matrix rows, for the whole run
-    int64_t e[kSmallRPT];
-    int32_t col[kSmallRPT][kSmallCH];
+    double2 *vec = reinterpret_cast<double2 *>(small_smem);
+    const uint32_t vec0 = (uint32_t)__cvta_generic_to_shared(vec);
+    const int E = sp.E, b = threadIdx.x % BT;
+    const int64_t n_el = sp.n_orb * BT, e0 = (int64_t)blockIdx.x * E;
+    // the thread's elements (local index le, -1: none) and their matrix rows, for the whole run
+    int le[kSmallRPT];
+    int32_t col[kSmallRPT][kSmallCH];       // element index (col * BT + b) of each neighbour, split below into (owner, local)
     double2 val[kSmallRPT][kSmallCH];
     double dg[kSmallRPT];
     int nr[kSmallRPT];
 #pragma unroll
     for (int i = 0; i < kSmallRPT; ++i) {
-        const int64_t row = (int64_t)blockIdx.x * kRowsPerBlock + threadIdx.x / BT + i * stride;
-        nr[i] = -1; e[i] = 0; dg[i] = 0.0;
+        le[i] = (int)threadIdx.x + i * kSmallThreads;
+        const int64_t e = e0 + le[i];
+        nr[i] = 0; dg[i] = 0.0;
 #pragma unroll
         for (int j = 0; j < kSmallCH; ++j) { col[i][j] = 0; val[i][j] = make_double2(0.0, 0.0); }
-        if (row < sp.n_orb) {
-            e[i] = row * BT + b;
-            const uint32_t q0 = sp.uniform ? (uint32_t)row * (uint32_t)sp.max_row_off : __ldg(sp.orp + row);
-            const uint32_t q1 = sp.uniform ? q0 + (uint32_t)sp.max_row_off : __ldg(sp.orp + row + 1);
-            nr[i] = (int)(q1 - q0);
-            for (int j = 0; j < nr[i]; ++j) {
-                const uint32_t w = (uint32_t)__ldg(sp.ocol + q0 + j);
-                const uint32_t id = sp.packed ? (w >> 31) << 15 : (uint32_t)__ldg(sp.oidx + q0 + j);
-                col[i][j] = (int32_t)(w & 0x7fffffffu);
-                val[i][j] = table_value(__ldg(sp.vtab + (id & 0x7fffu)), id);
-            }
-            if (sp.diag) dg[i] = __ldg(sp.diag + row);
+        if (le[i] >= E || e >= n_el) { le[i] = -1; continue; }
+        const int64_t row = e / BT;                         // E is a multiple of BT: e % BT == threadIdx.x % BT == b
+        const uint32_t q0 = sp.uniform ? (uint32_t)row * (uint32_t)sp.max_row_off : __ldg(sp.orp + row);
+        const uint32_t q1 = sp.uniform ? q0 + (uint32_t)sp.max_row_off : __ldg(sp.orp + row + 1);
+        nr[i] = (int)(q1 - q0);
+        for (int j = 0; j < nr[i]; ++j) {
+            const uint32_t w = (uint32_t)__ldg(sp.ocol + q0 + j);
+            const uint32_t id = sp.packed ? (w >> 31) << 15 : (uint32_t)__ldg(sp.oidx + q0 + j);
+            col[i][j] = (int32_t)((w & 0x7fffffffu) * BT + b);
+            val[i][j] = table_value(__ldg(sp.vtab + (id & 0x7fffu)), id);
         }
+        if (sp.diag) dg[i] = __ldg(sp.diag + row);
+        // psi and the bra of the tile come in from global memory; the other two buffers are written before they are read
+        vec[(size_t)sp.start_slot * E + le[i]] = sp.buf[sp.start_slot][e];
+        vec[(size_t)3 * E + le[i]] = sp.bra[e];
     }
     __syncthreads();
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
     int slot = sp.start_slot;
     for (int n = 0; n < sp.n_step; ++n) {
         for (int k = 1; k < sp.K; ++k) {
             const TermLite &t = tl[slot * sp.K + k];
             const bool sub_y = t.flags & F_SUB_Y, reduce = t.flags & F_REDUCE, wy = t.flags & F_WRITE_Y;
             const bool need_y = sub_y || t.n_acc == 3, need_acc = t.n_acc > 0 && !(t.flags & F_ACC_INIT);
+            const uint32_t xbase = vec0 + (uint32_t)t.ix * (uint32_t)E * 16u;
+            double2 *yv = vec + (size_t)t.iy * E, *av = vec + (size_t)t.iacc * E;
+            const double2 *xl = vec + (size_t)t.ix * E, *zv = vec + (size_t)3 * E;
             double s_re = 0.0, s_im = 0.0, s_nn = 0.0;
 #pragma unroll
             for (int i = 0; i < kSmallRPT; ++i) {
-                if (nr[i] < 0) continue;
+                if (le[i] < 0) continue;
                 double2 xv[kSmallCH];
 #pragma unroll
-                for (int j = 0; j < kSmallCH; ++j) xv[j] = j < nr[i] ? __ldcg(t.x + (int64_t)col[i][j] * BT + b) : make_double2(0.0, 0.0);
-                const double2 xrow = __ldcg(t.x + e[i]);
+                for (int j = 0; j < kSmallCH; ++j) {
+                    xv[j] = make_double2(0.0, 0.0);
+                    if (j < nr[i]) { const uint32_t owner = (uint32_t)col[i][j] / (uint32_t)E, loc = (uint32_t)col[i][j] - owner * (uint32_t)E; xv[j] = ld_dsmem(xbase + loc * 16u, owner); }
+                }
+                const double2 xrow = xl[le[i]];
                 double2 yold = make_double2(0.0, 0.0), aold = yold, z = yold;
-                if (need_y) yold = __ldcg(t.y + e[i]);
-                if (need_acc) aold = __ldcg(t.acc + e[i]);
-                if (reduce) z = __ldg(sp.psi0 + e[i]);
+                if (need_y) yold = yv[le[i]];
+                if (need_acc) aold = av[le[i]];
+                if (reduce) z = zv[le[i]];
                 double2 h = make_double2(0.0, 0.0);
 #pragma unroll
                 for (int j = 0; j < kSmallCH; ++j) cfma(h, val[i][j], xv[j]);
                 h.x = fma(dg[i], xrow.x, h.x); h.y = fma(dg[i], xrow.y, h.y);
                 h.x *= t.a; h.y *= t.a;
                 if (sub_y) { h.x -= yold.x; h.y -= yold.y; }
-                if (wy) t.y[e[i]] = h;
+                if (wy) yv[le[i]] = h;
                 if (t.n_acc > 0) {
                     double2 s = aold;
                     cfma(s, t.ca, h);
                     if (t.n_acc >= 2) cfma(s, t.cb, xrow);
                     if (t.n_acc == 3) cfma(s, t.cc, yold);
-                    t.acc[e[i]] = s;
+                    av[le[i]] = s;
                     if (reduce) {
                         s_re = fma(z.x, s.x, s_re); s_re = fma(z.y, s.y, s_re);
                         s_im = fma(z.x, s.y, s_im); s_im = fma(-z.y, s.x, s_im);
@@ -277,7 +301,8 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_small_steps(const SmallPar
                 }
             }
             if (reduce) block_partial<BT, kSmallThreads>(s_re, s_im, s_nn, sp.partial, blockIdx.x);
-            // T_k (and the partials) become visible to the whole cluster: every block of the grid is in it
+            // T_k in shared memory (and the partials in global memory) become visible to the whole cluster
+            if (reduce) __threadfence();
             asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
         }
         if (blockIdx.x == 0 && threadIdx.x < sp.n_valid * 3) {
@@ -290,6 +315,9 @@ __global__ void __launch_bounds__(kSmallThreads, 1) k_small_steps(const SmallPar
         }
         slot = (slot + 2) % 3;
     }
+#pragma unroll
+    for (int i = 0; i < kSmallRPT; ++i)
+        if (le[i] >= 0) sp.buf[slot][e0 + le[i]] = vec[(size_t)slot * E + le[i]];
 }
 
 // NEXT-4, dynamic polarisation: a DIAGONAL complex operator d (the density operator exp(i q.r)) on one tile of interleaved states.
@@ -709,31 +737,47 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
                            n_el <= (int64_t)kSmallRPT * kSmallCluster * kSmallThreads && H->opt_kernel == 0 && knob("small", 1);
         if (small) {
             std::vector<TermLite> all((size_t)3 * K);
+            auto which = [&](const double2 *q) { return q == buf[0] ? 0 : (q == buf[1] ? 1 : 2); };
             for (int sl = 0; sl < 3; ++sl) {
                 step_terms(tp, K, cf, rescale, false, buf[sl], buf[(sl + 1) % 3], buf[(sl + 2) % 3], term);
                 for (int k = 1; k < K; ++k) {
                     const TermParams &q = term[k];
-                    all[(size_t)sl * K + k] = TermLite{q.x, q.y, q.acc, q.a, q.ca, q.cb, q.cc, q.n_acc, q.flags};
+                    all[(size_t)sl * K + k] = TermLite{which(q.x), which(q.y), which(q.acc), q.n_acc, q.flags, q.a, q.ca, q.cb, q.cc};
                 }
             }
             TermLite *d_terms = reinterpret_cast<TermLite *>(W + P.aux_off);
             // pageable source: the call returns once the data is staged, so `all` may go out of scope
             TBPM_CUDA_TRY(cudaMemcpyAsync(d_terms, all.data(), all.size() * sizeof(TermLite), cudaMemcpyHostToDevice, st));
-            SmallParams sp{d_terms, tp.orp, tp.ocol, tp.oidx, tp.vtab, tp.diag, bra, H->n_orb, K, n_step, start_slot, n_valid, state0,
-                           tp.packed, tp.uniform, tp.max_row_off, corr, norm2, partial};
+            constexpr int kSmallSmem = 4 * kSmallRPT * kSmallThreads * (int)sizeof(double2);   // 128 KB: the most a block can be asked for
+            static int cluster_size[kMaxDevices][4] = {};   // per device and tile width: 16 blocks (opt-in cluster size) if they fit, else 8
+            const int bi = bt == 1 ? 0 : (bt == 2 ? 1 : (bt == 4 ? 2 : 3));
+            if (H->device < 0 || H->device >= kMaxDevices) return TBPM_EINVAL;
+            const void *kern = bt == 1 ? (const void *)k_small_steps<1> : bt == 2 ? (const void *)k_small_steps<2> :
+                               bt == 4 ? (const void *)k_small_steps<4> : (const void *)k_small_steps<8>;
             cudaLaunchConfig_t cfg{};
-            cfg.gridDim = dim3(kSmallCluster); cfg.blockDim = dim3(kSmallThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
             cudaLaunchAttribute attr[1];
             attr[0].id = cudaLaunchAttributeClusterDimension;
-            attr[0].val.clusterDim.x = kSmallCluster; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-            cfg.attrs = attr; cfg.numAttrs = 1;
-            cudaError_t le = cudaErrorInvalidValue;
-            switch (bt) {
-            case 1: le = cudaLaunchKernelEx(&cfg, k_small_steps<1>, sp); break;
-            case 2: le = cudaLaunchKernelEx(&cfg, k_small_steps<2>, sp); break;
-            case 4: le = cudaLaunchKernelEx(&cfg, k_small_steps<4>, sp); break;
-            case 8: le = cudaLaunchKernelEx(&cfg, k_small_steps<8>, sp); break;
+            attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+            cfg.blockDim = dim3(kSmallThreads); cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
+            if (cluster_size[H->device][bi] == 0) {
+                TBPM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmallSmem));
+                int cs = kSmallCluster, n_cl = 0;
+                if (cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
+                    cfg.gridDim = dim3(kSmallClusterMax); cfg.dynamicSmemBytes = kSmallSmem / 2;
+                    attr[0].val.clusterDim.x = kSmallClusterMax;
+                    if (cudaOccupancyMaxActiveClusters(&n_cl, kern, &cfg) == cudaSuccess && n_cl >= 1) cs = kSmallClusterMax;
+                }
+                (void)cudaGetLastError();
+                cluster_size[H->device][bi] = cs;
             }
+            const int cs = cluster_size[H->device][bi];
+            const int E = (int)(((n_el + cs - 1) / cs + bt - 1) / bt * bt);
+            SmallParams sp{d_terms, tp.orp, tp.ocol, tp.oidx, tp.vtab, tp.diag, {buf[0], buf[1], buf[2]}, bra, H->n_orb, E, K, n_step,
+                           start_slot, n_valid, state0, tp.packed, tp.uniform, tp.max_row_off, corr, norm2, partial};
+            cfg.gridDim = dim3(cs); cfg.dynamicSmemBytes = (size_t)4 * E * sizeof(double2);
+            attr[0].val.clusterDim.x = cs;
+            void *kargs[] = {&sp};
+            cudaError_t le = cudaLaunchKernelExC(&cfg, kern, kargs);
             TBPM_CUDA_TRY(le);
             count_launches(1);
             slot = (start_slot + 2 * n_step) % 3;
