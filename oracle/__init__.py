@@ -3,6 +3,10 @@
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may import this package.
 It imports nothing from paper_2509_26309_b200 (the CUDA path) and shares no code with it.  All arrays are numpy,
 complex128 viewed as (re, im) float64 pairs.  See the header of tbpm_oracle.c for the algorithm and its citations.
+
+The NEXT rows of SURVEY.md 8(f) are plain numpy on top of the C routines (quasi_eigenstates, haydock, haydock_ldos,
+fermi_cheb_coeff, apply_cheb_series, corr_ac, corr_dp), each pinned in tests/test_oracle_next_pins.py by exact diagonalisation,
+closed forms or brute force.  Parity unpinned: none.
 """
 from __future__ import annotations
 
