@@ -341,6 +341,20 @@ def test_prefix_determinism_and_edge_calls(dev, oracle_mod):
     assert dn is None and torch.equal(d, c)
 
 
+@pytest.mark.parametrize("cfg,over", [(5, dict(L=32)), (4, dict(Lx=128, Ly=32, phi_den=32)), (1, {})])
+def test_lattice_and_cluster_kernels_are_deterministic(dev, cfg, over):
+    """term_l3, term_sq and k_small_steps: bit-identical reruns and the prefix property (what the parity protocols at scale rest on)."""
+    w = W.make_workload(cfg, device=dev, **over)
+    n_state = 1 if cfg == 1 else 8
+    psi0 = w.psi0(device=dev, n_state=n_state)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    a, an, _ = tbpm.tbpm_propagate(H, psi0, 14, w.dt, w.rescale)
+    b, bn, _ = tbpm.tbpm_propagate(H, psi0, 14, w.dt, w.rescale)
+    c, cn, _ = tbpm.tbpm_propagate(H, psi0, 6, w.dt, w.rescale)
+    assert torch.equal(a, b) and torch.equal(an, bn)
+    assert torch.equal(a[:, :6], c) and torch.equal(an[:, :6], cn)
+
+
 def test_windowed_parity_from_snapshot(dev, oracle_mod):
     """Reading/§8(d)(3): download psi at a late step from the GPU, let the oracle advance it and compare the window."""
     w = W.make_workload(2, device=dev, Na=64, Nb=48)
