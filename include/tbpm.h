@@ -181,6 +181,11 @@ int tbpm_propagate_qe(tbpm_ham *H, const double *psi0, int n_state, int n_step, 
  * kernel), then the three-vector update fused with the norm. */
 int tbpm_haydock(tbpm_ham *H, const int64_t *sites /* host */, int n_site, int n_iter, double *a /* device out */,
                  double *b /* device out */, void *workspace, size_t workspace_bytes, void *stream);
+/* The continued fraction on the device: ldos[s][j] = -Im G_s(energy[j] + i eta) / pi, cut after a_{n_iter-1} (the chain is simply
+ * finite; b_{n_iter} is not used).  a, b: device [n_site][n_iter] as written by tbpm_haydock; energy: device [n_energy];
+ * ldos: device out [n_site][n_energy]; eta > 0. */
+int tbpm_haydock_ldos(const double *a, const double *b, int n_site, int n_iter, const double *energy, int n_energy, double eta,
+                      double *ldos, void *stream);
 
 /* ---- NEXT-4: AC-conductivity correlation function ("AC conductivity (AC)"; Table 7; the current
  * operator acts through a sparse matrix-vector product, and has a CSR of its own) ------------------

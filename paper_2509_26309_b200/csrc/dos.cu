@@ -49,3 +49,40 @@ extern "C" int tbpm_dos(const double *corr, int n_state, int n_step, double dt, 
     TBPM_CUDA_TRY(cudaGetLastError());
     return TBPM_OK;
 }
+
+// NEXT-2, last step: LDOS from the Haydock coefficients by the continued fraction (reading #29)
+//     G(z) = 1 / (z - a_0 - b_1^2 / (z - a_1 - b_2^2 / ( ... - b_{n-1}^2 / (z - a_{n-1})))),  z = E + i eta,  ldos = -Im G / pi,
+// evaluated from the bottom up; one thread per (site, energy).  a, b as written by tbpm_haydock (b[.][n] = b_{n+1}).
+namespace {
+__global__ void k_haydock_ldos(const double *__restrict__ a, const double *__restrict__ b, int n_site, int n_iter, const double *__restrict__ energy,
+                               int n_e, double eta, double *ldos)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_site * n_e) return;
+    const int s = t / n_e, j = t - s * n_e;
+    const double zr = energy[j], zi = eta;
+    double gr = 0.0, gi = 0.0;                               // G of the levels below
+    for (int n = n_iter - 1; n >= 0; --n) {
+        const double bb = n < n_iter - 1 ? b[(size_t)s * n_iter + n] : 0.0;
+        const double dr = zr - a[(size_t)s * n_iter + n] - bb * bb * gr, di = zi - bb * bb * gi;
+        const double m = dr * dr + di * di;
+        gr = dr / m;
+        gi = -di / m;
+    }
+    ldos[t] = -gi / 3.14159265358979323846;
+}
+}  // namespace
+
+extern "C" int tbpm_haydock_ldos(const double *a, const double *b, int n_site, int n_iter, const double *energy, int n_energy, double eta,
+                                 double *ldos, void *stream)
+{
+    if (n_site < 0 || n_iter < 1 || n_energy < 0 || !(eta > 0.0)) return TBPM_EINVAL;
+    if (n_site == 0 || n_energy == 0) return TBPM_OK;
+    if (!a || !b || !energy || !ldos) return TBPM_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int total = n_site * n_energy, threads = 128;
+    k_haydock_ldos<<<(total + threads - 1) / threads, threads, 0, st>>>(a, b, n_site, n_iter, energy, n_energy, eta, ldos);
+    count_launches(1);
+    TBPM_CUDA_TRY(cudaGetLastError());
+    return TBPM_OK;
+}

@@ -62,6 +62,7 @@ def lib() -> C.CDLL:
         L.tbpm_corr_ac_bytes.argtypes = [vp, C.c_int, P(sz)]
         L.tbpm_corr_ac.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, dbl, dbl, dbl, dbl, vp, vp, sz, vp]
         L.tbpm_corr_dp.argtypes = [vp, vp, vp, vp, C.c_int, C.c_int, dbl, dbl, dbl, dbl, vp, vp, sz, vp]
+        L.tbpm_haydock_ldos.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, dbl, vp, vp]
         L.tbpm_last_launch_count.restype = i64
         L.tbpm_last_launch_count.argtypes = [vp]
         L.tbpm_set_option.argtypes = [vp, C.c_int, i64]
@@ -304,6 +305,18 @@ def tbpm_corr_dp(H: Hamiltonian, rho_a: torch.Tensor, rho_b: torch.Tensor, psi0:
                                 ws.numel(), _stream(dev))
     _check(rc, "tbpm_corr_dp")
     return corr
+
+
+def tbpm_haydock_ldos(a: torch.Tensor, b: torch.Tensor, energy: torch.Tensor, eta: float) -> torch.Tensor:
+    """LDOS [n_site][n_energy] from the recursion coefficients (device tensors as returned by tbpm_haydock) by the continued fraction."""
+    _need_cuda(a, b, energy)
+    a, b, energy = a.contiguous(), b.contiguous(), energy.to(torch.float64).contiguous()
+    n_site, n_iter = a.shape
+    out = torch.zeros((n_site, energy.numel()), dtype=torch.float64, device=a.device)
+    with torch.cuda.device(a.device):
+        _check(lib().tbpm_haydock_ldos(_ptr(a), _ptr(b), n_site, n_iter, _ptr(energy), energy.numel(), eta, _ptr(out), _stream(a.device)),
+               "tbpm_haydock_ldos")
+    return out
 
 
 def tbpm_dos(corr: torch.Tensor, dt: float, rescale: float):

@@ -111,6 +111,8 @@ def test_haydock_chain_closed_form_and_ldos(dev, oracle_mod):
     exact = -(np.abs(V[11]) ** 2 / (E[:, None] + 0.4j - Ej[None, :])).sum(axis=1).imag / np.pi
     got = oracle_mod.haydock_ldos(a[0].cpu().numpy(), b[0].cpu().numpy(), E, 0.4)
     assert np.abs(got - exact).max() <= 1e-9 * exact.max()
+    dev_ldos = tbpm.tbpm_haydock_ldos(a, b, torch.as_tensor(E, device=dev), 0.4)      # the continued fraction on the device
+    assert np.abs(dev_ldos[0].cpu().numpy() - got).max() <= 1e-12 * exact.max()
     assert tbpm.lib().tbpm_haydock(Hs.handle, None, 0, 5, None, None, None, 0, None) == tbpm.TBPM_OK   # n_site = 0
     with pytest.raises(tbpm.TbpmError):
         tbpm.tbpm_haydock(Hs, [64], 3)
