@@ -155,19 +155,55 @@ extern "C" int tbpm_corr_host(int64_t n_orb, const double *onsite, int64_t n_hop
     if ((rc = h2d(A.hop_j, hop_j, sizeof(int32_t) * (size_t)n_hop))) return rc;
     if ((rc = h2d(A.hop_val, hop_val, sizeof(double) * 2 * (size_t)n_hop))) return rc;
     if (onsite && (rc = h2d(A.onsite, onsite, sizeof(double) * (size_t)n_orb))) return rc;
-    if ((rc = h2d(A.psi0, psi0, sizeof(double) * 2 * (size_t)n_orb * (size_t)n_state))) return rc;
+    // psi0 goes up on a stream of its own, one tile of states at a time, so that the copy of tile t + 1 (and later) overlaps the
+    // build and the propagation of the tiles before it; the tiles are independent, so the results are those of one call, bit for bit.
+    const int tile = 8;
+    const int n_tile = (n_state + tile - 1) / tile;
+    cudaStream_t cs = nullptr;
+    std::vector<cudaEvent_t> ev((size_t)std::max(n_tile, 0), nullptr);
+    auto cleanup = [&]() {
+        for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e);
+        if (cs) cudaStreamDestroy(cs);
+    };
+    if (n_state > 0 && n_step > 0 && n_orb > 0) {
+        if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess) { note_cuda_error(cudaGetLastError()); return TBPM_ECUDA; }
+        cudaEvent_t e0 = nullptr;                           // whatever the caller queued on `stream` before this call comes first
+        if (cudaEventCreateWithFlags(&e0, cudaEventDisableTiming) == cudaSuccess) {
+            cudaEventRecord(e0, st);
+            cudaStreamWaitEvent(cs, e0, 0);
+            cudaEventDestroy(e0);
+        }
+        for (int t = 0; t < n_tile; ++t) {
+            const int s0 = t * tile, ns = std::min(tile, n_state - s0);
+            const size_t off = sizeof(double) * 2 * (size_t)n_orb * (size_t)s0, bytes = sizeof(double) * 2 * (size_t)n_orb * (size_t)ns;
+            if (cudaEventCreateWithFlags(&ev[t], cudaEventDisableTiming) != cudaSuccess ||
+                cudaMemcpyAsync(D + A.psi0 + off, reinterpret_cast<const char *>(psi0) + off, bytes, cudaMemcpyHostToDevice, cs) != cudaSuccess ||
+                cudaEventRecord(ev[t], cs) != cudaSuccess) {
+                note_cuda_error(cudaGetLastError());
+                cudaStreamSynchronize(cs);
+                cleanup();
+                return TBPM_ECUDA;
+            }
+            up += bytes;
+        }
+    }
 
     tbpm_ham *H = nullptr;
     rc = tbpm_build(n_orb, onsite ? reinterpret_cast<const double *>(D + A.onsite) : nullptr, n_hop,
                     reinterpret_cast<const int32_t *>(D + A.hop_i), reinterpret_cast<const int32_t *>(D + A.hop_j),
                     reinterpret_cast<const double *>(D + A.hop_val), flags, D + A.persist, A.persist_bytes, D + A.scratch,
                     A.scratch_bytes, stream, &H);
-    if (rc) return rc;
-    rc = tbpm_propagate(H, reinterpret_cast<const double *>(D + A.psi0), n_state, n_step, dt, rescale,
-                        reinterpret_cast<double *>(D + A.corr), reinterpret_cast<double *>(D + A.norm2), D + A.workspace,
-                        A.workspace_bytes, stream);
+    if (rc) { if (cs) cudaStreamSynchronize(cs); cleanup(); return rc; }
+    if (H->opt_tile != tile) { tbpm_free(H); if (cs) cudaStreamSynchronize(cs); cleanup(); return TBPM_EINVAL; }
+    for (int t = 0; t < n_tile && !rc && cs; ++t) {
+        const int s0 = t * tile, ns = std::min(tile, n_state - s0);
+        if (cudaStreamWaitEvent(st, ev[t], 0) != cudaSuccess) { note_cuda_error(cudaGetLastError()); rc = TBPM_ECUDA; break; }
+        rc = tbpm_propagate(H, reinterpret_cast<const double *>(D + A.psi0) + 2 * (size_t)n_orb * (size_t)s0, ns, n_step, dt, rescale,
+                            reinterpret_cast<double *>(D + A.corr) + 2 * (size_t)s0 * (size_t)n_step,
+                            reinterpret_cast<double *>(D + A.norm2) + (size_t)s0 * (size_t)n_step, D + A.workspace, A.workspace_bytes, stream);
+    }
     tbpm_free(H);
-    if (rc) return rc;
+    if (rc) { if (cs) cudaStreamSynchronize(cs); cudaStreamSynchronize(st); cleanup(); return rc; }
     const size_t nc = (size_t)n_state * (size_t)n_step;
     if (nc > 0) {
         TBPM_CUDA_TRY(cudaMemcpyAsync(corr, D + A.corr, sizeof(double) * 2 * nc, cudaMemcpyDeviceToHost, st));
@@ -177,7 +213,9 @@ extern "C" int tbpm_corr_host(int64_t n_orb, const double *onsite, int64_t n_hop
             down += sizeof(double) * nc;
         }
     }
-    TBPM_CUDA_TRY(cudaStreamSynchronize(st));
+    const cudaError_t se = cudaStreamSynchronize(st);
+    cleanup();
+    TBPM_CUDA_TRY(se);
     if (h2d_bytes) *h2d_bytes = up;
     if (d2h_bytes) *d2h_bytes = down;
     return TBPM_OK;
