@@ -254,14 +254,14 @@ class Runner:
 
     def roofline(self, prop_ms_per_step, peak, peak_src):
         """Algorithmic bytes (matrix as stored + 3 vectors) against the measured launch time of the fused term.
-        The matrix bytes are those of the layout the running kernel reads: on the two lattices the builder recognises (tiles of 8
-        states) that is a few bytes per row, not the general kernel layout; the figure with the general layout is given beside it."""
+        The matrix bytes are those of the layout the running kernel reads: on the lattices the builder recognises (tiles of 8
+        states; short rows with one real value for tiles of 1-4 states) that is a few bytes per row, not the general kernel layout; the figure with the general layout is given beside it."""
         H, w = self.H, self.w
         tile = min(8, 1 << max(self.n_state - 1, 0).bit_length())
         n_tile = -(-self.n_state // tile)
         term_launches = n_tile * self.block * (self.K - 1)
         avg_launch_s = prop_ms_per_step * 1e-3 / term_launches
-        lattice = tile == 8 and H.lattice_kind != 0
+        lattice = (tile == 8 and H.lattice_kind in (2, 3)) or (tile <= 4 and H.lattice_kind == 4)
         m_launch = H.lattice_bytes_per_term if lattice else H.matrix_bytes_per_term     # what ONE launch reads of H
         bytes_tile = m_launch + 48 * w.n_orb * min(tile, self.n_state)                    # one launch = one tile of states
         bytes_term_strict = m_launch + 48 * w.n_orb * self.n_state                        # one term for ALL states, matrix counted once
@@ -270,7 +270,8 @@ class Runner:
         achieved_tile = bytes_tile / avg_launch_s / 1e9
         traffic, tsrc = ncu_traffic(w.name + ("-ldos" if self.ldos else ""), self.K)
         kernel = {2: "k_term_l3 (fused Chebyshev term, three-dimensional lattice kernel, term_l3.cu)",
-                  3: "k_term_sq (fused Chebyshev term, square lattice with in-line hoppings, term_sq.cu)"}.get(
+                  3: "k_term_sq (fused Chebyshev term, square lattice with in-line hoppings, term_sq.cu)",
+                  4: "k_term_n16 (fused Chebyshev term, short rows with 16-bit column offsets, term_n16.cu)"}.get(
                       H.lattice_kind if lattice else 0, "k_term_ph (fused Chebyshev term, term_ph.cuh)")
         return {"bound": "hbm", "kernel": kernel,
                 "achieved": achieved_strict, "peak": peak, "unit": "GB/s", "frac": achieved_strict / peak,
@@ -457,7 +458,7 @@ def main_next(args):
         run = lambda: tbpm.tbpm_haydock(H, sites, block, workspace=ws)
         units = n_state * block * H.nnz                              # H applications x nnz
         tile = 8
-        mat = H.lattice_bytes_per_term if H.lattice_kind else H.matrix_bytes_per_term
+        mat = H.lattice_bytes_per_term if H.lattice_kind in (2, 3) else H.matrix_bytes_per_term
         # per recursion level and tile: H u (matrix, gather u, write t) + update (read t, u, u_prev, write u_next): matrix + 6 vectors
         bytes_step = (n_state // tile) * block * (mat + 6 * 16 * w.n_orb * tile)
         what = "Haydock recursion: H u fused with <u|H u> (k_term_l3, last-term shape) + three-vector update fused with the norm (k_haydock_update)"
@@ -469,8 +470,9 @@ def main_next(args):
         run = lambda: tbpm.tbpm_propagate_qe(H, psi0, energies, block, w.dt, w.rescale)
         units = n_state * block * (K - 1) * H.nnz
         # per time step: the K - 1 terms (matrix + 3 vectors each) + the accumulation sweep (read psi', read + write n_E vectors)
-        bytes_step = block * ((K - 1) * (H.matrix_bytes_per_term + 48 * w.n_orb * n_state) + (1 + 2 * len(energies)) * 16 * w.n_orb * n_state)
-        what = "propagation + quasi-eigenstates at 2 energies: k_term_ph per term, k_qe_axpy once per time step"
+        mat = H.lattice_bytes_per_term if (H.lattice_kind == 4 and n_state <= 4) else H.matrix_bytes_per_term
+        bytes_step = block * ((K - 1) * (mat + 48 * w.n_orb * n_state) + (1 + 2 * len(energies)) * 16 * w.n_orb * n_state)
+        what = "propagation + quasi-eigenstates at 2 energies: k_term_n16 / k_term_ph per term, k_qe_axpy once per time step"
         count = "per time step: (K - 1) x (matrix + 3 vectors) + (1 + 2 n_E) vectors of the accumulation sweep (workspace allocation and export included in the time)"
     for _ in range(max(args.warmup, 1)):
         run()

@@ -515,8 +515,33 @@ __global__ void k_sq8(int64_t n_orb, int64_t W, const int32_t *__restrict__ ocol
     if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicAdd(&status[ST_SQ8_BAD], 1);
 }
 
+// Short rows that reach no further than 32767 rows, one real hopping value (honeycomb and square lattices with vacancies or on-site
+// disorder, chains): the whole off-diagonal structure is kept a second time as 16-bit column offsets, d16[j][r] = col_j - r (modulo
+// n_orb, so that the neighbours across a periodic boundary count as near) for the entries of row r in column order and 0 for the
+// slots a shorter row leaves empty -- 2 W bytes per row instead of the row offsets and
+// column words (4 + 4 n bytes), read fully coalesced by term_n16.cu.
+__global__ void k_near16(int64_t n_orb, int W, const uint32_t *__restrict__ orp, const int32_t *__restrict__ ocol, int16_t *d16, int32_t *status)
+{
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool bad = false;
+    if (r < n_orb) {
+        const uint32_t b = orp[r], n = orp[r + 1] - b;
+        for (int j = 0; j < W; ++j) {
+            int64_t d = 0;
+            if ((uint32_t)j < n) d = (int64_t)(ocol[b + j] & 0x7fffffff) - r;
+            if (2 * d > n_orb) d -= n_orb;                  // taken round the periodic boundary: the kernel wraps row + d into [0, n_orb)
+            else if (2 * d < -n_orb) d += n_orb;
+            if (d > 32767 || d < -32767) { bad = true; d = 0; }
+            d16[(r >> 5) * (int64_t)(W * 32) + j * 32 + (r & 31)] = (int16_t)d;   // [32 rows][slot][row]: a warp reads 64 contiguous bytes per slot
+        }
+        bad = bad || n > (uint32_t)W;
+    }
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicAdd(&status[ST_N16_BAD], 1);
+}
+constexpr int kNear16MaxW = 4;
+
 struct PersistLayout {
-    size_t status, rowptr, col, val, orp, ocol, oidx, vtab, diag, latflag, dline, total;
+    size_t status, rowptr, col, val, orp, ocol, oidx, vtab, diag, latflag, dline, d16, total;
 };
 
 PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint32_t flags)
@@ -537,6 +562,7 @@ PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint3
     L.diag = has_onsite ? take(sizeof(double) * (size_t)n_orb) : 0;
     L.latflag = take(sizeof(uint32_t) * ((size_t)n_orb / 32 + 2));
     L.dline = take(sizeof(uint16_t) * 8 * (size_t)kSq8MaxLine);
+    L.d16 = take(sizeof(int16_t) * kNear16MaxW * ((size_t)n_orb + 32));
     L.total = o;
     return L;
 }
@@ -624,6 +650,7 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
     H->diag = has_onsite ? reinterpret_cast<double *>(P + PL.diag) : nullptr;
     H->lat_flags = reinterpret_cast<uint32_t *>(P + PL.latflag);
     H->dline = reinterpret_cast<uint16_t *>(P + PL.dline);
+    H->d16 = reinterpret_cast<int16_t *>(P + PL.d16);
     int32_t *cnt = reinterpret_cast<int32_t *>(S + SL.cnt);
     int32_t *cur = reinterpret_cast<int32_t *>(S + SL.cur);
     int64_t *bsum = reinterpret_cast<int64_t *>(S + SL.bsum);
@@ -710,6 +737,17 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
                 std::memcpy(&v0, reinterpret_cast<const char *>(host.data()) + 8192, sizeof(double2));
                 H->single_real = v0.y == 0.0;
             }
+            // short rows, one real value: 16-bit column offsets for term_n16.cu (every entry checked)
+            const int n_off_max = H->max_row_nnz - (has_onsite ? 1 : 0);
+            if (H->single_real && n_off_max >= 1 && n_off_max <= kNear16MaxW) {
+                const int W16 = n_off_max <= 3 ? 3 : 4;
+                k_near16<<<gr, kThreads, 0, st>>>(n_orb, W16, H->orp, H->ocol, H->d16, H->status);
+                count_launches(1);
+                int32_t bad16 = 0;
+                TRY_OR_FAIL(cudaMemcpyAsync(&bad16, H->status + ST_N16_BAD, sizeof(bad16), cudaMemcpyDeviceToHost, st));
+                TRY_OR_FAIL(cudaStreamSynchronize(st));
+                H->near16_w = bad16 == 0 ? W16 : 0;
+            }
             if (uniform) {
                 std::vector<std::vector<int64_t>> tup(kSampleRows, std::vector<int64_t>(n_off));
                 for (int i = 0; i < kSampleRows; ++i) {
@@ -794,6 +832,9 @@ extern "C" int tbpm_ham_lattice_info(const tbpm_ham *H, int32_t *kind, size_t *b
     } else if (H->sq8_line > 0 && H->sq8_line % 128 == 0) {
         k = TBPM_LATTICE_SQUARE8;                             // term_sq.cu: value indices by direction of one line + the value table
         b = sizeof(uint16_t) * 8 * (size_t)H->sq8_line + sizeof(double2) * (size_t)H->n_table + (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0);
+    } else if (H->near16_w > 0) {
+        k = TBPM_LATTICE_NEAR16;                              // term_n16.cu (tiles of 1-4 states): 16-bit column offsets + real diagonal
+        b = sizeof(int16_t) * (size_t)H->near16_w * (size_t)H->n_orb + (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0) + sizeof(double2);
     }
     if (kind) *kind = k;
     if (bytes_per_term) *bytes_per_term = b;

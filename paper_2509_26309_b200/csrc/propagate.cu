@@ -553,6 +553,7 @@ int launch_term(int bt, bool table, int kernel_opt, const TermParams &p, int num
     if (table && kernel_opt == 0 && term_l3_supported(bt, p)) return launch_term_l3(p, num_sms, st, grid_out);
     if (table && kernel_opt == 0 && term_sq_supported(bt, p)) return launch_term_sq(p, num_sms, st, grid_out);
     if (table && (kernel_opt == 0 || kernel_opt == 3) && term_rw_supported(bt, p)) return launch_term_rw(p, num_sms, st, grid_out);
+    if (table && kernel_opt == 0 && term_n16_supported(bt, p)) return launch_term_n16(bt, p, num_sms, st, grid_out);
     if (table && !general_only && term_ph_supported(bt, p)) {
         switch (bt) {
         case 1: return launch_term_ph_bt1(p, num_sms, st, grid_out);
@@ -628,6 +629,7 @@ TermParams matrix_params(const tbpm_ham *H, double *partial)
     mp.n_regular = H->n_regular;
     mp.lat_periodic3 = H->lat_periodic3;
     mp.sq8_line = H->sq8_line; mp.dline = H->dline;
+    mp.d16 = H->near16_w > 0 ? H->d16 : nullptr; mp.n16_w = H->near16_w;
     mp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     mp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));
     // L2 prefetch of the vector rows a few tiles ahead (term_ph.cuh, producer warp).  The leading edge of the gather

@@ -51,6 +51,8 @@ struct TermParams {
     int64_t n_regular;     // number of such rows
     int64_t sq8_line;      // > 0: periodic square lattice with next-nearest neighbours whose hoppings depend on the in-line position
     const uint16_t *dline; // only (build.cu, k_sq8): line length in rows and the [x][8] table of value indices by direction
+    const int16_t *d16;    // short rows, one real value (build.cu, k_near16): [row / 32][slot][row % 32] col - row modulo n_orb, 0 = empty slot
+    int n16_w;             // slots per row of d16 (3 or 4), 0: none
     int lat_periodic3;     // the bits are those of the periodic three-dimensional lattice (wrapped neighbours count as regular)
     int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
     int reverse;           // phased kernel: sweep the tiles from the last row block to the first
@@ -123,5 +125,11 @@ int launch_term_sq(const TermParams &p, int num_sms, cudaStream_t st, int *grid_
 // value (simple cubic and its anisotropic relatives); two-dimensional tiles with TMA-fed halos, walked along S2.
 bool term_l3_supported(int bt, const TermParams &p);
 int launch_term_l3(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
+
+
+// Short-row kernel (term_n16.cu): tiles of 1, 2 or 4 states, rows of <= 4 entries no further than 32767 rows away, one real hopping
+// value; reads the builder's 16-bit column offsets instead of row offsets and column words.
+bool term_n16_supported(int bt, const TermParams &p);
+int launch_term_n16(int bt, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
 }  // namespace tbpm_detail

@@ -16,7 +16,7 @@ from . import build as _build
 
 TBPM_VALIDATE, TBPM_HOPS_FULL, TBPM_NO_TABLE = 1, 2, 4
 TBPM_OPT_TILE, TBPM_OPT_KERNEL = 1, 2
-TBPM_LATTICE_CUBIC, TBPM_LATTICE_SQUARE8 = 2, 3
+TBPM_LATTICE_CUBIC, TBPM_LATTICE_SQUARE8, TBPM_LATTICE_NEAR16 = 2, 3, 4
 TBPM_OK, TBPM_EINVAL, TBPM_EINDEX, TBPM_EDIAG, TBPM_EDUP, TBPM_ENOMEM, TBPM_ECUDA, TBPM_EBOUND = 0, -1, -2, -3, -4, -5, -6, -7
 
 _lib = None

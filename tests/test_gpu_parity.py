@@ -228,6 +228,36 @@ def test_lattice_kernels_rows_off_the_lattice(dev, oracle_mod):
     assert H.lattice_kind == 0
 
 
+def test_short_row_kernel(dev, oracle_mod):
+    """term_n16.cu (tiles of one state, rows of <= 4 entries, one real value, 16-bit column offsets): honeycomb with vacancies (rows of
+    0-3 entries, periodic wrap entries stored modulo n_orb), the clean honeycomb lattice with on-site disorder (diagonal), a ring (only
+    +-1 neighbours: every gather is a warp shuffle except at the warp ends and across the ends of the ring), a square lattice with four
+    real neighbours (4 slots); and a lattice too wide for 16-bit offsets, which must stay on the phased kernel."""
+    w = W.make_workload(3, device=dev, Na=160, Nb=120)
+    H, _, _, _ = run_parity(dev, oracle_mod, w, 1, 12)
+    assert H.lattice_kind == tbpm.TBPM_LATTICE_NEAR16
+    w = W.make_workload(2, device=dev, Na=150, Nb=131)
+    H, _, _, _ = run_parity(dev, oracle_mod, w, 1, 9)
+    assert H.lattice_kind == tbpm.TBPM_LATTICE_NEAR16
+    n = 70001
+    i = torch.arange(n, device=dev, dtype=torch.int32)
+    w = W.Workload("ring", n, i, ((i + 1) % n).to(torch.int32), torch.full((n,), -1.0, dtype=torch.complex128, device=dev), None, 1, 10, 2.5)
+    H, _, _, _ = run_parity(dev, oracle_mod, w, 1, 10)
+    assert H.lattice_kind == tbpm.TBPM_LATTICE_NEAR16
+    n, hi, hj, hv = W.square_peierls_hops(320, 90, -1.0, 0.0, 1, 32, dev)
+    keep = hv.abs() > 0
+    w = W.Workload("square-nn", n, hi[keep].contiguous(), hj[keep].contiguous(), torch.full((int(keep.sum()),), -1.0, dtype=torch.complex128, device=dev),
+                   W.anderson_onsite(n, 2.0, device=dev), 1, 8, 5.5)
+    H, _, _, _ = run_parity(dev, oracle_mod, w, 1, 8)
+    assert H.lattice_kind == tbpm.TBPM_LATTICE_NEAR16
+    n, hi, hj, hv = W.square_peierls_hops(40000, 3, -1.0, 0.0, 1, 32, dev)      # line of 40000 rows: the line neighbours do not fit 16 bits
+    keep = hv.abs() > 0
+    w = W.Workload("square-wide", n, hi[keep].contiguous(), hj[keep].contiguous(), torch.full((int(keep.sum()),), -1.0, dtype=torch.complex128, device=dev),
+                   None, 1, 4, 4.5)
+    H, _, _, _ = run_parity(dev, oracle_mod, w, 1, 4)
+    assert H.lattice_kind == 0
+
+
 def test_anisotropic_box_lattice(dev, oracle_mod):
     """A 64 x 8 x 12 box (line of 64 rows = two tiles, plane of 8 lines = two tile rows, 12 planes: runs shorter than 64) with
     Anderson disorder: the three-dimensional lattice kernel away from the cube, 16 states = two tiles."""
