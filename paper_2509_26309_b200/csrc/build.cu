@@ -516,27 +516,45 @@ __global__ void k_sq8(int64_t n_orb, int64_t W, const int32_t *__restrict__ ocol
 }
 
 // Short rows that reach no further than 32767 rows, one real hopping value (honeycomb and square lattices with vacancies or on-site
-// disorder, chains): the whole off-diagonal structure is kept a second time as 16-bit column offsets, d16[j][r] = col_j - r (modulo
-// n_orb, so that the neighbours across a periodic boundary count as near) for the entries of row r in column order and 0 for the
-// slots a shorter row leaves empty -- 2 W bytes per row instead of the row offsets and
-// column words (4 + 4 n bytes), read fully coalesced by term_n16.cu.
-__global__ void k_near16(int64_t n_orb, int W, const uint32_t *__restrict__ orp, const int32_t *__restrict__ ocol, int16_t *d16, int32_t *status)
+// disorder, chains): the whole off-diagonal structure is kept a second time in 16-bit words, 1 + WF per row (term_n16.cu):
+//   word 0: bit 0 = the row has an entry at row + 1, bit 1 = at row - 1 (true neighbours in the row order, not across the boundary:
+//           the kernel takes them from the next lane by warp shuffle);
+//   words 1..WF: col - row of the other entries in column order, taken modulo n_orb when the plain difference does not fit (the
+//           neighbours across a periodic boundary then count as near; the kernel wraps row + d into [0, n_orb)), 0 = slot unused.
+// Layout [row / 32][word][row % 32]: a warp reads 64 contiguous bytes per word.  2 (1 + WF) bytes per row instead of the row offsets
+// and column words (4 + 4 n bytes).  pass 0 finds WF (the most far entries of any row) and checks every offset; pass 1 writes.
+__global__ void k_near16(int64_t n_orb, int pass, int WF, const uint32_t *__restrict__ orp, const int32_t *__restrict__ ocol, int16_t *d16,
+                         int32_t *status)
 {
     const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     bool bad = false;
+    int n_far = 0;
     if (r < n_orb) {
         const uint32_t b = orp[r], n = orp[r + 1] - b;
-        for (int j = 0; j < W; ++j) {
-            int64_t d = 0;
-            if ((uint32_t)j < n) d = (int64_t)(ocol[b + j] & 0x7fffffff) - r;
-            if (2 * d > n_orb) d -= n_orb;                  // taken round the periodic boundary: the kernel wraps row + d into [0, n_orb)
-            else if (2 * d < -n_orb) d += n_orb;
-            if (d > 32767 || d < -32767) { bad = true; d = 0; }
-            d16[(r >> 5) * (int64_t)(W * 32) + j * 32 + (r & 31)] = (int16_t)d;   // [32 rows][slot][row]: a warp reads 64 contiguous bytes per slot
+        const int S = 1 + WF;
+        int16_t *q = d16 + (r >> 5) * (int64_t)(S * 32) + (r & 31);
+        int flags = 0;
+        for (uint32_t j = 0; j < n; ++j) {
+            int64_t d = (int64_t)(ocol[b + j] & 0x7fffffff) - r;
+            if (d == 1) { flags |= 1; continue; }
+            if (d == -1) { flags |= 2; continue; }
+            if (d > 32767 || d < -32767) d += d < 0 ? n_orb : -n_orb;   // round the periodic boundary
+            if (d > 32767 || d < -32767 || d == 0) { bad = true; d = 0; }
+            if (pass == 1 && n_far < WF) q[(1 + n_far) * 32] = (int16_t)d;
+            ++n_far;
         }
-        bad = bad || n > (uint32_t)W;
+        if (pass == 1) {
+            q[0] = (int16_t)flags;
+            for (int j = n_far; j < WF; ++j) q[(1 + j) * 32] = 0;
+        }
     }
-    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicAdd(&status[ST_N16_BAD], 1);
+    if (pass == 0) {
+        const int m = __reduce_max_sync(0xffffffffu, n_far);
+        if ((threadIdx.x & 31) == 0) {
+            if (m > *(volatile int32_t *)&status[ST_N16_WF]) atomicMax(&status[ST_N16_WF], m);
+            if (__any_sync(0xffffffffu, bad)) atomicAdd(&status[ST_N16_BAD], 1);
+        }
+    }
 }
 constexpr int kNear16MaxW = 4;
 
@@ -562,7 +580,7 @@ PersistLayout persist_layout(int64_t n_orb, int64_t n_hop, int has_onsite, uint3
     L.diag = has_onsite ? take(sizeof(double) * (size_t)n_orb) : 0;
     L.latflag = take(sizeof(uint32_t) * ((size_t)n_orb / 32 + 2));
     L.dline = take(sizeof(uint16_t) * 8 * (size_t)kSq8MaxLine);
-    L.d16 = take(sizeof(int16_t) * kNear16MaxW * ((size_t)n_orb + 32));
+    L.d16 = take(sizeof(int16_t) * (1 + kNear16MaxW) * ((size_t)n_orb + 32));
     L.total = o;
     return L;
 }
@@ -739,14 +757,18 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
             }
             // short rows, one real value: 16-bit column offsets for term_n16.cu (every entry checked)
             const int n_off_max = H->max_row_nnz - (has_onsite ? 1 : 0);
-            if (H->single_real && n_off_max >= 1 && n_off_max <= kNear16MaxW) {
-                const int W16 = n_off_max <= 3 ? 3 : 4;
-                k_near16<<<gr, kThreads, 0, st>>>(n_orb, W16, H->orp, H->ocol, H->d16, H->status);
-                count_launches(1);
-                int32_t bad16 = 0;
-                TRY_OR_FAIL(cudaMemcpyAsync(&bad16, H->status + ST_N16_BAD, sizeof(bad16), cudaMemcpyDeviceToHost, st));
+            if (H->single_real && n_off_max >= 1 && n_off_max <= kNear16MaxW + 2) {
+                k_near16<<<gr, kThreads, 0, st>>>(n_orb, 0, 0, H->orp, H->ocol, H->d16, H->status);
+                int32_t back16[2] = {0, 0};                 // ST_N16_BAD, ST_N16_WF are neighbours
+                TRY_OR_FAIL(cudaMemcpyAsync(back16, H->status + ST_N16_BAD, sizeof(back16), cudaMemcpyDeviceToHost, st));
                 TRY_OR_FAIL(cudaStreamSynchronize(st));
-                H->near16_w = bad16 == 0 ? W16 : 0;
+                count_launches(1);
+                if (back16[0] == 0 && back16[1] <= kNear16MaxW) {
+                    const int WF = back16[1] <= 1 ? 1 : back16[1] == 2 ? 2 : 4;    // the widths term_n16.cu is instantiated for
+                    k_near16<<<gr, kThreads, 0, st>>>(n_orb, 1, WF, H->orp, H->ocol, H->d16, H->status);
+                    count_launches(1);
+                    H->near16_w = WF;
+                }
             }
             if (uniform) {
                 std::vector<std::vector<int64_t>> tup(kSampleRows, std::vector<int64_t>(n_off));
@@ -833,8 +855,8 @@ extern "C" int tbpm_ham_lattice_info(const tbpm_ham *H, int32_t *kind, size_t *b
         k = TBPM_LATTICE_SQUARE8;                             // term_sq.cu: value indices by direction of one line + the value table
         b = sizeof(uint16_t) * 8 * (size_t)H->sq8_line + sizeof(double2) * (size_t)H->n_table + (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0);
     } else if (H->near16_w > 0) {
-        k = TBPM_LATTICE_NEAR16;                              // term_n16.cu (tiles of 1-4 states): 16-bit column offsets + real diagonal
-        b = sizeof(int16_t) * (size_t)H->near16_w * (size_t)H->n_orb + (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0) + sizeof(double2);
+        k = TBPM_LATTICE_NEAR16;                              // term_n16.cu (tiles of 1-4 states): 16-bit flag word and far offsets + real diagonal
+        b = sizeof(int16_t) * (size_t)(1 + H->near16_w) * (size_t)H->n_orb + (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0) + sizeof(double2);
     }
     if (kind) *kind = k;
     if (bytes_per_term) *bytes_per_term = b;

@@ -45,7 +45,8 @@ enum StatusWord {
     ST_HALO = 7,         // widest |col - row| (circular): how far a row reaches into the vector
     ST_NREG = 8,         // rows whose entries sit exactly at the lattice offsets (k_lat_flags)
     ST_SQ8_BAD = 9,      // warps with a row that is not a site of the periodic square lattice with in-line hoppings (k_sq8)
-    ST_N16_BAD = 10      // warps with an entry further than 32767 rows from its row (k_near16)
+    ST_N16_BAD = 10,     // warps with an entry further than 32767 rows from its row, also round the boundary (k_near16)
+    ST_N16_WF = 11       // most entries of a row that are not at row +- 1 (k_near16)
 };
 
 // What the last tbpm_propagate / tbpm_ldos call of a handle left in a workspace (read by tbpm_get_state).
@@ -74,7 +75,7 @@ struct tbpm_ham {
     int64_t lat_delta[16] = {0};   // the same offsets signed, in the order of the sample row's entries (slot j -> col - row)
     int64_t n_regular = 0;         // rows that follow lat_delta exactly (bits of lat_flags)
     int64_t sq8_line = 0;          // > 0: periodic square lattice + next-nearest neighbours, line of this many rows, hoppings = dline
-    int32_t near16_w = 0;          // > 0: d16 holds the column offsets of every row, this many slots per row (term_n16.cu)
+    int32_t near16_w = 0;          // > 0: d16 holds a flag word and this many far column offsets per row (term_n16.cu)
     int32_t lat_periodic3 = 0;     // the bits were computed for the periodic three-dimensional lattice (wrapped neighbours count)
     double gershgorin = 0.0;
     int32_t n_table = 0;   // 0: kernels read complex128 values from the canonical CSR
@@ -93,7 +94,7 @@ struct tbpm_ham {
     double2 *vtab = nullptr;
     double *diag = nullptr;
     uint16_t *dline = nullptr;       // sq8_line > 0: value index of direction k at in-line position x, [x][8]
-    int16_t *d16 = nullptr;          // near16_w > 0: [row / 32][slot][row % 32] col - row (modulo n_orb) of the row's entries in column order, 0 = no entry
+    int16_t *d16 = nullptr;          // near16_w > 0: [row / 32][word][row % 32], word 0 = +-1 flags, words 1.. = far col - row (modulo n_orb) of the row's entries in column order, 0 = no entry
     uint32_t *lat_flags = nullptr;   // uniform lattices: bit r = row r follows lat_delta exactly
     int32_t *status = nullptr;
 

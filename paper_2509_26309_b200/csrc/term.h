@@ -51,8 +51,8 @@ struct TermParams {
     int64_t n_regular;     // number of such rows
     int64_t sq8_line;      // > 0: periodic square lattice with next-nearest neighbours whose hoppings depend on the in-line position
     const uint16_t *dline; // only (build.cu, k_sq8): line length in rows and the [x][8] table of value indices by direction
-    const int16_t *d16;    // short rows, one real value (build.cu, k_near16): [row / 32][slot][row % 32] col - row modulo n_orb, 0 = empty slot
-    int n16_w;             // slots per row of d16 (3 or 4), 0: none
+    const int16_t *d16;    // short rows, one real value (build.cu, k_near16): [row / 32][word][row % 32], +-1 flags | far offsets
+    int n16_w;             // far offsets per row of d16 (1, 2 or 4), 0: none
     int lat_periodic3;     // the bits are those of the periodic three-dimensional lattice (wrapped neighbours count as regular)
     int pol;               // phased kernel: cache-policy bits (1: T_k stored evict-first)
     int reverse;           // phased kernel: sweep the tiles from the last row block to the first
