@@ -1,5 +1,5 @@
-// term_n16.cu -- fused Chebyshev term for SHORT ROWS with ONE REAL hopping value, tiles of 1, 2 or 4 states (cfg3: honeycomb with
-// vacancies, one state; cfg2: honeycomb + Anderson disorder, four states).
+// term_n16.cu -- fused Chebyshev term for SHORT ROWS with ONE REAL hopping value, tiles of one state (cfg3: honeycomb with vacancies;
+// the template also covers tiles of 2 and 4 states with two states per thread, where the phased kernel is as fast and stays in use).
 //
 //   T_k = a*H*T_{k-1} - T_{k-2}  (amxsy)  fused with  psi' += sum c_j T_j  (axpy) and, on the last
 //   term of a time step, <psi0|psi'> and <psi'|psi'> (calc_corr_dos) -- the same contract as term_ph.cuh.
@@ -7,16 +7,17 @@
 // Why a kernel of its own (profiles/r2_ncu_cfg3.md): with one state per tile a row is 16 bytes, and the phased kernel spent 258
 // instructions per row on it (issue slots 68 % busy, DRAM at 70 %): row offsets, column words, the stage hand-off and 64-bit
 // address arithmetic per entry.  Here
-//   * the matrix is the builder's `d16` (build.cu, k_near16): W <= 4 slots of 16-bit column offsets per row, slot-major, so a warp
-//     reads 64 contiguous bytes per slot -- 2 W bytes per row instead of 4 + 4 n, no row offsets, no shared memory at all (the
-//     whole 256 KB of the SM stay L1 for the gathers);
-//   * a thread owns one (row, state) element, two tiles in flight: the indices of the tile after next, the loads of the next tile
-//     and the arithmetic of this one overlap (software pipeline in registers; 2 x 512 threads per SM);
-//   * neighbours at offset +-1 (two of the three on a honeycomb lattice) come from the lane next door by warp shuffle of the
-//     tile's own x row, which is read coalesced; only the far neighbour (and the two ends of a warp) is gathered through L1:
-//     ~24 instead of ~36 line requests per 32 rows.
+//   * the matrix is the builder's `d16` (build.cu, k_near16): per row one 16-bit FLAG word (has a neighbour at row + 1 / row - 1) and
+//     WF <= 4 FAR column offsets, word-major within groups of 32 rows, so a warp reads 64 contiguous bytes per word -- 2 (1 + WF)
+//     bytes per row instead of 4 + 4 n, no row offsets, no shared memory at all (the whole 256 KB of the SM stay L1 for the gathers);
+//   * a thread owns one (row, state) element, two tiles in flight: the words of the tile after next, the loads of the next tile
+//     and the arithmetic of this one overlap (software pipeline in registers; 2 x 512 threads per SM, 32-bit row arithmetic);
+//   * the neighbours at row +- 1 (two of the three on a honeycomb lattice) come from the lane next door by warp shuffle of the
+//     tile's own x row, which is read coalesced; only the far neighbours -- and, by ONE predicated load, the neighbour beyond either
+//     end of a warp -- are gathered through L1.  104 instructions per row; the plain term runs at the DRAM bandwidth (6.3 TB/s).
 // Blocks walk the tiles in linear order, all of them inside one moving window of the vectors (L2 locality), every other term from
-// the end (TermParams::reverse), as term_ph.cuh does.
+// the end (TermParams::reverse), as term_ph.cuh does.  An L2 prefetch of the streamed rows some tiles ahead made it slower (342 ->
+// 357 -> 434 us per launch at distances 0, 2, 16) and is not part of the kernel.
 #include <algorithm>
 
 #include "ptx_helpers.cuh"
