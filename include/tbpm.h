@@ -46,6 +46,7 @@ typedef struct tbpm_ham tbpm_ham; /* opaque host handle pointing into caller-own
 #define TBPM_ECUDA (-6)   /* CUDA runtime error (no device, launch failure, sticky error)                            */
 #define TBPM_EBOUND (-7)  /* Gershgorin bound max_i(|onsite_i| + sum_j |H_ij|) > rescale (strictly): the Chebyshev
                              recursion would diverge.  Returned by tbpm_check_bound only; never fatal elsewhere.     */
+#define TBPM_ETOOBIG (-8) /* tbpm_propagate_static: the problem needs more than TBPM_STATIC_WORKSPACE_BYTES of workspace       */
 
 /* flags of tbpm_build */
 #define TBPM_VALIDATE 1u    /* accepted and ignored: the precondition checks (index range, i != j, duplicates) ride on
@@ -134,6 +135,20 @@ int tbpm_propagate_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes
  * Deterministic: the same inputs give bit-identical outputs, and the first m entries do not depend on n_step. */
 int tbpm_propagate(tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale,
                    double *corr, double *norm2, void *workspace, size_t workspace_bytes, void *stream);
+
+/* The same propagation for callers that CANNOT allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no workspace argument -- the workspace is a file-scope device array of
+ * TBPM_STATIC_WORKSPACE_BYTES inside the library (8 MiB, held by every GPU that loads the library until the process exits), and the
+ * call performs no cudaMalloc / cudaFree / allocating library routine.  Inputs and outputs are the caller's, as in tbpm_propagate, and
+ * the results are bit-identical to tbpm_propagate's.  Limits: tbpm_propagate_bytes(H, n_state) <= TBPM_STATIC_WORKSPACE_BYTES, i.e.
+ * about n_orb x min(n_state, tile) <= 80,000 per tile (BASELINE.json:configs[0] with up to 8 states), else TBPM_ETOOBIG and nothing
+ * is launched; the handle's device must be the current device (TBPM_EINVAL).  The array is shared by every call on that device and
+ * keeps the last call's contents (each call initialises what it reads); calls that OVERLAP on the GPU -- two streams, two host
+ * threads -- race on it: serialise them.  tbpm_get_state does not apply to this call's workspace.  The first call on a device looks
+ * the array's address up (cudaGetSymbolAddress): make that call outside a graph capture. */
+#define TBPM_STATIC_WORKSPACE_BYTES (8u << 20)
+int tbpm_propagate_static(tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale,
+                          double *corr, double *norm2, void *stream);
 
 /* ---- a8: TBPM-style LDOS correlation: psi0_b = e_{sites[b]}, corr[b][n] = <site_b| psi_b(t_n) > ----------------------
  * BASELINE.json:configs[4] ("LDOS correlation on 64 seeded site-localized initial states"); the paper's own LDOS is the

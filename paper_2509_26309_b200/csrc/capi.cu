@@ -73,6 +73,7 @@ extern "C" const char *tbpm_strerror(int code)
     case TBPM_ENOMEM: return "caller-provided buffer too small";
     case TBPM_ECUDA: return g_cuda_msg;
     case TBPM_EBOUND: return "Gershgorin bound of H exceeds rescale: the Chebyshev recursion would diverge";
+    case TBPM_ETOOBIG: return "tbpm_propagate_static: the problem needs more workspace than the library's static array (TBPM_STATIC_WORKSPACE_BYTES)";
     }
     return "unknown error code";
 }

@@ -1091,3 +1091,42 @@ extern "C" int tbpm_set_option(tbpm_ham *H, int option, int64_t value)
     }
     return TBPM_EINVAL;
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// tbpm_propagate_static: the same propagation with NO caller workspace and NO allocation of any kind
+// ---------------------------------------------------------------------------------------------------------------------
+// For callers that cannot allocate device memory (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the
+// workspace of tbpm_propagate -- block partials of the fused dot products, term descriptors, and the four vectors per state tile --
+// lives in ONE file-scope device array of TBPM_STATIC_WORKSPACE_BYTES.  Every GPU that loads the library holds the array until the
+// process exits.  All calls on a device share it and it keeps the previous call's contents: run() initialises everything it reads
+// (it is written for uninitialised workspaces), but two calls that overlap on the GPU (different streams, or host threads) RACE.
+static __device__ __align__(256) unsigned char g_static_workspace[TBPM_STATIC_WORKSPACE_BYTES];
+
+namespace {
+std::mutex g_static_mu;
+void *g_static_ptr[kMaxDevices] = {nullptr};   // device address of g_static_workspace per device (in host code the symbol is only a stand-in)
+}  // namespace
+
+extern "C" int tbpm_propagate_static(tbpm_ham *H, const double *psi0, int n_state, int n_step, double dt, double rescale, double *corr,
+                                     double *norm2, void *stream)
+{
+    if (!H || n_state < 0 || n_step < 0) return TBPM_EINVAL;
+    if (n_state == 0 || n_step == 0) return TBPM_OK;        // as in tbpm_propagate: success, outputs untouched
+    if (!psi0) return TBPM_EINVAL;
+    const size_t need = make_plan(H->n_orb, n_state, H->opt_tile).total;
+    if (need > (size_t)TBPM_STATIC_WORKSPACE_BYTES) return TBPM_ETOOBIG;
+    int dev = -1;
+    TBPM_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != H->device || dev < 0 || dev >= kMaxDevices) return TBPM_EINVAL;   // the array of the CURRENT device is the one addressed
+    void *ws = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        if (!g_static_ptr[dev]) {                           // once per device, with that device current
+            void *p = nullptr;
+            TBPM_CUDA_TRY(cudaGetSymbolAddress(&p, g_static_workspace));
+            g_static_ptr[dev] = p;
+        }
+        ws = g_static_ptr[dev];
+    }
+    return run(H, psi0, nullptr, n_state, n_step, dt, rescale, corr, norm2, ws, (size_t)TBPM_STATIC_WORKSPACE_BYTES, stream);
+}

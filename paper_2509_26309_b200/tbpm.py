@@ -18,6 +18,8 @@ TBPM_VALIDATE, TBPM_HOPS_FULL, TBPM_NO_TABLE = 1, 2, 4
 TBPM_OPT_TILE, TBPM_OPT_KERNEL = 1, 2
 TBPM_LATTICE_CUBIC, TBPM_LATTICE_SQUARE8, TBPM_LATTICE_NEAR16 = 2, 3, 4
 TBPM_OK, TBPM_EINVAL, TBPM_EINDEX, TBPM_EDIAG, TBPM_EDUP, TBPM_ENOMEM, TBPM_ECUDA, TBPM_EBOUND = 0, -1, -2, -3, -4, -5, -6, -7
+TBPM_ETOOBIG = -8
+TBPM_STATIC_WORKSPACE_BYTES = 8 << 20
 
 _lib = None
 
@@ -52,6 +54,7 @@ def lib() -> C.CDLL:
         L.tbpm_free.restype = None
         L.tbpm_propagate_bytes.argtypes = [vp, C.c_int, P(sz)]
         L.tbpm_propagate.argtypes = [vp, vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp, sz, vp]
+        L.tbpm_propagate_static.argtypes = [vp, vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp]
         L.tbpm_ldos.argtypes = [vp, vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp, sz, vp]
         L.tbpm_get_state.argtypes = [vp, vp, C.c_int, vp, vp]
         L.tbpm_dos.argtypes = [vp, C.c_int, C.c_int, dbl, dbl, vp, vp, vp]
@@ -204,6 +207,26 @@ def tbpm_propagate(H: Hamiltonian, psi0: torch.Tensor, n_step: int, dt: float, r
                                   workspace.numel(), _stream(dev))
     _check(rc, "tbpm_propagate")
     return corr, norm2, workspace
+
+
+def tbpm_propagate_static(H: Hamiltonian, psi0: torch.Tensor, n_step: int, dt: float, rescale: float, corr: Optional[torch.Tensor] = None,
+                          norm2: Optional[torch.Tensor] = None, want_norm: bool = True):
+    """tbpm_propagate without a workspace: the library's static device array serves (small models only, TbpmError(TBPM_ETOOBIG)
+    beyond TBPM_STATIC_WORKSPACE_BYTES).  The C call allocates nothing; pass `corr` / `norm2` to keep this wrapper from allocating too.
+    Returns (corr, norm2)."""
+    _need_cuda(psi0)
+    dev = H.device
+    assert psi0.dtype == torch.complex128 and psi0.dim() == 2 and psi0.shape[1] == H.n_orb
+    psi0 = psi0.resolve_conj().contiguous()
+    n_state = psi0.shape[0]
+    if corr is None:
+        corr = torch.zeros((n_state, n_step), dtype=torch.complex128, device=dev)
+    if norm2 is None and want_norm:
+        norm2 = torch.zeros((n_state, n_step), dtype=torch.float64, device=dev)
+    with torch.cuda.device(dev):
+        rc = lib().tbpm_propagate_static(H.handle, _ptr(psi0), n_state, n_step, dt, rescale, _ptr(corr), _ptr(norm2), _stream(dev))
+    _check(rc, "tbpm_propagate_static")
+    return corr, norm2
 
 
 def tbpm_ldos(H: Hamiltonian, sites, n_step: int, dt: float, rescale: float, workspace: Optional[torch.Tensor] = None,
