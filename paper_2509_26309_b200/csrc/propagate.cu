@@ -549,6 +549,7 @@ int launch_term_t(const TermParams &p, int num_sms, cudaStream_t st, int *grid_o
 // 2: no lattice kernel; 3: of the lattice kernels only term_rw.
 int launch_term(int bt, bool table, int kernel_opt, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 {
+    if (kernel_opt == 4) kernel_opt = 0;                  // 4 only switches the two-terms-per-sweep path of run() off
     const bool general_only = kernel_opt == 1;
     if (table && kernel_opt == 0 && term_l3_supported(bt, p)) return launch_term_l3(p, num_sms, st, grid_out);
     if (table && kernel_opt == 0 && term_sq_supported(bt, p)) return launch_term_sq(p, num_sms, st, grid_out);
@@ -610,6 +611,56 @@ void step_terms(const TermParams &base, int K, const std::vector<double> &cf, do
     }
 }
 
+// The same time step with TWO terms per launch (term_sq2.cu).  ops[i].pair: launch_pair_sq, else launch_term (only a leading single
+// term when K - 1 is odd).  Buffers: psi (T_0), t1, and the two extra vectors e1, e2; a pair reads two of the four and writes the
+// other two (T_{k-2} is read with a halo, so nothing is updated in place).  psi' (acc) is touched when the oldest term not yet added
+// would otherwise leave the pair's window {k-2 .. k+1}: every second pair, four terms at a time.
+struct StepOp { bool pair; TermParams tp; };
+void step_pairs(const TermParams &base, int K, const std::vector<double> &cf, double rescale, double2 *psi, double2 *t1, double2 *acc,
+                double2 *e1, double2 *e2, std::vector<StepOp> &ops)
+{
+    auto C = [&](int k) { return make_double2(cf[2 * k], cf[2 * k + 1]); };
+    const double2 zero = make_double2(0.0, 0.0);
+    ops.clear();
+    int oldest = 0;                                       // lowest term not yet added to psi' (terms oldest .. k - 1 are pending)
+    bool any_flush = false;
+    double2 *X = psi, *Y = t1, *F1 = e1, *F2 = e2;        // T_{k-1}, T_{k-2}, and the two buffers free to be written
+    int k = 1;
+    if ((K - 1) % 2 == 1) {                               // odd number of terms: T_1 on its own, in t1
+        StepOp op{false, base};
+        op.tp.x = psi; op.tp.y = t1; op.tp.acc = acc; op.tp.a = 1.0 / rescale; op.tp.n_acc = 0; op.tp.flags = F_WRITE_Y; op.tp.reverse = 0;
+        ops.push_back(op);
+        X = t1; Y = psi;
+        k = 2;
+    }
+    for (; k + 1 < K; k += 2) {
+        StepOp op{true, base};
+        TermParams &tp = op.tp;
+        tp.x = X; tp.y = Y; tp.out1 = F1; tp.out2 = F2; tp.acc = acc;
+        tp.a = (k == 1 ? 1.0 : 2.0) / rescale;
+        tp.a2 = 2.0 / rescale;
+        int flags = k >= 2 ? F_SUB_Y : 0;
+        const bool last = k + 1 == K - 1;
+        tp.n_acc = 0;
+        tp.ca = tp.cb = tp.cc = tp.cd = zero;
+        if (oldest < k || last) {                         // terms oldest .. k + 1, all inside the window (oldest >= k - 2)
+            tp.n_acc = k + 2 - oldest;
+            tp.ca = C(k + 1); tp.cb = C(k);
+            if (oldest <= k - 1) tp.cc = C(k - 1);
+            if (oldest <= k - 2) tp.cd = C(k - 2);
+            if (!any_flush) flags |= F_ACC_INIT;
+            any_flush = true;
+            oldest = k + 2;
+        }
+        if (last) flags |= F_REDUCE;
+        tp.flags = flags;
+        tp.reverse = 0;
+        ops.push_back(op);
+        double2 *oX = X, *oY = Y;
+        Y = F1; X = F2; F1 = oX; F2 = oY;
+    }
+}
+
 // The matrix side of a term launch: everything of TermParams that comes from the handle.
 TermParams matrix_params(const tbpm_ham *H, double *partial)
 {
@@ -639,6 +690,15 @@ TermParams matrix_params(const tbpm_ham *H, double *partial)
     mp.pf_lead = H->n_lat_off > 0 ? H->lat_off[H->n_lat_off - 1] : H->halo_rows;
     if (knob("pf_lead", -1) >= 0) mp.pf_lead = knob("pf_lead", -1);
     return mp;
+}
+
+// Two extra vectors of a full tile behind the plan (shared by the tiles, which run one after the other) when the two-terms-per-sweep
+// kernel applies to this Hamiltonian; run() falls back to one term per sweep when the caller's workspace lacks them.
+size_t pair_extra_bytes(const tbpm_ham *H, const Plan &P)
+{
+    if (P.tile != 8 || H->n_table <= 0) return 0;
+    const TermParams mp = matrix_params(H, nullptr);
+    return pair_sq_supported(8, mp) ? 2 * P.full_vec : 0;
 }
 
 // Shared body of tbpm_propagate (psi0 != NULL) and tbpm_ldos (sites != NULL).
@@ -679,6 +739,7 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
     const bool table = H->n_table > 0;
     TermParams tp = matrix_params(H, partial);
     const bool reverse_odd = knob("rev", 1) != 0;         // odd terms sweep backwards (term_ph.cuh)
+    const int kernel_opt = H->opt_kernel;
 
     std::vector<TermParams> term;
     for (int t = 0; t < P.n_tile; ++t) {
@@ -718,6 +779,10 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
             count_launches(1);
         };
         if (qe && n_el > 0) qe_add(buf[start_slot], 0);
+        // two terms per sweep where term_sq2.cu applies (full tiles of 8 states, default kernel choice, room for the two extra vectors)
+        const bool pairs = !qe && table && H->opt_kernel == 0 && K >= 3 && bt == 8 && n_el > 0 && pair_sq_supported(bt, tp) &&
+                           workspace_bytes >= P.total + 2 * P.full_vec;
+        std::vector<StepOp> ops;
         auto one_step = [&](int n, cudaStream_t s2) -> int {
             double2 *psi = buf[slot], *t1 = buf[(slot + 1) % 3], *acc = buf[(slot + 2) % 3];
             int grid = 1;
@@ -727,9 +792,17 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
                 t0.ca = make_double2(cf[0], cf[1]); t0.n_acc = 1; t0.flags = F_SKIP_H | F_ACC_INIT | F_REDUCE;
                 if ((rc = launch_term(bt, table, 1, t0, H->num_sms, s2, &grid))) return rc;
             }
-            step_terms(tp, K, cf, rescale, reverse_odd, psi, t1, acc, term);
-            for (int k = 1; k < K; ++k)
-                if ((rc = launch_term(bt, table, H->opt_kernel, term[k], H->num_sms, s2, &grid))) return rc;
+            if (pairs) {
+                step_pairs(tp, K, cf, rescale, psi, t1, acc, reinterpret_cast<double2 *>(W + P.total),
+                           reinterpret_cast<double2 *>(W + P.total + P.full_vec), ops);
+                for (const StepOp &op : ops)
+                    if ((rc = op.pair ? launch_pair_sq(op.tp, H->num_sms, s2, &grid) : launch_term(bt, table, 0, op.tp, H->num_sms, s2, &grid)))
+                        return rc;
+            } else {
+                step_terms(tp, K, cf, rescale, reverse_odd, psi, t1, acc, term);
+                for (int k = 1; k < K; ++k)
+                    if ((rc = launch_term(bt, table, kernel_opt, term[k], H->num_sms, s2, &grid))) return rc;
+            }
             k_reduce_final<<<bt, 96, 0, s2>>>(partial, grid, bt, n_valid, state0, n_step, n, corr, norm2);
             count_launches(1);
             return TBPM_OK;
@@ -813,7 +886,8 @@ int run(tbpm_ham *H, const double *psi0, const int64_t *sites, int n_state, int 
 extern "C" int tbpm_propagate_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes)
 {
     if (!H || n_state < 0 || !workspace_bytes) return TBPM_EINVAL;
-    *workspace_bytes = make_plan(H->n_orb, n_state, H->opt_tile).total;
+    const Plan P = make_plan(H->n_orb, n_state, H->opt_tile);
+    *workspace_bytes = P.total + pair_extra_bytes(H, P);
     return TBPM_OK;
 }
 
@@ -1085,7 +1159,7 @@ extern "C" int tbpm_set_option(tbpm_ham *H, int option, int64_t value)
         H->opt_tile = (int)value;
         return TBPM_OK;
     case TBPM_OPT_KERNEL:
-        if (value < 0 || value > 3) return TBPM_EINVAL;
+        if (value < 0 || value > 4) return TBPM_EINVAL;
         H->opt_kernel = (int)value;
         return TBPM_OK;
     }

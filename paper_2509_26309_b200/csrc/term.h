@@ -33,6 +33,10 @@ struct TermParams {
     double *partial;       // [grid][BT][3]
     double a;              // 1/s (k = 1) or 2/s
     double2 ca, cb, cc;    // coefficients of T_k, T_{k-1}, T_{k-2} in this flush
+    // two terms per sweep (term_sq2.cu): T_k -> out1, T_{k+1} = a2*H*T_k - T_{k-1} -> out2; ca, cb, cc, cd then belong to T_{k+1} .. T_{k-2}
+    double2 *out1, *out2;
+    double a2;
+    double2 cd;
     int n_acc;             // 0: psi' untouched; 1..3 terms added
     int flags;
     int n_table;           // entries of vtab (kernel layout)
@@ -120,6 +124,10 @@ int launch_term_rw(const TermParams &p, int num_sms, cudaStream_t st, int *grid_
 // values depend on the in-line position only; neither column words nor value indices are read per row.
 bool term_sq_supported(int bt, const TermParams &p);
 int launch_term_sq(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
+
+// Two terms per sweep on the same lattice without a diagonal (term_sq2.cu); see launch_pair_sq for the meaning of the fields.
+bool pair_sq_supported(int bt, const TermParams &p);
+int launch_pair_sq(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
 // Three-dimensional lattice kernel (term_l3.cu): tiles of 8 states on lattices with offsets {+-1, +-S1, +-S2} and one real hopping
 // value (simple cubic and its anisotropic relatives); two-dimensional tiles with TMA-fed halos, walked along S2.

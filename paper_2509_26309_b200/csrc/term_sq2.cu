@@ -1,0 +1,407 @@
+// term_sq2.cu -- TWO Chebyshev terms per sweep on the periodic square lattice with next-nearest neighbours and in-line hoppings
+// (BASELINE.json:configs[3]; the lattice of term_sq.cu, tiles of 8 interleaved states, no diagonal).
+//
+//   T_k     = a1*H*T_{k-1} - T_{k-2}      (amxsy)
+//   T_{k+1} = a2*H*T_k     - T_{k-1}
+//   psi'   += ca*T_{k+1} + cb*T_k + cc*T_{k-1} + cd*T_{k-2}   (the axpy of PAPER.md:440 for up to FOUR terms at once), and on the last
+//   pair of a time step <psi0|psi'>, <psi'|psi'> (calc_corr_dos).
+//
+// Why: term_sq.cu runs at the DRAM bandwidth (profiles/r2_ncu_cfg4.md), so the only way on is to move fewer bytes.  One term reads
+// T_{k-1} and T_{k-2} and writes T_k: 3 vectors.  Here a block walks DOWN the lattice at a fixed in-line position, as in term_sq.cu,
+// and keeps the last three lines of T_k it has just computed in a second shared-memory ring: T_{k+1} of line L - 1 follows as soon
+// as T_k of line L exists.  A pair of terms then reads 2 vectors and writes 2 (4 instead of 6), and psi' is touched once per FOUR
+// terms instead of three: 52 instead of 74 vector transfers per time step of 20 terms.
+//   halo     T_{k+1} on rows [x0, x0 + 128) needs T_k on [x0 - 1, x0 + 129): the block computes those two extra rows itself (65 row
+//            pairs instead of 64: +1.6 %), from T_{k-1} on [x0 - 2, x0 + 130) -- ring slots of 132 rows -- and T_{k-2} on 130 rows;
+//            along the walk it computes T_k on one extra line above and below its run of 64 lines (+3 %).
+//   buffers  T_{k-2} is now read with a halo, so T_k cannot overwrite it in place: both results go to buffers of their own
+//            (TermParams::out1 / out2), which the next pair reads while it writes the two this pair read.
+//   sync     consumers: 9 warps (65 row pairs x 4 lanes; thread = 2 states of 2 adjacent rows, the values of those two rows in
+//            registers for a whole run, serving both stages).  Per line: stage 1 -> named barrier (the line of T_k is in the ring)
+//            -> stage 2.  Ring B slot (it % 4) is rewritten two barriers after its last reader passed one: no further hand-shake.
+#include <algorithm>
+
+#include "term_ph.cuh"
+
+namespace tbpm_detail {
+namespace sq2 {
+
+using namespace ph;
+
+constexpr int kBT = 8, kNW = 9, kConsumers = kNW * 32, kThreads = kConsumers + 64;
+constexpr int kR = 128;                                    // rows of a tile that this block OWNS (stores)
+constexpr int kPairs = kR / 2 + 1;                         // row pairs computed in stage 1: tile rows (2p - 1, 2p), p = 0 .. 64
+constexpr int kRowBytes = kBT * 16;
+constexpr int kSlotRows = kR + 4;                          // tile rows -2 .. 129
+constexpr int kSlotBytes = kSlotRows * kRowBytes;          // 16,896
+constexpr int kYRows = kR + 2;                             // tile rows -1 .. 128
+constexpr int kYBytes = kYRows * kRowBytes;                // 16,640
+constexpr int kMaxRing = 8;
+constexpr int kNB = 4;                                     // slots of the T_k ring
+constexpr int kCH = 8;
+
+struct Geom {
+    int64_t W, d0, n_lines;
+    int len, n_ring, n_stage;
+};
+
+struct RingPos {
+    uint32_t i, ph;
+    __device__ __forceinline__ void adv(uint32_t nr) { if (++i == nr) { i = 0; ph ^= 1u; } }
+};
+
+__device__ __forceinline__ void lds_c(double2 &v, uint32_t a)
+{
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+}
+__device__ __forceinline__ void sts_c(uint32_t a, double2 v)
+{
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v.x), "d"(v.y) : "memory");
+}
+
+struct Row2 { double2 a, b; };                             // the thread's two states of one row (slot a / slot b, see `par`)
+struct Out4 { double2 Aa, Ab, Ba, Bb; };                   // rows A and B, slots a and b
+
+// H * v on the thread's two rows from three consecutive lines held in 132-row slots (bp / bo / bn: address of slot row 2p of the
+// line above / the own line / the line below); xA, xB return the own rows of the middle line.
+__device__ __forceinline__ void apply_h(uint32_t bp, uint32_t bo, uint32_t bn, uint32_t oa, uint32_t ob, const double2 (&vA)[kCH],
+                                        const double2 (&vB)[kCH], Out4 &h, Row2 &xA, Row2 &xB)
+{
+    h.Aa = h.Ab = h.Ba = h.Bb = make_double2(0.0, 0.0);
+    Row2 r[4];
+    auto load4 = [&](uint32_t base) {                      // rows A - 1, A, B, B + 1 of one line
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { lds_c(r[i].a, base + (uint32_t)i * kRowBytes + oa); lds_c(r[i].b, base + (uint32_t)i * kRowBytes + ob); }
+    };
+    load4(bp);                                             // line above: directions 0, 1, 2 = in-line offsets -1, 0, +1
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        cfma(h.Aa, vA[k], r[k].a); cfma(h.Ab, vA[k], r[k].b);
+        cfma(h.Ba, vB[k], r[k + 1].a); cfma(h.Bb, vB[k], r[k + 1].b);
+    }
+    load4(bo);                                             // own line: directions 3, 4 = -1, +1; r[1], r[2] are the own rows
+    cfma(h.Aa, vA[3], r[0].a); cfma(h.Ab, vA[3], r[0].b);
+    cfma(h.Ba, vB[3], r[1].a); cfma(h.Bb, vB[3], r[1].b);
+    cfma(h.Aa, vA[4], r[2].a); cfma(h.Ab, vA[4], r[2].b);
+    cfma(h.Ba, vB[4], r[3].a); cfma(h.Bb, vB[4], r[3].b);
+    xA = r[1]; xB = r[2];
+    load4(bn);                                             // line below: directions 5, 6, 7
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        cfma(h.Aa, vA[5 + k], r[k].a); cfma(h.Ab, vA[5 + k], r[k].b);
+        cfma(h.Ba, vB[5 + k], r[k + 1].a); cfma(h.Bb, vB[5 + k], r[k + 1].b);
+    }
+}
+
+template <bool FLUSH, bool REDUCE>
+__global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, const Geom g)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ __align__(8) uint64_t bars[2 * kMaxStages + 2 * kMaxRing];   // stage full | stage empty | ring full | ring empty
+    __shared__ double red_s[REDUCE ? kNW : 1][REDUCE ? kBT : 1][3];
+
+    const int tid = threadIdx.x;
+    const bool sub_y = p.flags & F_SUB_Y;                  // stage 1 subtracts T_{k-2}: always, except on the pair (1, 2)
+    const bool need_acc = FLUSH && !(p.flags & F_ACC_INIT);
+    const int S = g.n_stage;
+    const uint32_t NA = (uint32_t)g.n_ring;
+    const uint32_t bar0 = smem_u32(bars), smem0 = smem_u32(smem);
+    const uint32_t b_sfull = bar0, b_sempty = bar0 + 8 * kMaxStages, b_rfull = bar0 + 16 * kMaxStages, b_rempty = b_rfull + 8 * kMaxRing;
+    const uint32_t ringA0 = smem0, ringB0 = ringA0 + NA * kSlotBytes, stage0 = ringB0 + kNB * kSlotBytes;
+
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) { mbar_init(b_sfull + 8 * s, 1); mbar_init(b_sempty + 8 * s, kNW); }
+        for (uint32_t s = 0; s < NA; ++s) { mbar_init(b_rfull + 8 * s, 1); mbar_init(b_rempty + 8 * s, kNW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // Runs: run u covers in-line position u % d0 of the lines [(u / d0) * len, ...); dealt to the blocks round-robin.
+    const int64_t n_chunks = (g.n_lines + g.len - 1) / g.len;
+    const int64_t n_runs = g.d0 * n_chunks;
+    struct Run { int64_t line0, pos; int len; };
+    auto run_of = [&](int64_t u) -> Run {
+        Run r;
+        const int64_t chunk = u / g.d0;
+        r.pos = u - chunk * g.d0;
+        r.line0 = chunk * g.len;
+        r.len = (int)min((int64_t)g.len, g.n_lines - r.line0);
+        return r;
+    };
+    auto wrap_line = [&](int64_t line) -> int64_t { return line < 0 ? line + g.n_lines : (line >= g.n_lines ? line - g.n_lines : line); };
+
+    if (tid >= kConsumers) {
+        // ------------------------------- producers: one thread of each of the two producer warps -------------------------------
+        if ((tid & 31) != 0) return;
+        // `halo` rows on either side of the tile's 128, taken round the periodic line
+        auto load_rows = [&](uint32_t dst, const double2 *line_base, int64_t x0, int halo, uint32_t full) {
+            const bool wrap_lo = x0 == 0, wrap_hi = x0 + kR == g.W;
+            const int lo = wrap_lo ? 0 : -halo, hi = wrap_hi ? kR : kR + halo;
+            bulk_g2s(dst + (uint32_t)(lo + halo) * kRowBytes, line_base + (x0 + lo) * kBT, (uint32_t)(hi - lo) * kRowBytes, full);
+            if (wrap_lo) bulk_g2s(dst, line_base + (g.W - halo) * kBT, (uint32_t)halo * kRowBytes, full);
+            if (wrap_hi) bulk_g2s(dst + (uint32_t)(kR + halo) * kRowBytes, line_base, (uint32_t)halo * kRowBytes, full);
+        };
+        if (tid == kConsumers) {
+            RingPos rp{0u, 1u};
+            for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
+                const Run r = run_of(u);
+                for (int j = -2; j < r.len + 2; ++j) {     // T_{k-1}: lines line0 - 2 .. line0 + len + 1, rows x0 - 2 .. x0 + 129
+                    mbar_wait(b_rempty + 8 * rp.i, rp.ph);
+                    const uint32_t full = b_rfull + 8 * rp.i;
+                    mbar_expect_tx(full, kSlotBytes);
+                    load_rows(ringA0 + rp.i * kSlotBytes, p.x + wrap_line(r.line0 + j) * g.W * kBT, r.pos * kR, 2, full);
+                    rp.adv(NA);
+                }
+            }
+        } else if (sub_y) {
+            int s = 0;
+            uint32_t sph = 1;
+            for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
+                const Run r = run_of(u);
+                for (int j = -1; j < r.len + 1; ++j) {     // T_{k-2}: lines line0 - 1 .. line0 + len, rows x0 - 1 .. x0 + 128
+                    mbar_wait(b_sempty + 8 * s, sph);
+                    const uint32_t full = b_sfull + 8 * s;
+                    mbar_expect_tx(full, kYBytes);
+                    load_rows(stage0 + (uint32_t)s * kYBytes, p.y + wrap_line(r.line0 + j) * g.W * kBT, r.pos * kR, 1, full);
+                    if (++s == S) { s = 0; sph ^= 1u; }
+                }
+            }
+        }
+        return;
+    }
+
+    // ---------------------------------------------------- consumer warps ----------------------------------------------------
+    // thread = states 2q, 2q + 1 of the tile rows A = 2 pr - 1 and B = 2 pr (pr = 0 .. 64: the tile's 128 rows and one halo row on
+    // either side); "slot a" of a thread is state 2q + par, "slot b" state 2q + 1 - par (conflict-free 128-bit accesses, term_sq.cu).
+    const bool act = (tid >> 2) < kPairs;                  // the last warp holds one pair; its other lanes only keep the barriers company
+    const int pr = act ? (tid >> 2) : kPairs - 1, q = tid & 3, par = pr & 1;
+    const bool okA = act && pr >= 1, okB = act && pr < kR / 2;   // rows that belong to the tile (stored)
+    const uint32_t oa = (uint32_t)(2 * q + par) * 16u, ob = (uint32_t)(2 * q + 1 - par) * 16u;
+    const uint32_t rows2p = (uint32_t)(2 * pr) * kRowBytes;      // 132-row slots: slot row 2p = tile row A - 1; 130-row stage: row 2p = A
+    double2 vA[kCH], vB[kCH];                              // hopping values of the two rows by direction, kept for a whole run
+    double sa_re = 0.0, sa_im = 0.0, sa_nn = 0.0, sb_re = 0.0, sb_im = 0.0, sb_nn = 0.0;
+    Row2 partA, partB;                                     // cc*T_{k-1} + cd*T_{k-2} on the rows of the line that stage 2 takes next
+    partA.a = partA.b = partB.a = partB.b = make_double2(0.0, 0.0);
+
+    RingPos a0{0u, 0u}, a1{1u % NA, 0u}, a2{2u % NA, 0u};  // ring A loads holding the line above / the own line / the line below of stage 1
+    int s = 0;
+    uint32_t sph = 0;
+    uint32_t it = 0;                                       // lines this block has taken: T_k of line `it` sits in ring B slot it % 4
+
+#pragma unroll 1
+    for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
+        const Run run = run_of(u);
+        {   // the values of the thread's two rows: dline[x][direction] -> table entry (+ conjugate bit); the same on every line
+            int64_t xa = run.pos * kR + 2 * pr - 1, xb = xa + 1;
+            if (xa < 0) xa += g.W;
+            if (xb >= g.W) xb -= g.W;
+            const uint4 ia = __ldg(reinterpret_cast<const uint4 *>(p.dline + xa * kCH));
+            const uint4 ib = __ldg(reinterpret_cast<const uint4 *>(p.dline + xb * kCH));
+            const uint32_t wa[4] = {ia.x, ia.y, ia.z, ia.w}, wb[4] = {ib.x, ib.y, ib.z, ib.w};
+#pragma unroll
+            for (int k = 0; k < kCH; ++k) {
+                const uint32_t ida = (wa[k >> 1] >> ((k & 1) * 16)) & 0xffffu, idb = (wb[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
+                vA[k] = table_value(__ldg(p.vtab + (ida & 0x7fffu)), ida);
+                vB[k] = table_value(__ldg(p.vtab + (idb & 0x7fffu)), idb);
+            }
+        }
+        const int64_t rowA0 = run.pos * kR + 2 * pr - 1;   // in-line position of row A
+#pragma unroll 1
+        for (int i = 0; i < run.len + 2; ++i, ++it) {
+            // stage 1 takes line line0 - 1 + i (stored when it is one of the run's), stage 2 line line0 - 2 + i (when i >= 2)
+            const bool st2 = i >= 2;
+            const int64_t e2A = ((run.line0 + i - 2) * g.W + rowA0) * kBT + 2 * q, e2B = e2A + kBT;
+            // ---- stage 2's operands that are not staged (HBM latency: issue first)
+            CVec<2> aoldA, aoldB, zA, zB;
+            if (FLUSH) { aoldA.stream_if(p.acc + e2A, st2 && okA && need_acc); aoldB.stream_if(p.acc + e2B, st2 && okB && need_acc); }
+            if (REDUCE) { zA.stream_if(p.psi0 + e2A, st2 && okA); zB.stream_if(p.psi0 + e2B, st2 && okB); }
+            if (i == 0) {
+                mbar_wait(b_rfull + 8 * a0.i, a0.ph);
+                mbar_wait(b_rfull + 8 * a1.i, a1.ph);
+            }
+            mbar_wait(b_rfull + 8 * a2.i, a2.ph);
+            if (sub_y) mbar_wait(b_sfull + 8 * s, sph);
+            const uint32_t sa0 = ringA0 + a0.i * kSlotBytes + rows2p, sa1 = ringA0 + a1.i * kSlotBytes + rows2p,
+                           sa2 = ringA0 + a2.i * kSlotBytes + rows2p, sy = stage0 + (uint32_t)s * kYBytes + rows2p;
+            uint32_t rel;
+            {   // ---- stage 1: T_k = a1 * H * T_{k-1} - T_{k-2} on rows A, B of line line0 - 1 + i
+                Out4 h;
+                Row2 xA, xB;
+                apply_h(sa0, sa1, sa2, oa, ob, vA, vB, h, xA, xB);
+                h.Aa.x *= p.a; h.Aa.y *= p.a; h.Ab.x *= p.a; h.Ab.y *= p.a; h.Ba.x *= p.a; h.Ba.y *= p.a; h.Bb.x *= p.a; h.Bb.y *= p.a;
+                if (sub_y) {
+                    Row2 yA, yB;
+                    lds_c(yA.a, sy + oa); lds_c(yA.b, sy + ob); lds_c(yB.a, sy + kRowBytes + oa); lds_c(yB.b, sy + kRowBytes + ob);
+                    h.Aa.x -= yA.a.x; h.Aa.y -= yA.a.y; h.Ab.x -= yA.b.x; h.Ab.y -= yA.b.y;
+                    h.Ba.x -= yB.a.x; h.Ba.y -= yB.a.y; h.Bb.x -= yB.b.x; h.Bb.y -= yB.b.y;
+                }
+                rel = (uint32_t)(__double2hiint(h.Aa.x) ^ __double2hiint(h.Ab.x) ^ __double2hiint(h.Ba.x) ^ __double2hiint(h.Bb.x));
+                const uint32_t wb = ringB0 + (it % kNB) * kSlotBytes + rows2p + kRowBytes;   // slot rows 2p + 1, 2p + 2 = rows A, B
+                if (act) { sts_c(wb + oa, h.Aa); sts_c(wb + ob, h.Ab); sts_c(wb + kRowBytes + oa, h.Ba); sts_c(wb + kRowBytes + ob, h.Bb); }
+                if (!REDUCE && i >= 1 && i <= run.len) {   // T_k of the run's own lines: read by the next pair, a whole sweep later
+                    const int64_t e1A = ((run.line0 + i - 1) * g.W + rowA0) * kBT + 2 * q;
+                    CVec<2> out;
+                    if (okA) { out.v[0] = par ? h.Ab : h.Aa; out.v[1] = par ? h.Aa : h.Ab; out.st_stream(p.out1 + e1A); }
+                    if (okB) { out.v[0] = par ? h.Bb : h.Ba; out.v[1] = par ? h.Ba : h.Bb; out.st_stream(p.out1 + e1A + kBT); }
+                }
+            }
+            asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");   // line `it` of T_k is complete in ring B
+            if (st2) {
+                // ---- stage 2: T_{k+1} = a2 * H * T_k - T_{k-1} on rows A, B of line line0 - 2 + i (T_k lines it - 2, it - 1, it)
+                const uint32_t sb0 = ringB0 + ((it - 2) % kNB) * kSlotBytes + rows2p, sb1 = ringB0 + ((it - 1) % kNB) * kSlotBytes + rows2p,
+                               sb2 = ringB0 + (it % kNB) * kSlotBytes + rows2p;
+                Out4 h;
+                Row2 tA, tB, xA, xB;                       // T_k and T_{k-1} on the own rows
+                apply_h(sb0, sb1, sb2, oa, ob, vA, vB, h, tA, tB);
+                lds_c(xA.a, sa0 + kRowBytes + oa); lds_c(xA.b, sa0 + kRowBytes + ob);
+                lds_c(xB.a, sa0 + 2 * kRowBytes + oa); lds_c(xB.b, sa0 + 2 * kRowBytes + ob);
+                h.Aa.x = fma(p.a2, h.Aa.x, -xA.a.x); h.Aa.y = fma(p.a2, h.Aa.y, -xA.a.y); h.Ab.x = fma(p.a2, h.Ab.x, -xA.b.x); h.Ab.y = fma(p.a2, h.Ab.y, -xA.b.y);
+                h.Ba.x = fma(p.a2, h.Ba.x, -xB.a.x); h.Ba.y = fma(p.a2, h.Ba.y, -xB.a.y); h.Bb.x = fma(p.a2, h.Bb.x, -xB.b.x); h.Bb.y = fma(p.a2, h.Bb.y, -xB.b.y);
+                rel ^= (uint32_t)(__double2hiint(h.Aa.x) ^ __double2hiint(h.Ab.x) ^ __double2hiint(h.Ba.x) ^ __double2hiint(h.Bb.x));
+                CVec<2> out;
+                if (!REDUCE) {
+                    if (okA) { out.v[0] = par ? h.Ab : h.Aa; out.v[1] = par ? h.Aa : h.Ab; out.st_stream(p.out2 + e2A); }
+                    if (okB) { out.v[0] = par ? h.Bb : h.Ba; out.v[1] = par ? h.Ba : h.Bb; out.st_stream(p.out2 + e2B); }
+                }
+                if (FLUSH) {
+                    double2 aAa = par ? aoldA.v[1] : aoldA.v[0], aAb = par ? aoldA.v[0] : aoldA.v[1];
+                    double2 aBa = par ? aoldB.v[1] : aoldB.v[0], aBb = par ? aoldB.v[0] : aoldB.v[1];
+                    aAa.x += partA.a.x; aAa.y += partA.a.y; aAb.x += partA.b.x; aAb.y += partA.b.y;
+                    aBa.x += partB.a.x; aBa.y += partB.a.y; aBb.x += partB.b.x; aBb.y += partB.b.y;
+                    cfma(aAa, p.cb, tA.a); cfma(aAb, p.cb, tA.b); cfma(aBa, p.cb, tB.a); cfma(aBb, p.cb, tB.b);
+                    cfma(aAa, p.ca, h.Aa); cfma(aAb, p.ca, h.Ab); cfma(aBa, p.ca, h.Ba); cfma(aBb, p.ca, h.Bb);
+                    CVec<2> oA, oB;
+                    oA.v[0] = par ? aAb : aAa; oA.v[1] = par ? aAa : aAb;
+                    oB.v[0] = par ? aBb : aBa; oB.v[1] = par ? aBa : aBb;
+                    if (REDUCE) {
+                        const double2 zAa = par ? zA.v[1] : zA.v[0], zAb = par ? zA.v[0] : zA.v[1];
+                        const double2 zBa = par ? zB.v[1] : zB.v[0], zBb = par ? zB.v[0] : zB.v[1];
+                        auto acc3 = [](double &re, double &im, double &nn, double2 z, double2 v) {
+                            re = fma(z.x, v.x, re); re = fma(z.y, v.y, re);
+                            im = fma(z.x, v.y, im); im = fma(-z.y, v.x, im);
+                            nn = fma(v.x, v.x, nn); nn = fma(v.y, v.y, nn);
+                        };
+                        if (okA) { acc3(sa_re, sa_im, sa_nn, zAa, aAa); acc3(sb_re, sb_im, sb_nn, zAb, aAb); oA.st(p.acc + e2A); }
+                        if (okB) { acc3(sa_re, sa_im, sa_nn, zBa, aBa); acc3(sb_re, sb_im, sb_nn, zBb, aBb); oB.st(p.acc + e2B); }
+                    } else {
+                        if (okA) oA.st_stream(p.acc + e2A);
+                        if (okB) oB.st_stream(p.acc + e2B);
+                    }
+                }
+            }
+            if (FLUSH) {   // the part of psi' that stage 2 cannot reach a line later: cc*T_{k-1} + cd*T_{k-2} on rows A, B of stage 1's line
+                Row2 xA, xB;
+                lds_c(xA.a, sa1 + kRowBytes + oa); lds_c(xA.b, sa1 + kRowBytes + ob);
+                lds_c(xB.a, sa1 + 2 * kRowBytes + oa); lds_c(xB.b, sa1 + 2 * kRowBytes + ob);
+                partA.a = partA.b = partB.a = partB.b = make_double2(0.0, 0.0);
+                cfma(partA.a, p.cc, xA.a); cfma(partA.b, p.cc, xA.b); cfma(partB.a, p.cc, xB.a); cfma(partB.b, p.cc, xB.b);
+                if (sub_y) {
+                    Row2 yA, yB;
+                    lds_c(yA.a, sy + oa); lds_c(yA.b, sy + ob); lds_c(yB.a, sy + kRowBytes + oa); lds_c(yB.b, sy + kRowBytes + ob);
+                    cfma(partA.a, p.cd, yA.a); cfma(partA.b, p.cd, yA.b); cfma(partB.a, p.cd, yB.a); cfma(partB.b, p.cd, yB.b);
+                }
+                rel ^= (uint32_t)(__double2hiint(partA.a.x) ^ __double2hiint(partA.b.x) ^ __double2hiint(partB.a.x) ^ __double2hiint(partB.b.x));
+            }
+            // Every shared-memory read of this line must have RETURNED before the stage and the oldest ring slot are handed back:
+            // the barrier addresses depend on the registers they filled (`rel` is 0: p.zero is 0, but only at run time).
+            rel &= (uint32_t)p.zero;
+            __syncwarp();
+            if ((tid & 31) == 0) {
+                if (sub_y) mbar_arrive(b_sempty + 8 * s + rel);
+                mbar_arrive(b_rempty + 8 * a0.i + rel);
+                if (i == run.len + 1) { mbar_arrive(b_rempty + 8 * a1.i + rel); mbar_arrive(b_rempty + 8 * a2.i + rel); }
+            }
+            if (sub_y) { if (++s == S) { s = 0; sph ^= 1u; } }
+            a0.adv(NA); a1.adv(NA); a2.adv(NA);
+        }
+        a0.adv(NA); a0.adv(NA); a1.adv(NA); a1.adv(NA); a2.adv(NA); a2.adv(NA);   // len + 2 lines consume len + 4 ring loads
+    }
+
+    if (REDUCE) {
+        double s_re[2] = {par ? sb_re : sa_re, par ? sa_re : sb_re};   // state order 2q, 2q + 1
+        double s_im[2] = {par ? sb_im : sa_im, par ? sa_im : sb_im};
+        double s_nn[2] = {par ? sb_nn : sa_nn, par ? sa_nn : sb_nn};
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+#pragma unroll
+            for (int o = 16; o >= 4; o >>= 1) {
+                s_re[k] += __shfl_xor_sync(0xffffffffu, s_re[k], o);
+                s_im[k] += __shfl_xor_sync(0xffffffffu, s_im[k], o);
+                s_nn[k] += __shfl_xor_sync(0xffffffffu, s_nn[k], o);
+            }
+        }
+        const int lane = tid & 31, warp = tid >> 5;
+        if (lane < 4) {
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                red_s[warp][lane * 2 + k][0] = s_re[k];
+                red_s[warp][lane * 2 + k][1] = s_im[k];
+                red_s[warp][lane * 2 + k][2] = s_nn[k];
+            }
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");   // consumers only (the producer warps have left)
+        if (tid < kBT * 3) {
+            const int bb = tid / 3, c = tid % 3;
+            double t = 0.0;
+#pragma unroll
+            for (int w2 = 0; w2 < kNW; ++w2) t += red_s[w2][bb][c];
+            p.partial[((int64_t)blockIdx.x * kBT + bb) * 3 + c] = t;
+        }
+    }
+}
+
+bool make_geom(const TermParams &p, Geom &g)
+{
+    if (p.sq8_line <= 0 || !p.dline || !p.uniform || p.max_row_off != kCH || p.n_table <= 1 || p.packed || p.diag) return false;
+    const int64_t W = p.sq8_line;
+    if (W % kR != 0 || p.n_orb % W != 0 || p.n_orb / W < 4 || p.n_orb >= ((int64_t)1 << 31)) return false;
+    g.W = W; g.d0 = W / kR; g.n_lines = p.n_orb / W;
+    g.len = (int)std::min<int64_t>(std::max(1, knob("sq2_len", 64)), g.n_lines);
+    g.n_ring = std::min(kMaxRing, std::max(4, knob("sq2_ring", 5)));
+    g.n_stage = std::min(kMaxStages, std::max(2, knob("sq2_stages", 3)));
+    return (size_t)(g.n_ring + kNB) * kSlotBytes + (size_t)g.n_stage * kYBytes <= kSmemMax - 4096;
+}
+
+template <bool FLUSH, bool REDUCE>
+int launch_one(const TermParams &p, const Geom &g, int num_sms, cudaStream_t st, int *grid_out)
+{
+    const size_t dyn = (size_t)(g.n_ring + kNB) * kSlotBytes + (size_t)g.n_stage * kYBytes;
+    auto kern = k_pair_sq<FLUSH, REDUCE>;
+    static size_t configured[kMaxDevices] = {0};
+    if (p.device < 0 || p.device >= kMaxDevices) return TBPM_EINVAL;
+    if (dyn > configured[p.device]) {
+        TBPM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmemMax - 4096)));
+        configured[p.device] = kSmemMax - 4096;
+    }
+    const int64_t n_runs = g.d0 * ((g.n_lines + g.len - 1) / g.len);
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>({n_runs, (int64_t)num_sms, (int64_t)kMaxGrid}));
+    kern<<<grid, kThreads, dyn, st>>>(p, g);
+    count_launches(1);
+    *grid_out = grid;
+    return TBPM_OK;
+}
+
+}  // namespace sq2
+
+// Tiles of 8 states on the square lattice that term_sq.cu runs on, without a diagonal.
+bool pair_sq_supported(int bt, const TermParams &p)
+{
+    if (bt != sq2::kBT || !knob("sq2", 1)) return false;
+    sq2::Geom g;
+    return sq2::make_geom(p, g);
+}
+
+// p.x = T_{k-1}, p.y = T_{k-2} (read only), p.out1 <- T_k, p.out2 <- T_{k+1} (neither is stored with F_REDUCE), p.a / p.a2 the two
+// scale factors, p.n_acc > 0: psi' (p.acc) += ca*T_{k+1} + cb*T_k + cc*T_{k-1} + cd*T_{k-2} (F_ACC_INIT: psi' = ...), F_SUB_Y: T_{k-2}
+// exists (k >= 2), F_REDUCE: the dot products of the last pair (implies n_acc > 0).
+int launch_pair_sq(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
+{
+    sq2::Geom g;
+    if (!sq2::make_geom(p, g) || !p.out1 || !p.out2) return TBPM_EINVAL;
+    const bool red = p.flags & F_REDUCE;
+    if (red) return p.n_acc > 0 ? sq2::launch_one<true, true>(p, g, num_sms, st, grid_out) : TBPM_EINVAL;
+    if (p.n_acc > 0) return sq2::launch_one<true, false>(p, g, num_sms, st, grid_out);
+    return sq2::launch_one<false, false>(p, g, num_sms, st, grid_out);
+}
+
+}  // namespace tbpm_detail
