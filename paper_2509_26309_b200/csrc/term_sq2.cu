@@ -28,9 +28,10 @@ namespace sq2 {
 
 using namespace ph;
 
-constexpr int kBT = 8, kNW = 9, kConsumers = kNW * 32, kThreads = kConsumers + 64;
+constexpr int kBT = 8, kMainW = 8, kMain = kMainW * 32;    // main consumers: 64 row pairs x 4 lanes
+constexpr int kNW = kMainW + 1, kConsumers = kNW * 32;     // + the halo warp
+constexpr int kThreads = kConsumers + 64;                  // + two producer warps
 constexpr int kR = 128;                                    // rows of a tile that this block OWNS (stores)
-constexpr int kPairs = kR / 2 + 1;                         // row pairs computed in stage 1: tile rows (2p - 1, 2p), p = 0 .. 64
 constexpr int kRowBytes = kBT * 16;
 constexpr int kSlotRows = kR + 4;                          // tile rows -2 .. 129
 constexpr int kSlotBytes = kSlotRows * kRowBytes;          // 16,896
@@ -53,6 +54,20 @@ struct RingPos {
 __device__ __forceinline__ void lds_c(double2 &v, uint32_t a)
 {
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+}
+// producer-side wait: poll with a pause, so that the spinning thread does not take issue slots from the consumer warps of its
+// scheduler (a fifth of all issued instructions were these polls)
+__device__ __forceinline__ void mbar_wait_idle(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    for (;;) {
+        asm volatile("{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\nselp.u32 %0, 1, 0, q;\n}"
+                     : "=r"(done)
+                     : "r"(bar), "r"(parity)
+                     : "memory");
+        if (done) break;
+        __nanosleep(64);
+    }
 }
 __device__ __forceinline__ void sts_c(uint32_t a, double2 v)
 {
@@ -98,7 +113,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t bars[2 * kMaxStages + 2 * kMaxRing];   // stage full | stage empty | ring full | ring empty
-    __shared__ double red_s[REDUCE ? kNW : 1][REDUCE ? kBT : 1][3];
+    __shared__ double red_s[REDUCE ? kMainW : 1][REDUCE ? kBT : 1][3];
 
     const int tid = threadIdx.x;
     const bool sub_y = p.flags & F_SUB_Y;                  // stage 1 subtracts T_{k-2}: always, except on the pair (1, 2)
@@ -146,7 +161,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
             for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
                 const Run r = run_of(u);
                 for (int j = -2; j < r.len + 2; ++j) {     // T_{k-1}: lines line0 - 2 .. line0 + len + 1, rows x0 - 2 .. x0 + 129
-                    mbar_wait(b_rempty + 8 * rp.i, rp.ph);
+                    mbar_wait_idle(b_rempty + 8 * rp.i, rp.ph);
                     const uint32_t full = b_rfull + 8 * rp.i;
                     mbar_expect_tx(full, kSlotBytes);
                     load_rows(ringA0 + rp.i * kSlotBytes, p.x + wrap_line(r.line0 + j) * g.W * kBT, r.pos * kR, 2, full);
@@ -159,7 +174,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
             for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
                 const Run r = run_of(u);
                 for (int j = -1; j < r.len + 1; ++j) {     // T_{k-2}: lines line0 - 1 .. line0 + len, rows x0 - 1 .. x0 + 128
-                    mbar_wait(b_sempty + 8 * s, sph);
+                    mbar_wait_idle(b_sempty + 8 * s, sph);
                     const uint32_t full = b_sfull + 8 * s;
                     mbar_expect_tx(full, kYBytes);
                     load_rows(stage0 + (uint32_t)s * kYBytes, p.y + wrap_line(r.line0 + j) * g.W * kBT, r.pos * kR, 1, full);
@@ -171,30 +186,92 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
     }
 
     // ---------------------------------------------------- consumer warps ----------------------------------------------------
-    // thread = states 2q, 2q + 1 of the tile rows A = 2 pr - 1 and B = 2 pr (pr = 0 .. 64: the tile's 128 rows and one halo row on
-    // either side); "slot a" of a thread is state 2q + par, "slot b" state 2q + 1 - par (conflict-free 128-bit accesses, term_sq.cu).
-    const bool act = (tid >> 2) < kPairs;                  // the last warp holds one pair; its other lanes only keep the barriers company
-    const int pr = act ? (tid >> 2) : kPairs - 1, q = tid & 3, par = pr & 1;
-    const bool okA = act && pr >= 1, okB = act && pr < kR / 2;   // rows that belong to the tile (stored)
-    const uint32_t oa = (uint32_t)(2 * q + par) * 16u, ob = (uint32_t)(2 * q + 1 - par) * 16u;
-    const uint32_t rows2p = (uint32_t)(2 * pr) * kRowBytes;      // 132-row slots: slot row 2p = tile row A - 1; 130-row stage: row 2p = A
-    double2 vA[kCH], vB[kCH];                              // hopping values of the two rows by direction, kept for a whole run
-    double sa_re = 0.0, sa_im = 0.0, sa_nn = 0.0, sb_re = 0.0, sb_im = 0.0, sb_nn = 0.0;
-    Row2 partA, partB;                                     // cc*T_{k-1} + cd*T_{k-2} on the rows of the line that stage 2 takes next
-    partA.a = partA.b = partB.a = partB.b = make_double2(0.0, 0.0);
-
     RingPos a0{0u, 0u}, a1{1u % NA, 0u}, a2{2u % NA, 0u};  // ring A loads holding the line above / the own line / the line below of stage 1
     int s = 0;
     uint32_t sph = 0;
     uint32_t it = 0;                                       // lines this block has taken: T_k of line `it` sits in ring B slot it % 4
 
+    if (tid >= kMain) {
+        // ---- halo warp: stage 1 for the two rows just outside the tile (tile rows -1 and 128), which stage 2 of the edge rows needs.
+        // lane = (row, state, half of the eight directions); 4 complex FMAs per lane and line, the halves added by one shuffle.
+        const int lane = tid & 31, hr = lane >> 4, state = (lane >> 1) & 7, dh = lane & 1;
+        const uint32_t srow = hr ? (uint32_t)(kR + 2) : 1u;            // slot row of the halo row (slot row = tile row + 2)
+        const uint32_t so = srow * kRowBytes + (uint32_t)state * 16u;
+        // directions 0..7 = (line, in-line offset): (above, -1 0 +1), (own, -1 +1), (below, -1 0 +1)
+        const int ln[4] = {dh ? 1 : 0, dh ? 2 : 0, dh ? 2 : 0, dh ? 2 : 1};
+        const int dx[4] = {dh ? 1 : -1, dh ? -1 : 0, dh ? 0 : 1, dh ? 1 : -1};
+        double2 hv[4];
+#pragma unroll 1
+        for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
+            const Run run = run_of(u);
+            {
+                int64_t x = run.pos * kR + (hr ? kR : -1);
+                if (x < 0) x += g.W;
+                if (x >= g.W) x -= g.W;
+                const uint2 w = __ldg(reinterpret_cast<const uint2 *>(p.dline + x * kCH + dh * 4));
+                const uint32_t id[4] = {w.x & 0xffffu, w.x >> 16, w.y & 0xffffu, w.y >> 16};
+#pragma unroll
+                for (int j = 0; j < 4; ++j) hv[j] = table_value(__ldg(p.vtab + (id[j] & 0x7fffu)), id[j]);
+            }
+#pragma unroll 1
+            for (int i = 0; i < run.len + 2; ++i, ++it) {
+                if (i == 0) {
+                    mbar_wait(b_rfull + 8 * a0.i, a0.ph);
+                    mbar_wait(b_rfull + 8 * a1.i, a1.ph);
+                }
+                mbar_wait(b_rfull + 8 * a2.i, a2.ph);
+                if (sub_y) mbar_wait(b_sfull + 8 * s, sph);
+                const uint32_t sl[3] = {ringA0 + a0.i * kSlotBytes, ringA0 + a1.i * kSlotBytes, ringA0 + a2.i * kSlotBytes};
+                double2 h = make_double2(0.0, 0.0);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    double2 xv;
+                    lds_c(xv, (ln[j] == 0 ? sl[0] : ln[j] == 1 ? sl[1] : sl[2]) + so + (uint32_t)(dx[j] * kRowBytes));
+                    cfma(h, hv[j], xv);
+                }
+                h.x += __shfl_xor_sync(0xffffffffu, h.x, 1);
+                h.y += __shfl_xor_sync(0xffffffffu, h.y, 1);
+                h.x *= p.a; h.y *= p.a;
+                if (sub_y) {                               // stage row = tile row + 1
+                    double2 yv;
+                    lds_c(yv, stage0 + (uint32_t)s * kYBytes + (hr ? (uint32_t)(kR + 1) : 0u) * kRowBytes + (uint32_t)state * 16u);
+                    h.x -= yv.x; h.y -= yv.y;
+                }
+                if (dh == 0) sts_c(ringB0 + (it % kNB) * kSlotBytes + so, h);
+                const uint32_t rel = (uint32_t)__double2hiint(h.x) & (uint32_t)p.zero;
+                asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");
+                __syncwarp();
+                if (lane == 0) {
+                    if (sub_y) mbar_arrive(b_sempty + 8 * s + rel);
+                    mbar_arrive(b_rempty + 8 * a0.i + rel);
+                    if (i == run.len + 1) { mbar_arrive(b_rempty + 8 * a1.i + rel); mbar_arrive(b_rempty + 8 * a2.i + rel); }
+                }
+                if (sub_y) { if (++s == S) { s = 0; sph ^= 1u; } }
+                a0.adv(NA); a1.adv(NA); a2.adv(NA);
+            }
+            a0.adv(NA); a0.adv(NA); a1.adv(NA); a1.adv(NA); a2.adv(NA); a2.adv(NA);
+        }
+        if (REDUCE) asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");   // the final reduction's barrier
+        return;
+    }
+
+    // ---- main consumers: thread = states 2q, 2q + 1 of the tile rows A = 2 pr and B = 2 pr + 1 (pr = 0 .. 63), in both stages;
+    // "slot a" of a thread is state 2q + par, "slot b" state 2q + 1 - par (conflict-free 128-bit accesses, term_sq.cu).
+    const int pr = tid >> 2, q = tid & 3, par = pr & 1;
+    constexpr bool act = true, okA = true, okB = true;
+    const uint32_t oa = (uint32_t)(2 * q + par) * 16u, ob = (uint32_t)(2 * q + 1 - par) * 16u;
+    const uint32_t rows2p = (uint32_t)(2 * pr + 1) * kRowBytes;  // 132-row slots: the slot row of tile row A - 1
+    const uint32_t rowsy = (uint32_t)(2 * pr + 1) * kRowBytes;   // 130-row stage: the stage row of tile row A
+    double2 vA[kCH], vB[kCH];                              // hopping values of the two rows by direction, kept for a whole run
+    double sa_re = 0.0, sa_im = 0.0, sa_nn = 0.0, sb_re = 0.0, sb_im = 0.0, sb_nn = 0.0;
+    Row2 partA, partB;                                     // cc*T_{k-1} + cd*T_{k-2} on the rows of the line that stage 2 takes next
+    partA.a = partA.b = partB.a = partB.b = make_double2(0.0, 0.0);
+
 #pragma unroll 1
     for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
         const Run run = run_of(u);
         {   // the values of the thread's two rows: dline[x][direction] -> table entry (+ conjugate bit); the same on every line
-            int64_t xa = run.pos * kR + 2 * pr - 1, xb = xa + 1;
-            if (xa < 0) xa += g.W;
-            if (xb >= g.W) xb -= g.W;
+            const int64_t xa = run.pos * kR + 2 * pr, xb = xa + 1;
             const uint4 ia = __ldg(reinterpret_cast<const uint4 *>(p.dline + xa * kCH));
             const uint4 ib = __ldg(reinterpret_cast<const uint4 *>(p.dline + xb * kCH));
             const uint32_t wa[4] = {ia.x, ia.y, ia.z, ia.w}, wb[4] = {ib.x, ib.y, ib.z, ib.w};
@@ -205,7 +282,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 vB[k] = table_value(__ldg(p.vtab + (idb & 0x7fffu)), idb);
             }
         }
-        const int64_t rowA0 = run.pos * kR + 2 * pr - 1;   // in-line position of row A
+        const int64_t rowA0 = run.pos * kR + 2 * pr;       // in-line position of row A
 #pragma unroll 1
         for (int i = 0; i < run.len + 2; ++i, ++it) {
             // stage 1 takes line line0 - 1 + i (stored when it is one of the run's), stage 2 line line0 - 2 + i (when i >= 2)
@@ -222,7 +299,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
             mbar_wait(b_rfull + 8 * a2.i, a2.ph);
             if (sub_y) mbar_wait(b_sfull + 8 * s, sph);
             const uint32_t sa0 = ringA0 + a0.i * kSlotBytes + rows2p, sa1 = ringA0 + a1.i * kSlotBytes + rows2p,
-                           sa2 = ringA0 + a2.i * kSlotBytes + rows2p, sy = stage0 + (uint32_t)s * kYBytes + rows2p;
+                           sa2 = ringA0 + a2.i * kSlotBytes + rows2p, sy = stage0 + (uint32_t)s * kYBytes + rowsy;
             uint32_t rel;
             {   // ---- stage 1: T_k = a1 * H * T_{k-1} - T_{k-2} on rows A, B of line line0 - 1 + i
                 Out4 h;
@@ -344,7 +421,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
             const int bb = tid / 3, c = tid % 3;
             double t = 0.0;
 #pragma unroll
-            for (int w2 = 0; w2 < kNW; ++w2) t += red_s[w2][bb][c];
+            for (int w2 = 0; w2 < kMainW; ++w2) t += red_s[w2][bb][c];
             p.partial[((int64_t)blockIdx.x * kBT + bb) * 3 + c] = t;
         }
     }
