@@ -120,12 +120,16 @@ void tbpm_free(tbpm_ham *H);
                              three-dimensional / square-lattice / rolling-window kernel; tiles of 1-4 states on short rows with one
                              real value: the 16-bit-offset kernel; else phased; else general);
                              1: every term on the general kernel; 2: no lattice kernel (phased, else general);
-                             3: of the lattice kernels only the rolling-window one (tests)                               */
+                             3: of the lattice kernels only the rolling-window one (tests); 4: as 0, but always ONE Chebyshev
+                             term per launch (0 runs two terms per sweep on the square lattice of configs[3], which needs two
+                             more vectors of workspace: tbpm_propagate_bytes accounts for them)                          */
 int tbpm_set_option(tbpm_ham *H, int option, int64_t value);
 
 /* ---- a2-a7: propagate ------------------------------------------------------------------------------------------------
  * Size of the caller-owned `workspace` for n_state states: four vectors [n_orb][tile] complex128 per tile of states (the
- * rotating p0 / p1 / wf_out of PAPER.md:437-443 and the bra psi0 of calc_corr_dos) + block partials. */
+ * rotating p0 / p1 / wf_out of PAPER.md:437-443 and the bra psi0 of calc_corr_dos) + block partials, + two more
+ * vectors of one tile where the two-terms-per-sweep kernel applies (a smaller workspace of at least the plain size is accepted:
+ * the call then runs one term per sweep). */
 int tbpm_propagate_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes);
 
 /* psi0: device [n_state][n_orb][2], state-major (one random initial state per row; one independent propagation per

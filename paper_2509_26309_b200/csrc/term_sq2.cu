@@ -434,7 +434,9 @@ bool make_geom(const TermParams &p, Geom &g)
     if (W % kR != 0 || p.n_orb % W != 0 || p.n_orb / W < 4 || p.n_orb >= ((int64_t)1 << 31)) return false;
     g.W = W; g.d0 = W / kR; g.n_lines = p.n_orb / W;
     g.len = (int)std::min<int64_t>(std::max(1, knob("sq2_len", 64)), g.n_lines);
-    g.n_ring = std::min(kMaxRing, std::max(4, knob("sq2_ring", 5)));
+    // Less is more: every KB of shared memory is a KB less of L1 for the streamed stores and the psi' loads in flight
+    // (cfg4: 1080 us per term with 5 + 3 slots, 1009 with 4 + 3, 1016 with 5 + 2).
+    g.n_ring = std::min(kMaxRing, std::max(4, knob("sq2_ring", 4)));
     g.n_stage = std::min(kMaxStages, std::max(2, knob("sq2_stages", 3)));
     return (size_t)(g.n_ring + kNB) * kSlotBytes + (size_t)g.n_stage * kYBytes <= kSmemMax - 4096;
 }

@@ -198,9 +198,10 @@ RW_CASES = [
 
 
 @pytest.mark.parametrize("cfg,over,n_state,n_step", RW_CASES)
-@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4])
 def test_lattice_kernels_agree_with_oracle(dev, oracle_mod, cfg, over, n_state, n_step, kernel):
-    """The same lattices on the lattice kernels (default: term_l3 where it applies, else term_rw), the general kernel
+    """The same lattices on the lattice kernels (default: term_l3 where it applies, else term_rw; on the square lattice two terms
+    per sweep, term_sq2 -- one term per sweep, term_sq, with TBPM_OPT_KERNEL = 4), the general kernel
     (TBPM_OPT_KERNEL = 1), the phased kernel (2) and term_rw alone (3): every element against the serial oracle; rows on the
     seams of the periodic lattice are gathered entry by entry inside the lattice kernels."""
     w = W.make_workload(cfg, device=dev, **over)
@@ -226,6 +227,49 @@ def test_lattice_kernels_rows_off_the_lattice(dev, oracle_mod):
     w.hop_val[777] = w.hop_val[777] * 0.5
     H, _, _, _ = run_parity(dev, oracle_mod, w, 8, 5)
     assert H.lattice_kind == 0
+
+
+@pytest.mark.parametrize("tau_scale", [1.0, 0.9, 0.5, 0.3, 0.05])
+def test_two_terms_per_sweep(dev, oracle_mod, tau_scale):
+    """term_sq2.cu (two Chebyshev terms per launch on the square lattice of cfg4): time steps whose series have an even and an odd
+    number of terms (K = 21, 20, 16, 14, 9: a leading single term when K - 1 is odd, psi' touched every second pair), a lattice of
+    three tiles per line and more lines than one run holds, 16 states = two tiles; against the oracle, against the one-term-per-sweep
+    path (TBPM_OPT_KERNEL = 4), and by the launch count (the pairs really ran)."""
+    w = W.make_workload(4, device=dev, Lx=384, Ly=150, phi_den=128)
+    dt = w.dt * tau_scale
+    K = len(tbpm.tbpm_cheb_coeff(w.rescale * dt))
+    n_step, n_state = 4, 16
+    H, psi0, corr, norm2 = run_parity(dev, oracle_mod, w, n_state, n_step, dt=dt)
+    assert H.lattice_kind == tbpm.TBPM_LATTICE_SQUARE8
+    n_launch = (K - 1) // 2 + (K - 1) % 2                               # pairs (+ a leading single term)
+    assert tbpm.tbpm_last_launch_count(H) == 2 * (1 + n_step * (n_launch + 1))   # per tile: set-up + per step the launches + reduction
+    tbpm.tbpm_set_option(H, tbpm.TBPM_OPT_KERNEL, 4)
+    c1, n1, _ = tbpm.tbpm_propagate(H, psi0, n_step, dt, w.rescale)
+    assert tbpm.tbpm_last_launch_count(H) == 2 * (1 + n_step * K)
+    assert (c1 - corr).abs().max().item() <= 1e-13 and (n1 - norm2).abs().max().item() <= 1e-13
+    # a caller workspace without the two extra vectors: the call falls back to one term per sweep instead of failing
+    tbpm.tbpm_set_option(H, tbpm.TBPM_OPT_KERNEL, 0)
+    full = tbpm.tbpm_propagate_bytes(H, n_state)
+    small = torch.empty(full - 2 * 16 * w.n_orb * 8, dtype=torch.uint8, device=dev)
+    c2, n2, _ = tbpm.tbpm_propagate(H, psi0, n_step, dt, w.rescale, workspace=small)
+    assert tbpm.tbpm_last_launch_count(H) == 2 * (1 + n_step * K)
+    assert torch.equal(c2.view(torch.float64), c1.view(torch.float64))
+
+
+def test_two_terms_per_sweep_ldos_and_determinism(dev, oracle_mod):
+    """The pair path under tbpm_ldos (unit initial vectors) and twice in a row: bit-identical."""
+    w = W.make_workload(4, device=dev, Lx=128, Ly=40, phi_den=32)
+    H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val)
+    sites = W.ldos_sites(w.n_orb, 8)
+    c1, n1, _ = tbpm.tbpm_ldos(H, sites, 6, w.dt, w.rescale)
+    assert tbpm.tbpm_last_launch_count(H) == 1 + 6 * 11                  # unit-vector set-up + 6 x (10 pairs + reduction)
+    c2, n2, _ = tbpm.tbpm_ldos(H, sites, 6, w.dt, w.rescale)
+    assert torch.equal(c1.view(torch.float64), c2.view(torch.float64)) and torch.equal(n1, n2)
+    psi0 = torch.zeros((8, w.n_orb), dtype=torch.complex128, device=dev)
+    psi0[torch.arange(8), torch.as_tensor(sites, device=dev)] = 1.0
+    hi, hj, hv, on = to_np(w)
+    ref, refn = oracle_mod.propagate(w.n_orb, on, hi, hj, hv, psi0.cpu().numpy(), 6, w.dt, w.rescale)[:2]
+    assert np.abs(c1.cpu().numpy() - ref).max() <= CORR_TOL and np.abs(n1.cpu().numpy() - refn).max() <= NORM_TOL
 
 
 def test_short_row_kernel(dev, oracle_mod):
