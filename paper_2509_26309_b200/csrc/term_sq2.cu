@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
             // ---- stage 2's operands that are not staged (HBM latency: issue first)
             CVec<2> aoldA, aoldB, zA, zB;
             if (FLUSH) { aoldA.stream_if(p.acc + e2A, st2 && okA && need_acc); aoldB.stream_if(p.acc + e2B, st2 && okB && need_acc); }
-            if (REDUCE) { zA.stream_if(p.psi0 + e2A, st2 && okA); zB.stream_if(p.psi0 + e2B, st2 && okB); }
+            if (REDUCE && st2 && q == 0) { prefetch_l2(p.psi0 + e2A); prefetch_l2(p.psi0 + e2B); }   // loaded after stage 1: 8 registers less there
             if (i == 0) {
                 mbar_wait(b_rfull + 8 * a0.i, a0.ph);
                 mbar_wait(b_rfull + 8 * a1.i, a1.ph);
@@ -323,6 +323,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 }
             }
             asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");   // line `it` of T_k is complete in ring B
+            if (REDUCE) { zA.stream_if(p.psi0 + e2A, st2 && okA); zB.stream_if(p.psi0 + e2B, st2 && okB); }
             if (st2) {
                 // ---- stage 2: T_{k+1} = a2 * H * T_k - T_{k-1} on rows A, B of line line0 - 2 + i (T_k lines it - 2, it - 1, it)
                 const uint32_t sb0 = ringB0 + ((it - 2) % kNB) * kSlotBytes + rows2p, sb1 = ringB0 + ((it - 1) % kNB) * kSlotBytes + rows2p,
