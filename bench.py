@@ -82,6 +82,8 @@ def ncu_traffic(workload_name: str, K: int):
             if r["workload"] == workload_name.split(":")[0] + ("-ldos" if workload_name.endswith("-ldos") else ""):
                 rows[r["launch"]] = float(r["dram_mbytes"])
                 src = r["source"]
+    if "step_total" in rows:                                              # two terms per launch (cfg4): all launches of a time step of 20 terms
+        return (1e6 * rows["step_total"] / (K - 1), src) if K == 21 else (None, None)
     need = ("first", "first_flush", "plain", "flush", "last")
     if any(k not in rows for k in need):
         return None, None
@@ -270,7 +272,7 @@ class Runner:
         achieved_tile = bytes_tile / avg_launch_s / 1e9
         traffic, tsrc = ncu_traffic(w.name + ("-ldos" if self.ldos else ""), self.K)
         kernel = {2: "k_term_l3 (fused Chebyshev term, three-dimensional lattice kernel, term_l3.cu)",
-                  3: "k_term_sq (fused Chebyshev term, square lattice with in-line hoppings, term_sq.cu)",
+                  3: "k_pair_sq (TWO fused Chebyshev terms per launch, square lattice with in-line hoppings, term_sq2.cu)",
                   4: "k_term_n16 (fused Chebyshev term, short rows with 16-bit column offsets, term_n16.cu)"}.get(
                       H.lattice_kind if lattice else 0, "k_term_ph (fused Chebyshev term, term_ph.cuh)")
         return {"bound": "hbm", "kernel": kernel,
@@ -286,7 +288,9 @@ class Runner:
                 "achieved_per_tile": achieved_tile, "frac_per_tile": achieved_tile / peak, "n_tile": n_tile,
                 "frac_general_layout": bytes_term_general / (avg_launch_s * n_tile) / 1e9 / peak,
                 "frac_of_nominal_8000": achieved_strict / 8000.0,
-                "note": "avg launch = CUDA-event time of tbpm_propagate / term launches (includes the <1% of tiny kernels); traffic = "
+                "note": "avg launch = CUDA-event time of tbpm_propagate / TERMS x tiles (includes the <1% of tiny kernels; on cfg4 one "
+                        "launch computes two terms, so this is the time per term, and a pair moves 4 vectors where the count has 6: "
+                        "frac can exceed the traffic-based figure); traffic = "
                         "DRAM bytes per launch measured by ncu (read + write) averaged over the launches of a time step, "
                         "frac_traffic = traffic / avg launch / peak"}
 

@@ -66,7 +66,7 @@ __device__ __forceinline__ void mbar_wait_idle(uint32_t bar, uint32_t parity)
                      : "r"(bar), "r"(parity)
                      : "memory");
         if (done) break;
-        __nanosleep(64);
+        __nanosleep(400);
     }
 }
 __device__ __forceinline__ void sts_c(uint32_t a, double2 v)
