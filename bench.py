@@ -257,13 +257,13 @@ class Runner:
     def roofline(self, prop_ms_per_step, peak, peak_src):
         """Algorithmic bytes (matrix as stored + 3 vectors) against the measured launch time of the fused term.
         The matrix bytes are those of the layout the running kernel reads: on the lattices the builder recognises (tiles of 8
-        states; short rows with one real value for tiles of 1-4 states) that is a few bytes per row, not the general kernel layout; the figure with the general layout is given beside it."""
+        states; short rows with one real value for tiles of one state) that is a few bytes per row, not the general kernel layout; the figure with the general layout is given beside it."""
         H, w = self.H, self.w
         tile = min(8, 1 << max(self.n_state - 1, 0).bit_length())
         n_tile = -(-self.n_state // tile)
         term_launches = n_tile * self.block * (self.K - 1)
         avg_launch_s = prop_ms_per_step * 1e-3 / term_launches
-        lattice = (tile == 8 and H.lattice_kind in (2, 3)) or (tile <= 4 and H.lattice_kind == 4)
+        lattice = (tile == 8 and H.lattice_kind in (2, 3)) or (tile == 1 and H.lattice_kind == 4)
         m_launch = H.lattice_bytes_per_term if lattice else H.matrix_bytes_per_term     # what ONE launch reads of H
         bytes_tile = m_launch + 48 * w.n_orb * min(tile, self.n_state)                    # one launch = one tile of states
         bytes_term_strict = m_launch + 48 * w.n_orb * self.n_state                        # one term for ALL states, matrix counted once
@@ -474,7 +474,7 @@ def main_next(args):
         run = lambda: tbpm.tbpm_propagate_qe(H, psi0, energies, block, w.dt, w.rescale)
         units = n_state * block * (K - 1) * H.nnz
         # per time step: the K - 1 terms (matrix + 3 vectors each) + the accumulation sweep (read psi', read + write n_E vectors)
-        mat = H.lattice_bytes_per_term if (H.lattice_kind == 4 and n_state <= 4) else H.matrix_bytes_per_term
+        mat = H.lattice_bytes_per_term if (H.lattice_kind == 4 and n_state == 1) else H.matrix_bytes_per_term
         bytes_step = block * ((K - 1) * (mat + 48 * w.n_orb * n_state) + (1 + 2 * len(energies)) * 16 * w.n_orb * n_state)
         what = "propagation + quasi-eigenstates at 2 energies: k_term_n16 / k_term_ph per term, k_qe_axpy once per time step"
         count = "per time step: (K - 1) x (matrix + 3 vectors) + (1 + 2 n_E) vectors of the accumulation sweep (workspace allocation and export included in the time)"

@@ -93,7 +93,7 @@ int tbpm_ham_info(const tbpm_ham *H, int64_t *n_orb, int64_t *nnz, int32_t *max_
 /* Lattices the builder recognises: tiles of 8 states then run on a kernel that reads no column words and
  * no per-entry value indices for the rows that sit on the lattice.  kind: 0 none, TBPM_LATTICE_CUBIC (offsets {+-1, +-S1, +-S2},
  * one real hopping value: BASELINE.json:configs[4]), TBPM_LATTICE_SQUARE8 (periodic square lattice with next-nearest neighbours,
- * hoppings that depend on the in-line position only: configs[3]); and, for tiles of 1, 2 or 4 states, TBPM_LATTICE_NEAR16 (rows of
+ * hoppings that depend on the in-line position only: configs[3]); and, for tiles of ONE state, TBPM_LATTICE_NEAR16 (rows of
  * at most 4 off-diagonal entries, none further than 32767 rows from its own, one real hopping value -- honeycomb or square lattice
  * with vacancies or on-site disorder: configs[0..2]; that kernel reads 16-bit column offsets).  bytes_per_term = the bytes of H THAT
  * kernel reads per Chebyshev term (what bench.py counts as the matrix when it runs on it); 0 when kind is 0.  Outputs may be NULL. */
@@ -117,7 +117,7 @@ void tbpm_free(tbpm_ham *H);
 #define TBPM_OPT_TILE 1   /* states propagated together per tile (SpMM width, PAPER.md:554 runs one state at a time):
                              1, 2, 4, 8 (default: 8 interleaved complex128 = one 128-byte line per row), 16, 32        */
 #define TBPM_OPT_KERNEL 2 /* 0 (default): the fastest kernel that applies (tiles of 8 states on a recognised lattice: the
-                             three-dimensional / square-lattice / rolling-window kernel; tiles of 1-4 states on short rows with one
+                             three-dimensional / square-lattice / rolling-window kernel; tiles of one state on short rows with one
                              real value: the 16-bit-offset kernel; else phased; else general);
                              1: every term on the general kernel; 2: no lattice kernel (phased, else general);
                              3: of the lattice kernels only the rolling-window one (tests); 4: as 0, but always ONE Chebyshev

@@ -855,7 +855,7 @@ extern "C" int tbpm_ham_lattice_info(const tbpm_ham *H, int32_t *kind, size_t *b
         k = TBPM_LATTICE_SQUARE8;                             // term_sq.cu: value indices by direction of one line + the value table
         b = sizeof(uint16_t) * 8 * (size_t)H->sq8_line + sizeof(double2) * (size_t)H->n_table + (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0);
     } else if (H->near16_w > 0) {
-        k = TBPM_LATTICE_NEAR16;                              // term_n16.cu (tiles of 1-4 states): 16-bit flag word and far offsets + real diagonal
+        k = TBPM_LATTICE_NEAR16;                              // term_n16.cu (tiles of ONE state): 16-bit flag word and far offsets + real diagonal
         b = sizeof(int16_t) * (size_t)(1 + H->near16_w) * (size_t)H->n_orb + (H->has_onsite ? sizeof(double) * (size_t)H->n_orb : 0) + sizeof(double2);
     }
     if (kind) *kind = k;

@@ -135,7 +135,7 @@ bool term_l3_supported(int bt, const TermParams &p);
 int launch_term_l3(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
 
-// Short-row kernel (term_n16.cu): tiles of 1, 2 or 4 states, rows of <= 4 entries no further than 32767 rows away, one real hopping
+// Short-row kernel (term_n16.cu): tiles of ONE state (wider tiles stay on the phased kernel), rows of <= 4 entries no further than 32767 rows away, one real hopping
 // value; reads the builder's 16-bit column offsets instead of row offsets and column words.
 bool term_n16_supported(int bt, const TermParams &p);
 int launch_term_n16(int bt, const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);

@@ -289,7 +289,7 @@ int launch_bt(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out)
 }  // namespace n16
 
 // The builder kept 16-bit column offsets (rows of <= 4 entries within 32767 rows of their own, one real hopping value), the tile
-// holds 1, 2 or 4 states, and the term is one of the five (n_acc, reduce) shapes of a time step.
+// holds ONE state, and the term is one of the five (n_acc, reduce) shapes of a time step.
 bool term_n16_supported(int bt, const TermParams &p)
 {
     if (!p.d16 || (p.n16_w != 1 && p.n16_w != 2 && p.n16_w != 4) || !p.single_real || p.n_table != 1 || (p.flags & F_SKIP_H)) return false;
