@@ -11,14 +11,16 @@
 // and keeps the last three lines of T_k it has just computed in a second shared-memory ring: T_{k+1} of line L - 1 follows as soon
 // as T_k of line L exists.  A pair of terms then reads 2 vectors and writes 2 (4 instead of 6), and psi' is touched once per FOUR
 // terms instead of three: 52 instead of 74 vector transfers per time step of 20 terms.
-//   halo     T_{k+1} on rows [x0, x0 + 128) needs T_k on [x0 - 1, x0 + 129): the block computes those two extra rows itself (65 row
-//            pairs instead of 64: +1.6 %), from T_{k-1} on [x0 - 2, x0 + 130) -- ring slots of 132 rows -- and T_{k-2} on 130 rows;
-//            along the walk it computes T_k on one extra line above and below its run of 64 lines (+3 %).
+//   halo     T_{k+1} on rows [x0, x0 + 128) needs T_k on [x0 - 1, x0 + 129), from T_{k-1} on [x0 - 2, x0 + 130) -- ring slots of 132
+//            rows -- and T_{k-2} on 130 rows; the two rows outside the tile are computed by a light "halo warp" (lane = row, state,
+//            half of the directions).  Along the walk T_k is computed on one extra line above and below the run of 64 lines (+3 %).
 //   buffers  T_{k-2} is now read with a halo, so T_k cannot overwrite it in place: both results go to buffers of their own
 //            (TermParams::out1 / out2), which the next pair reads while it writes the two this pair read.
-//   sync     consumers: 9 warps (65 row pairs x 4 lanes; thread = 2 states of 2 adjacent rows, the values of those two rows in
-//            registers for a whole run, serving both stages).  Per line: stage 1 -> named barrier (the line of T_k is in the ring)
-//            -> stage 2.  Ring B slot (it % 4) is rewritten two barriers after its last reader passed one: no further hand-shake.
+//   sync     8 main consumer warps (64 row pairs x 4 lanes; thread = 2 states of 2 adjacent rows, the values of those two rows in
+//            registers for a whole run, serving both stages) + the halo warp.  Per line: stage 1 -> named barrier (the line of T_k
+//            is in ring B) -> stage 2.  Ring B slot (it % 4) is rewritten two barriers after its last reader passed one: no
+//            further hand-shake.  (A ninth FULL warp for a 65th row pair cost what the pairing won: 9 warps over 4 schedulers.)
+//   less shared memory is faster here: it is L1 taken from the streamed stores (4 ring slots + 3 stages, not 5 + 4).
 #include <algorithm>
 
 #include "term_ph.cuh"
