@@ -291,7 +291,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
             const bool st2 = i >= 2;
             const int64_t e2A = ((run.line0 + i - 2) * g.W + rowA0) * kBT + 2 * q, e2B = e2A + kBT;
             // ---- stage 2's operands that are not staged (HBM latency: issue first)
-            CVec<2> aoldA, aoldB, zA, zB;
+            CVec<2> aoldA, aoldB;
+            double2 zAa, zAb, zBa, zBb;                    // psi0 on rows A, B in slot order (state 2q + par, 2q + 1 - par)
             if (FLUSH) { aoldA.stream_if(p.acc + e2A, st2 && okA && need_acc); aoldB.stream_if(p.acc + e2B, st2 && okB && need_acc); }
             if (REDUCE && st2 && q == 0) { prefetch_l2(p.psi0 + e2A); prefetch_l2(p.psi0 + e2B); }   // loaded after stage 1: 8 registers less there
             if (i == 0) {
@@ -325,7 +326,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 }
             }
             asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");   // line `it` of T_k is complete in ring B
-            if (REDUCE) { zA.stream_if(p.psi0 + e2A, st2 && okA); zB.stream_if(p.psi0 + e2B, st2 && okB); }
+            if (REDUCE && st2) {   // four 128-bit loads straight into slot order: no selects that would wait for the data here (L2 hits)
+                zAa = __ldcs(p.psi0 + e2A + par); zAb = __ldcs(p.psi0 + e2A + (1 - par));
+                zBa = __ldcs(p.psi0 + e2B + par); zBb = __ldcs(p.psi0 + e2B + (1 - par));
+            }
             if (st2) {
                 // ---- stage 2: T_{k+1} = a2 * H * T_k - T_{k-1} on rows A, B of line line0 - 2 + i (T_k lines it - 2, it - 1, it)
                 const uint32_t sb0 = ringB0 + ((it - 2) % kNB) * kSlotBytes + rows2p, sb1 = ringB0 + ((it - 1) % kNB) * kSlotBytes + rows2p,
@@ -354,8 +358,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                     oA.v[0] = par ? aAb : aAa; oA.v[1] = par ? aAa : aAb;
                     oB.v[0] = par ? aBb : aBa; oB.v[1] = par ? aBa : aBb;
                     if (REDUCE) {
-                        const double2 zAa = par ? zA.v[1] : zA.v[0], zAb = par ? zA.v[0] : zA.v[1];
-                        const double2 zBa = par ? zB.v[1] : zB.v[0], zBb = par ? zB.v[0] : zB.v[1];
                         auto acc3 = [](double &re, double &im, double &nn, double2 z, double2 v) {
                             re = fma(z.x, v.x, re); re = fma(z.y, v.y, re);
                             im = fma(z.x, v.y, im); im = fma(-z.y, v.x, im);
