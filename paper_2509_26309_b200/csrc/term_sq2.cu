@@ -291,9 +291,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
             const bool st2 = i >= 2;
             const int64_t e2A = ((run.line0 + i - 2) * g.W + rowA0) * kBT + 2 * q, e2B = e2A + kBT;
             // ---- stage 2's operands that are not staged (HBM latency: issue first)
-            CVec<2> aoldA, aoldB;
+            double2 aAa, aAb, aBa, aBb;                    // psi' on rows A, B in slot order
+            aAa = aAb = aBa = aBb = make_double2(0.0, 0.0);
             double2 zAa, zAb, zBa, zBb;                    // psi0 on rows A, B in slot order (state 2q + par, 2q + 1 - par)
-            if (FLUSH) { aoldA.stream_if(p.acc + e2A, st2 && okA && need_acc); aoldB.stream_if(p.acc + e2B, st2 && okB && need_acc); }
+            if (FLUSH && st2 && need_acc) {                // 128-bit loads straight into slot order (no selects on arrival)
+                aAa = __ldcs(p.acc + e2A + par); aAb = __ldcs(p.acc + e2A + (1 - par));
+                aBa = __ldcs(p.acc + e2B + par); aBb = __ldcs(p.acc + e2B + (1 - par));
+            }
             if (REDUCE && st2 && q == 0) { prefetch_l2(p.psi0 + e2A); prefetch_l2(p.psi0 + e2B); }   // loaded after stage 1: 8 registers less there
             if (i == 0) {
                 mbar_wait(b_rfull + 8 * a0.i, a0.ph);
@@ -348,8 +352,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                     if (okB) { out.v[0] = par ? h.Bb : h.Ba; out.v[1] = par ? h.Ba : h.Bb; out.st_stream(p.out2 + e2B); }
                 }
                 if (FLUSH) {
-                    double2 aAa = par ? aoldA.v[1] : aoldA.v[0], aAb = par ? aoldA.v[0] : aoldA.v[1];
-                    double2 aBa = par ? aoldB.v[1] : aoldB.v[0], aBb = par ? aoldB.v[0] : aoldB.v[1];
                     aAa.x += partA.a.x; aAa.y += partA.a.y; aAb.x += partA.b.x; aAb.y += partA.b.y;
                     aBa.x += partB.a.x; aBa.y += partB.a.y; aBb.x += partB.b.x; aBb.y += partB.b.y;
                     cfma(aAa, p.cb, tA.a); cfma(aAb, p.cb, tA.b); cfma(aBa, p.cb, tB.a); cfma(aBb, p.cb, tB.b);
