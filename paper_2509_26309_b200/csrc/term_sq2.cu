@@ -1,5 +1,5 @@
 // term_sq2.cu -- TWO Chebyshev terms per sweep on the periodic square lattice with next-nearest neighbours and in-line hoppings
-// (BASELINE.json:configs[3]; the lattice of term_sq.cu, tiles of 8 interleaved states, no diagonal).
+// (BASELINE.json:configs[3]; the lattice of term_sq.cu, tiles of 8 interleaved states; a real diagonal rides in the y stage).
 //
 //   T_k     = a1*H*T_{k-1} - T_{k-2}      (amxsy)
 //   T_{k+1} = a2*H*T_k     - T_{k-1}
@@ -39,13 +39,15 @@ constexpr int kSlotRows = kR + 4;                          // tile rows -2 .. 12
 constexpr int kSlotBytes = kSlotRows * kRowBytes;          // 16,896
 constexpr int kYRows = kR + 2;                             // tile rows -1 .. 128
 constexpr int kYBytes = kYRows * kRowBytes;                // 16,640
+constexpr int kDiagRows = kR + 4;                          // diagonal of tile rows -2 .. 129 (16-byte aligned bulk copies), behind the y rows
+constexpr int kDiagBytes = 1152;                           // 132 x 8 = 1,056, padded to a multiple of 128
 constexpr int kMaxRing = 8;
 constexpr int kNB = 4;                                     // slots of the T_k ring
 constexpr int kCH = 8;
 
 struct Geom {
     int64_t W, d0, n_lines;
-    int len, n_ring, n_stage;
+    int len, n_ring, n_stage, stage_bytes;
 };
 
 struct RingPos {
@@ -110,7 +112,7 @@ __device__ __forceinline__ void apply_h(uint32_t bp, uint32_t bo, uint32_t bn, u
     }
 }
 
-template <bool FLUSH, bool REDUCE>
+template <bool FLUSH, bool REDUCE, bool DIAG>
 __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, const Geom g)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -120,6 +122,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
     const int tid = threadIdx.x;
     const bool sub_y = p.flags & F_SUB_Y;                  // stage 1 subtracts T_{k-2}: always, except on the pair (1, 2)
     const bool need_acc = FLUSH && !(p.flags & F_ACC_INIT);
+    const bool use_st = sub_y || DIAG;                     // the stage carries T_{k-2} and / or the diagonal
+    const uint32_t stb = (uint32_t)g.stage_bytes;
     const int S = g.n_stage;
     const uint32_t NA = (uint32_t)g.n_ring;
     const uint32_t bar0 = smem_u32(bars), smem0 = smem_u32(smem);
@@ -151,12 +155,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
         // ------------------------------- producers: one thread of each of the two producer warps -------------------------------
         if ((tid & 31) != 0) return;
         // `halo` rows on either side of the tile's 128, taken round the periodic line
-        auto load_rows = [&](uint32_t dst, const double2 *line_base, int64_t x0, int halo, uint32_t full) {
+        auto load_rows = [&](uint32_t dst, const void *line_base_v, int64_t x0, int halo, uint32_t full, uint32_t rb = kRowBytes) {
+            const char *line_base = static_cast<const char *>(line_base_v);   // rb = bytes per row (128: a vector row, 8: the diagonal)
             const bool wrap_lo = x0 == 0, wrap_hi = x0 + kR == g.W;
             const int lo = wrap_lo ? 0 : -halo, hi = wrap_hi ? kR : kR + halo;
-            bulk_g2s(dst + (uint32_t)(lo + halo) * kRowBytes, line_base + (x0 + lo) * kBT, (uint32_t)(hi - lo) * kRowBytes, full);
-            if (wrap_lo) bulk_g2s(dst, line_base + (g.W - halo) * kBT, (uint32_t)halo * kRowBytes, full);
-            if (wrap_hi) bulk_g2s(dst + (uint32_t)(kR + halo) * kRowBytes, line_base, (uint32_t)halo * kRowBytes, full);
+            bulk_g2s(dst + (uint32_t)(lo + halo) * rb, line_base + (x0 + lo) * (int64_t)rb, (uint32_t)(hi - lo) * rb, full);
+            if (wrap_lo) bulk_g2s(dst, line_base + (g.W - halo) * (int64_t)rb, (uint32_t)halo * rb, full);
+            if (wrap_hi) bulk_g2s(dst + (uint32_t)(kR + halo) * rb, line_base, (uint32_t)halo * rb, full);
         };
         if (tid == kConsumers) {
             RingPos rp{0u, 1u};
@@ -170,7 +175,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                     rp.adv(NA);
                 }
             }
-        } else if (sub_y) {
+        } else if (use_st) {
             int s = 0;
             uint32_t sph = 1;
             for (int64_t u = blockIdx.x; u < n_runs; u += gridDim.x) {
@@ -178,8 +183,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 for (int j = -1; j < r.len + 1; ++j) {     // T_{k-2}: lines line0 - 1 .. line0 + len, rows x0 - 1 .. x0 + 128
                     mbar_wait_idle(b_sempty + 8 * s, sph);
                     const uint32_t full = b_sfull + 8 * s;
-                    mbar_expect_tx(full, kYBytes);
-                    load_rows(stage0 + (uint32_t)s * kYBytes, p.y + wrap_line(r.line0 + j) * g.W * kBT, r.pos * kR, 1, full);
+                    mbar_expect_tx(full, (sub_y ? (uint32_t)kYBytes : 0u) + (DIAG ? (uint32_t)kDiagRows * 8u : 0u));
+                    const int64_t line = wrap_line(r.line0 + j);
+                    if (sub_y) load_rows(stage0 + (uint32_t)s * stb, p.y + line * g.W * kBT, r.pos * kR, 1, full);
+                    if (DIAG) load_rows(stage0 + (uint32_t)s * stb + kYBytes, p.diag + line * g.W, r.pos * kR, 2, full, 8u);   // halo 2: 16-byte aligned
                     if (++s == S) { s = 0; sph ^= 1u; }
                 }
             }
@@ -222,7 +229,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                     mbar_wait(b_rfull + 8 * a1.i, a1.ph);
                 }
                 mbar_wait(b_rfull + 8 * a2.i, a2.ph);
-                if (sub_y) mbar_wait(b_sfull + 8 * s, sph);
+                if (use_st) mbar_wait(b_sfull + 8 * s, sph);
                 const uint32_t sl[3] = {ringA0 + a0.i * kSlotBytes, ringA0 + a1.i * kSlotBytes, ringA0 + a2.i * kSlotBytes};
                 double2 h = make_double2(0.0, 0.0);
 #pragma unroll
@@ -233,10 +240,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 }
                 h.x += __shfl_xor_sync(0xffffffffu, h.x, 1);
                 h.y += __shfl_xor_sync(0xffffffffu, h.y, 1);
+                if (DIAG) {                                // + d * x on the halo row itself (diagonal stage index = tile row + 2)
+                    double2 xo;
+                    lds_c(xo, sl[1] + so);
+                    const double d = lds_f64(stage0 + (uint32_t)s * stb + kYBytes + srow * 8u);
+                    h.x = fma(d, xo.x, h.x); h.y = fma(d, xo.y, h.y);
+                }
                 h.x *= p.a; h.y *= p.a;
                 if (sub_y) {                               // stage row = tile row + 1
                     double2 yv;
-                    lds_c(yv, stage0 + (uint32_t)s * kYBytes + (hr ? (uint32_t)(kR + 1) : 0u) * kRowBytes + (uint32_t)state * 16u);
+                    lds_c(yv, stage0 + (uint32_t)s * stb + (hr ? (uint32_t)(kR + 1) : 0u) * kRowBytes + (uint32_t)state * 16u);
                     h.x -= yv.x; h.y -= yv.y;
                 }
                 if (dh == 0) sts_c(ringB0 + (it % kNB) * kSlotBytes + so, h);
@@ -244,11 +257,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");
                 __syncwarp();
                 if (lane == 0) {
-                    if (sub_y) mbar_arrive(b_sempty + 8 * s + rel);
+                    if (use_st) mbar_arrive(b_sempty + 8 * s + rel);
                     mbar_arrive(b_rempty + 8 * a0.i + rel);
                     if (i == run.len + 1) { mbar_arrive(b_rempty + 8 * a1.i + rel); mbar_arrive(b_rempty + 8 * a2.i + rel); }
                 }
-                if (sub_y) { if (++s == S) { s = 0; sph ^= 1u; } }
+                if (use_st) { if (++s == S) { s = 0; sph ^= 1u; } }
                 a0.adv(NA); a1.adv(NA); a2.adv(NA);
             }
             a0.adv(NA); a0.adv(NA); a1.adv(NA); a1.adv(NA); a2.adv(NA); a2.adv(NA);
@@ -267,6 +280,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
     double2 vA[kCH], vB[kCH];                              // hopping values of the two rows by direction, kept for a whole run
     double sa_re = 0.0, sa_im = 0.0, sa_nn = 0.0, sb_re = 0.0, sb_im = 0.0, sb_nn = 0.0;
     Row2 partA, partB;                                     // cc*T_{k-1} + cd*T_{k-2} on the rows of the line that stage 2 takes next
+    double dA = 0.0, dB = 0.0, dPA = 0.0, dPB = 0.0;       // DIAG: diagonal of rows A, B on stage 1's line / on stage 2's line (the line before)
     partA.a = partA.b = partB.a = partB.b = make_double2(0.0, 0.0);
 
 #pragma unroll 1
@@ -289,6 +303,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
         for (int i = 0; i < run.len + 2; ++i, ++it) {
             // stage 1 takes line line0 - 1 + i (stored when it is one of the run's), stage 2 line line0 - 2 + i (when i >= 2)
             const bool st2 = i >= 2;
+            if (DIAG) { dPA = dA; dPB = dB; }
             const int64_t e2A = ((run.line0 + i - 2) * g.W + rowA0) * kBT + 2 * q, e2B = e2A + kBT;
             // ---- stage 2's operands that are not staged (HBM latency: issue first)
             double2 aAa, aAb, aBa, aBb;                    // psi' on rows A, B in slot order
@@ -304,14 +319,20 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 mbar_wait(b_rfull + 8 * a1.i, a1.ph);
             }
             mbar_wait(b_rfull + 8 * a2.i, a2.ph);
-            if (sub_y) mbar_wait(b_sfull + 8 * s, sph);
+            if (use_st) mbar_wait(b_sfull + 8 * s, sph);
             const uint32_t sa0 = ringA0 + a0.i * kSlotBytes + rows2p, sa1 = ringA0 + a1.i * kSlotBytes + rows2p,
-                           sa2 = ringA0 + a2.i * kSlotBytes + rows2p, sy = stage0 + (uint32_t)s * kYBytes + rowsy;
+                           sa2 = ringA0 + a2.i * kSlotBytes + rows2p, sy = stage0 + (uint32_t)s * stb + rowsy;
             uint32_t rel;
             {   // ---- stage 1: T_k = a1 * H * T_{k-1} - T_{k-2} on rows A, B of line line0 - 1 + i
                 Out4 h;
                 Row2 xA, xB;
                 apply_h(sa0, sa1, sa2, oa, ob, vA, vB, h, xA, xB);
+                if (DIAG) {                                // diagonal of rows A, B of this line (stage index = tile row + 2); kept for stage 2 of the next line
+                    const uint32_t sd = stage0 + (uint32_t)s * stb + kYBytes + (uint32_t)(2 * pr + 2) * 8u;
+                    dA = lds_f64(sd); dB = lds_f64(sd + 8u);
+                    h.Aa.x = fma(dA, xA.a.x, h.Aa.x); h.Aa.y = fma(dA, xA.a.y, h.Aa.y); h.Ab.x = fma(dA, xA.b.x, h.Ab.x); h.Ab.y = fma(dA, xA.b.y, h.Ab.y);
+                    h.Ba.x = fma(dB, xB.a.x, h.Ba.x); h.Ba.y = fma(dB, xB.a.y, h.Ba.y); h.Bb.x = fma(dB, xB.b.x, h.Bb.x); h.Bb.y = fma(dB, xB.b.y, h.Bb.y);
+                }
                 h.Aa.x *= p.a; h.Aa.y *= p.a; h.Ab.x *= p.a; h.Ab.y *= p.a; h.Ba.x *= p.a; h.Ba.y *= p.a; h.Bb.x *= p.a; h.Bb.y *= p.a;
                 if (sub_y) {
                     Row2 yA, yB;
@@ -320,6 +341,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                     h.Ba.x -= yB.a.x; h.Ba.y -= yB.a.y; h.Bb.x -= yB.b.x; h.Bb.y -= yB.b.y;
                 }
                 rel = (uint32_t)(__double2hiint(h.Aa.x) ^ __double2hiint(h.Ab.x) ^ __double2hiint(h.Ba.x) ^ __double2hiint(h.Bb.x));
+                if (DIAG) rel ^= (uint32_t)(__double2hiint(dA) ^ __double2hiint(dB));
                 const uint32_t wb = ringB0 + (it % kNB) * kSlotBytes + rows2p + kRowBytes;   // slot rows 2p + 1, 2p + 2 = rows A, B
                 if (act) { sts_c(wb + oa, h.Aa); sts_c(wb + ob, h.Ab); sts_c(wb + kRowBytes + oa, h.Ba); sts_c(wb + kRowBytes + ob, h.Bb); }
                 if (!REDUCE && i >= 1 && i <= run.len) {   // T_k of the run's own lines: read by the next pair, a whole sweep later
@@ -341,6 +363,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 Out4 h;
                 Row2 tA, tB, xA, xB;                       // T_k and T_{k-1} on the own rows
                 apply_h(sb0, sb1, sb2, oa, ob, vA, vB, h, tA, tB);
+                if (DIAG) {
+                    h.Aa.x = fma(dPA, tA.a.x, h.Aa.x); h.Aa.y = fma(dPA, tA.a.y, h.Aa.y); h.Ab.x = fma(dPA, tA.b.x, h.Ab.x); h.Ab.y = fma(dPA, tA.b.y, h.Ab.y);
+                    h.Ba.x = fma(dPB, tB.a.x, h.Ba.x); h.Ba.y = fma(dPB, tB.a.y, h.Ba.y); h.Bb.x = fma(dPB, tB.b.x, h.Bb.x); h.Bb.y = fma(dPB, tB.b.y, h.Bb.y);
+                }
                 lds_c(xA.a, sa0 + kRowBytes + oa); lds_c(xA.b, sa0 + kRowBytes + ob);
                 lds_c(xB.a, sa0 + 2 * kRowBytes + oa); lds_c(xB.b, sa0 + 2 * kRowBytes + ob);
                 h.Aa.x = fma(p.a2, h.Aa.x, -xA.a.x); h.Aa.y = fma(p.a2, h.Aa.y, -xA.a.y); h.Ab.x = fma(p.a2, h.Ab.x, -xA.b.x); h.Ab.y = fma(p.a2, h.Ab.y, -xA.b.y);
@@ -391,11 +417,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
             rel &= (uint32_t)p.zero;
             __syncwarp();
             if ((tid & 31) == 0) {
-                if (sub_y) mbar_arrive(b_sempty + 8 * s + rel);
+                if (use_st) mbar_arrive(b_sempty + 8 * s + rel);
                 mbar_arrive(b_rempty + 8 * a0.i + rel);
                 if (i == run.len + 1) { mbar_arrive(b_rempty + 8 * a1.i + rel); mbar_arrive(b_rempty + 8 * a2.i + rel); }
             }
-            if (sub_y) { if (++s == S) { s = 0; sph ^= 1u; } }
+            if (use_st) { if (++s == S) { s = 0; sph ^= 1u; } }
             a0.adv(NA); a1.adv(NA); a2.adv(NA);
         }
         a0.adv(NA); a0.adv(NA); a1.adv(NA); a1.adv(NA); a2.adv(NA); a2.adv(NA);   // len + 2 lines consume len + 4 ring loads
@@ -436,7 +462,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
 
 bool make_geom(const TermParams &p, Geom &g)
 {
-    if (p.sq8_line <= 0 || !p.dline || !p.uniform || p.max_row_off != kCH || p.n_table <= 1 || p.packed || p.diag) return false;
+    if (p.sq8_line <= 0 || !p.dline || !p.uniform || p.max_row_off != kCH || p.n_table <= 1 || p.packed) return false;
     const int64_t W = p.sq8_line;
     if (W % kR != 0 || p.n_orb % W != 0 || p.n_orb / W < 4 || p.n_orb >= ((int64_t)1 << 31)) return false;
     g.W = W; g.d0 = W / kR; g.n_lines = p.n_orb / W;
@@ -445,14 +471,15 @@ bool make_geom(const TermParams &p, Geom &g)
     // (cfg4: 1080 us per term with 5 + 3 slots, 1009 with 4 + 3, 1016 with 5 + 2).
     g.n_ring = std::min(kMaxRing, std::max(4, knob("sq2_ring", 4)));
     g.n_stage = std::min(kMaxStages, std::max(2, knob("sq2_stages", 3)));
-    return (size_t)(g.n_ring + kNB) * kSlotBytes + (size_t)g.n_stage * kYBytes <= kSmemMax - 4096;
+    g.stage_bytes = kYBytes + (p.diag ? kDiagBytes : 0);
+    return (size_t)(g.n_ring + kNB) * kSlotBytes + (size_t)g.n_stage * g.stage_bytes <= kSmemMax - 4096;
 }
 
-template <bool FLUSH, bool REDUCE>
+template <bool FLUSH, bool REDUCE, bool DIAG>
 int launch_one(const TermParams &p, const Geom &g, int num_sms, cudaStream_t st, int *grid_out)
 {
-    const size_t dyn = (size_t)(g.n_ring + kNB) * kSlotBytes + (size_t)g.n_stage * kYBytes;
-    auto kern = k_pair_sq<FLUSH, REDUCE>;
+    const size_t dyn = (size_t)(g.n_ring + kNB) * kSlotBytes + (size_t)g.n_stage * g.stage_bytes;
+    auto kern = k_pair_sq<FLUSH, REDUCE, DIAG>;
     static size_t configured[kMaxDevices] = {0};
     if (p.device < 0 || p.device >= kMaxDevices) return TBPM_EINVAL;
     if (dyn > configured[p.device]) {
@@ -469,7 +496,7 @@ int launch_one(const TermParams &p, const Geom &g, int num_sms, cudaStream_t st,
 
 }  // namespace sq2
 
-// Tiles of 8 states on the square lattice that term_sq.cu runs on, without a diagonal.
+// Tiles of 8 states on the square lattice that term_sq.cu runs on (with or without a real diagonal).
 bool pair_sq_supported(int bt, const TermParams &p)
 {
     if (bt != sq2::kBT || !knob("sq2", 1)) return false;
@@ -485,9 +512,15 @@ int launch_pair_sq(const TermParams &p, int num_sms, cudaStream_t st, int *grid_
     sq2::Geom g;
     if (!sq2::make_geom(p, g) || !p.out1 || !p.out2) return TBPM_EINVAL;
     const bool red = p.flags & F_REDUCE;
-    if (red) return p.n_acc > 0 ? sq2::launch_one<true, true>(p, g, num_sms, st, grid_out) : TBPM_EINVAL;
-    if (p.n_acc > 0) return sq2::launch_one<true, false>(p, g, num_sms, st, grid_out);
-    return sq2::launch_one<false, false>(p, g, num_sms, st, grid_out);
+    if (red && p.n_acc <= 0) return TBPM_EINVAL;
+    if (p.diag) {
+        if (red) return sq2::launch_one<true, true, true>(p, g, num_sms, st, grid_out);
+        if (p.n_acc > 0) return sq2::launch_one<true, false, true>(p, g, num_sms, st, grid_out);
+        return sq2::launch_one<false, false, true>(p, g, num_sms, st, grid_out);
+    }
+    if (red) return sq2::launch_one<true, true, false>(p, g, num_sms, st, grid_out);
+    if (p.n_acc > 0) return sq2::launch_one<true, false, false>(p, g, num_sms, st, grid_out);
+    return sq2::launch_one<false, false, false>(p, g, num_sms, st, grid_out);
 }
 
 }  // namespace tbpm_detail

@@ -256,6 +256,23 @@ def test_two_terms_per_sweep(dev, oracle_mod, tau_scale):
     assert torch.equal(c2.view(torch.float64), c1.view(torch.float64))
 
 
+@pytest.mark.parametrize("tau_scale", [1.0, 0.45])
+def test_two_terms_per_sweep_with_diagonal(dev, oracle_mod, tau_scale):
+    """The pair kernel with a real diagonal (square lattice + flux + Anderson disorder: the diagonal of 132 rows per line rides in
+    the y stage, also on the first pair, which has no T_{k-2}): even and odd numbers of terms, two tiles of states, both paths."""
+    n, hi, hj, hv = W.square_peierls_hops(256, 70, -1.0, 0.2, 1, 64, dev)
+    w = W.Workload("square-flux-anderson", n, hi, hj, hv, W.anderson_onsite(n, 3.0, device=dev), 16, 5, 6.4)
+    dt = w.dt * tau_scale
+    K = len(tbpm.tbpm_cheb_coeff(w.rescale * dt))
+    H, psi0, corr, norm2 = run_parity(dev, oracle_mod, w, 16, 5, dt=dt)
+    assert H.lattice_kind == tbpm.TBPM_LATTICE_SQUARE8
+    assert tbpm.tbpm_last_launch_count(H) == 2 * (1 + 5 * ((K - 1) // 2 + (K - 1) % 2 + 1))
+    tbpm.tbpm_set_option(H, tbpm.TBPM_OPT_KERNEL, 4)
+    c1, n1, _ = tbpm.tbpm_propagate(H, psi0, 5, dt, w.rescale)
+    assert tbpm.tbpm_last_launch_count(H) == 2 * (1 + 5 * K)
+    assert (c1 - corr).abs().max().item() <= 1e-13 and (n1 - norm2).abs().max().item() <= 1e-13
+
+
 def test_two_terms_per_sweep_ldos_and_determinism(dev, oracle_mod):
     """The pair path under tbpm_ldos (unit initial vectors) and twice in a row: bit-identical."""
     w = W.make_workload(4, device=dev, Lx=128, Ly=40, phi_den=32)
