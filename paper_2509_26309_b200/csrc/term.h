@@ -125,7 +125,7 @@ int launch_term_rw(const TermParams &p, int num_sms, cudaStream_t st, int *grid_
 bool term_sq_supported(int bt, const TermParams &p);
 int launch_term_sq(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
-// Two terms per sweep on the same lattice without a diagonal (term_sq2.cu); see launch_pair_sq for the meaning of the fields.
+// Two terms per sweep on the same lattice (term_sq2.cu); see launch_pair_sq for the meaning of the fields.
 bool pair_sq_supported(int bt, const TermParams &p);
 int launch_pair_sq(const TermParams &p, int num_sms, cudaStream_t st, int *grid_out);
 
