@@ -256,11 +256,12 @@ def test_two_terms_per_sweep(dev, oracle_mod, tau_scale):
     assert torch.equal(c2.view(torch.float64), c1.view(torch.float64))
 
 
+@pytest.mark.parametrize("Lx,Ly,phi_den", [(256, 70, 64), (128, 40, 32)])                # two tiles per line / one (both line ends in one tile)
 @pytest.mark.parametrize("tau_scale", [1.0, 0.45])
-def test_two_terms_per_sweep_with_diagonal(dev, oracle_mod, tau_scale):
+def test_two_terms_per_sweep_with_diagonal(dev, oracle_mod, tau_scale, Lx, Ly, phi_den):
     """The pair kernel with a real diagonal (square lattice + flux + Anderson disorder: the diagonal of 132 rows per line rides in
     the y stage, also on the first pair, which has no T_{k-2}): even and odd numbers of terms, two tiles of states, both paths."""
-    n, hi, hj, hv = W.square_peierls_hops(256, 70, -1.0, 0.2, 1, 64, dev)
+    n, hi, hj, hv = W.square_peierls_hops(Lx, Ly, -1.0, 0.2, 1, phi_den, dev)
     w = W.Workload("square-flux-anderson", n, hi, hj, hv, W.anderson_onsite(n, 3.0, device=dev), 16, 5, 6.4)
     dt = w.dt * tau_scale
     K = len(tbpm.tbpm_cheb_coeff(w.rescale * dt))
