@@ -237,7 +237,9 @@ int tbpm_corr_dp(tbpm_ham *H, const double *rho_a /* device */, const double *rh
 /* ---- end to end with HOST buffers ------------------------------------------------------------------------------------
  * Whole path for host-resident inputs: H2D of the list and psi0, tbpm_build, tbpm_propagate, D2H of corr/norm2, then a
  * stream synchronise.  `arena` is caller-owned device memory of at least tbpm_corr_host_bytes(); host buffers should be
- * pinned for full copy bandwidth.  h2d_bytes / d2h_bytes (may be NULL) report what was copied. */
+ * pinned for full copy bandwidth.  h2d_bytes / d2h_bytes (may be NULL) report what was copied.  The arena is sized before the
+ * lattice is known and holds the plain workspace only: on the square lattice of configs[3] this call therefore runs one Chebyshev
+ * term per sweep (same results; use tbpm_build + tbpm_propagate for the two-terms-per-sweep kernel). */
 int tbpm_corr_host_bytes(int64_t n_orb, int64_t n_hop, int has_onsite, int n_state, int n_step, uint32_t flags,
                          size_t *arena_bytes);
 int tbpm_corr_host(int64_t n_orb, const double *onsite /* host or NULL */, int64_t n_hop, const int32_t *hop_i /* host */,
