@@ -421,7 +421,7 @@ __global__ void k_qe_export(const double2 *__restrict__ qe_ws, size_t stride, in
 //     u_{n+1} = t / beta_n - (a_n / beta_n) u_n - (beta_n / beta_{n-1}) u_{n-1},   a_n = Re<u_n|t> / beta_n^2,   b_{n+1} = ||u_{n+1}||
 // which is the textbook  b_{n+1} phi_{n+1} = H phi_n - a_n phi_n - b_n phi_{n-1}  with b_n = beta_n.
 // sc[b] = {Re<u_n|t>, beta_n, beta_{n-1}, unused}; a zero beta (Krylov space exhausted, or a padding state) gives zeros from then on.
-__global__ void k_haydock_update(const double2 *__restrict__ t, const double2 *__restrict__ u, double2 *u_prev, int64_t n_orb, int bt,
+__global__ void k_haydock_update(const double2 *__restrict__ t, const double2 *__restrict__ u, double2 *__restrict__ u_prev, int64_t n_orb, int bt,
                                  const double *__restrict__ sc, double *partial)
 {
     __shared__ double sm[256 / 32][kMaxBT];
@@ -432,15 +432,26 @@ __global__ void k_haydock_update(const double2 *__restrict__ t, const double2 *_
     const double c_prev = beta_p > 0.0 ? beta / beta_p : 0.0;
     double nn = 0.0;
     const int64_t n_el = n_orb * bt;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_el; i += (int64_t)gridDim.x * blockDim.x) {   // stride is a multiple of bt
-        const double2 tv = t[i], uv = u[i], pv = u_prev[i];
+    // The grid is small (its partials live in the 64 KB aux area), so every thread keeps EIGHT elements in flight: 24 independent
+    // 16-byte loads before the first use (~170 KB per SM; with one element per trip the kernel ran at 4.9 TB/s).
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;              // a multiple of bt: a thread stays with its state
+    auto one = [&](int64_t i, double2 tv, double2 uv, double2 pv) {
         double2 w;
         w.x = (tv.x - a_n * uv.x) * ib - c_prev * pv.x;
         w.y = (tv.y - a_n * uv.y) * ib - c_prev * pv.y;
         u_prev[i] = w;
         nn = fma(w.x, w.x, nn);
         nn = fma(w.y, w.y, nn);
+    };
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 7 * stride < n_el; i += 8 * stride) {
+        double2 tv[8], uv[8], pv[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { tv[k] = __ldcs(t + i + k * stride); uv[k] = __ldcs(u + i + k * stride); pv[k] = __ldcs(u_prev + i + k * stride); }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) one(i + k * stride, tv[k], uv[k], pv[k]);
     }
+    for (; i < n_el; i += stride) one(i, __ldcs(t + i), __ldcs(u + i), __ldcs(u_prev + i));
     for (int o = 16; o >= bt; o >>= 1) nn += __shfl_xor_sync(0xffffffffu, nn, o);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (lane < bt) sm[warp][lane] = nn;
