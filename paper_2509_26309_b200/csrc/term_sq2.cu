@@ -273,7 +273,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
     // ---- main consumers: thread = states 2q, 2q + 1 of the tile rows A = 2 pr and B = 2 pr + 1 (pr = 0 .. 63), in both stages;
     // "slot a" of a thread is state 2q + par, "slot b" state 2q + 1 - par (conflict-free 128-bit accesses, term_sq.cu).
     const int pr = tid >> 2, q = tid & 3, par = pr & 1;
-    constexpr bool act = true, okA = true, okB = true;
     const uint32_t oa = (uint32_t)(2 * q + par) * 16u, ob = (uint32_t)(2 * q + 1 - par) * 16u;
     const uint32_t rows2p = (uint32_t)(2 * pr + 1) * kRowBytes;  // 132-row slots: the slot row of tile row A - 1
     const uint32_t rowsy = (uint32_t)(2 * pr + 1) * kRowBytes;   // 130-row stage: the stage row of tile row A
@@ -343,12 +342,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 rel = (uint32_t)(__double2hiint(h.Aa.x) ^ __double2hiint(h.Ab.x) ^ __double2hiint(h.Ba.x) ^ __double2hiint(h.Bb.x));
                 if (DIAG) rel ^= (uint32_t)(__double2hiint(dA) ^ __double2hiint(dB));
                 const uint32_t wb = ringB0 + (it % kNB) * kSlotBytes + rows2p + kRowBytes;   // slot rows 2p + 1, 2p + 2 = rows A, B
-                if (act) { sts_c(wb + oa, h.Aa); sts_c(wb + ob, h.Ab); sts_c(wb + kRowBytes + oa, h.Ba); sts_c(wb + kRowBytes + ob, h.Bb); }
+                sts_c(wb + oa, h.Aa); sts_c(wb + ob, h.Ab); sts_c(wb + kRowBytes + oa, h.Ba); sts_c(wb + kRowBytes + ob, h.Bb);
                 if (!REDUCE && i >= 1 && i <= run.len) {   // T_k of the run's own lines: read by the next pair, a whole sweep later
                     const int64_t e1A = ((run.line0 + i - 1) * g.W + rowA0) * kBT + 2 * q;
                     CVec<2> out;
-                    if (okA) { out.v[0] = par ? h.Ab : h.Aa; out.v[1] = par ? h.Aa : h.Ab; out.st_stream(p.out1 + e1A); }
-                    if (okB) { out.v[0] = par ? h.Bb : h.Ba; out.v[1] = par ? h.Ba : h.Bb; out.st_stream(p.out1 + e1A + kBT); }
+                    out.v[0] = par ? h.Ab : h.Aa; out.v[1] = par ? h.Aa : h.Ab; out.st_stream(p.out1 + e1A);
+                    out.v[0] = par ? h.Bb : h.Ba; out.v[1] = par ? h.Ba : h.Bb; out.st_stream(p.out1 + e1A + kBT);
                 }
             }
             asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");   // line `it` of T_k is complete in ring B
@@ -374,8 +373,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                 rel ^= (uint32_t)(__double2hiint(h.Aa.x) ^ __double2hiint(h.Ab.x) ^ __double2hiint(h.Ba.x) ^ __double2hiint(h.Bb.x));
                 CVec<2> out;
                 if (!REDUCE) {
-                    if (okA) { out.v[0] = par ? h.Ab : h.Aa; out.v[1] = par ? h.Aa : h.Ab; out.st_stream(p.out2 + e2A); }
-                    if (okB) { out.v[0] = par ? h.Bb : h.Ba; out.v[1] = par ? h.Ba : h.Bb; out.st_stream(p.out2 + e2B); }
+                    out.v[0] = par ? h.Ab : h.Aa; out.v[1] = par ? h.Aa : h.Ab; out.st_stream(p.out2 + e2A);
+                    out.v[0] = par ? h.Bb : h.Ba; out.v[1] = par ? h.Ba : h.Bb; out.st_stream(p.out2 + e2B);
                 }
                 if (FLUSH) {
                     aAa.x += partA.a.x; aAa.y += partA.a.y; aAb.x += partA.b.x; aAb.y += partA.b.y;
@@ -391,11 +390,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                             im = fma(z.x, v.y, im); im = fma(-z.y, v.x, im);
                             nn = fma(v.x, v.x, nn); nn = fma(v.y, v.y, nn);
                         };
-                        if (okA) { acc3(sa_re, sa_im, sa_nn, zAa, aAa); acc3(sb_re, sb_im, sb_nn, zAb, aAb); oA.st(p.acc + e2A); }
-                        if (okB) { acc3(sa_re, sa_im, sa_nn, zBa, aBa); acc3(sb_re, sb_im, sb_nn, zBb, aBb); oB.st(p.acc + e2B); }
+                        acc3(sa_re, sa_im, sa_nn, zAa, aAa); acc3(sb_re, sb_im, sb_nn, zAb, aAb); oA.st(p.acc + e2A);
+                        acc3(sa_re, sa_im, sa_nn, zBa, aBa); acc3(sb_re, sb_im, sb_nn, zBb, aBb); oB.st(p.acc + e2B);
                     } else {
-                        if (okA) oA.st_stream(p.acc + e2A);
-                        if (okB) oB.st_stream(p.acc + e2B);
+                        oA.st_stream(p.acc + e2A);
+                        oB.st_stream(p.acc + e2B);
                     }
                 }
             }
