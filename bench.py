@@ -7,7 +7,7 @@ tbpm_build (hop list -> CSR + kernel layout) followed by tbpm_propagate of ALL t
 tile, per-step correlation + norm).  Inputs are resident in HBM when the timed region starts.
 `value` = n_state * n_block * (K-1) * nnz / step time, summed over ranks.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5|5ldos|3qe|5haydock] [--block B] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5|5ldos|3qe|5haydock|4ac] [--block B] [--impl reference]
 
 Default workload: BASELINE.json:configs[4] (cubic 256^3 + Anderson disorder, 16,777,216 orbitals x 32 states): the largest
 single-GPU configuration, one of the >= 16 M-orbital configs `north_star` sets its target on.  The full run length of a
@@ -17,7 +17,8 @@ the line also carries `per_workload`: cfg3, cfg4 and cfg5's 64-site LDOS leg mea
 Multi-GPU: states are independent, so every rank propagates its own batch of seeded states on a replica of
 H (paper_2509_26309_b200/replicas.py); no data-path collective; scaling is weak.
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
-`--workload 3qe` (cfg3 + quasi-eigenstates at 2 energies, NEXT-3) and `--workload 5haydock` (Haydock recursion from cfg5's 64
+`--workload 3qe` (cfg3 + quasi-eigenstates at 2 energies, NEXT-3), `--workload 4ac` (AC-conductivity correlation on cfg4's lattice,
+NEXT-4) and `--workload 5haydock` (Haydock recursion from cfg5's 64
 sites, NEXT-2) time the two NEXT rows that have kernels of their own (one GPU, one JSON line with `roofline`).
 """
 from __future__ import annotations
@@ -436,7 +437,7 @@ def main_ours(args):
 
 
 # ---------------------------------------------------------------------------------------------------------------------
-# the NEXT rows with kernels of their own: quasi-eigenstates (3qe) and the Haydock recursion (5haydock); one GPU
+# the NEXT rows: quasi-eigenstates (3qe), AC-conductivity correlation (4ac) and the Haydock recursion (5haydock); one GPU
 # ---------------------------------------------------------------------------------------------------------------------
 def main_next(args):
     import torch
@@ -450,12 +451,31 @@ def main_next(args):
     peak, peak_src = load_peaks()
     cfg = int(args.workload[0])
     haydock = args.workload.endswith("haydock")
+    ac = args.workload.endswith("ac")
     w = W.make_workload(cfg, device=dev)
     H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val, 0)
     block = args.block or 8
     K = len(tbpm.tbpm_cheb_coeff(w.rescale * w.dt))
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    if haydock:
+    if ac:
+        # NEXT-4: AC-conductivity correlation <psi2(t)|J_x|psi1(t)> on the lattice of cfg4 (Fermi-operator Chebyshev filters, two states
+        # propagated side by side, one current-operator product per time step); beta = 2 / |t|, mu = 0.5 |t|
+        n_state, beta, mu = w.n_state, 2.0, 0.5
+        psi0 = w.psi0(device=dev, n_state=n_state)
+        _, ji, jj, jv = W.square_current_hops(w.meta["Lx"], w.meta["Ly"], 0, phi_den=w.meta["phi_den"], device=dev)
+        J = tbpm.tbpm_build(w.n_orb, None, ji, jj, jv)
+        run = lambda: tbpm.tbpm_corr_ac(H, J, J, psi0, block, w.dt, w.rescale, beta, mu)
+        Kf = len(tbpm.tbpm_fermi_coeff(beta, mu, w.rescale, False)); Kg = len(tbpm.tbpm_fermi_coeff(beta, mu, w.rescale, True))
+        apps = (Kf - 1) + (Kg - 1) + 2 * block * (K - 1)             # H applications per state
+        units = n_state * apps * H.nnz
+        mat = H.lattice_bytes_per_term if H.lattice_kind in (2, 3) else H.matrix_bytes_per_term
+        vec = 16 * w.n_orb * n_state
+        bytes_step = apps * (mat + 3 * vec) + (J.matrix_bytes_per_term + 2 * vec) + (block + 1) * (J.matrix_bytes_per_term + 3 * vec)
+        what = (f"AC-conductivity correlation: Fermi filters of {Kf} and {Kg} Chebyshev terms, then {block} time steps of two states "
+                "(k_pair_sq: two Chebyshev terms per launch, as in the filters) with one current-operator product fused with the dot product per step")
+        count = ("per H application: matrix bytes of the running kernel's layout + 3 vectors; J_b psi0: current matrix + 2 vectors; per "
+                 "<psi2|J_a|psi1>: current matrix + 3 vectors (workspace allocation included in the time)")
+    elif haydock:
         n_state = w.ldos_n_site
         sites = W.ldos_sites(w.n_orb, n_state)
         ws = torch.empty(tbpm.tbpm_propagate_bytes(H, n_state), dtype=torch.uint8, device=dev)
@@ -493,15 +513,17 @@ def main_next(args):
     clocks = sampler.stop()
     ms = sum(a.elapsed_time(b) for a, b in evs)
     achieved = args.steps * bytes_step / (ms * 1e-3) / 1e9
-    line = {"metric": "Hamiltonian applications*nnz/sec (complex128)" if haydock else METRIC, "value": args.steps * units / (ms * 1e-3), "unit": UNIT,
+    line = {"metric": "Hamiltonian applications*nnz/sec (complex128)" if (haydock or ac) else METRIC, "value": args.steps * units / (ms * 1e-3), "unit": UNIT,
             "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "complex128", "data": "synthetic",
-            "config": {"workload": w.name + ("-haydock" if haydock else "-qe"), "n_orb": w.n_orb, "nnz": H.nnz, "n_state": n_state,
+            "config": {"workload": w.name + ("-ac" if ac else "-haydock" if haydock else "-qe"), "n_orb": w.n_orb, "nnz": H.nnz, "n_state": n_state,
                        "n_step_per_bench_step": block, "what": what, "l2": "256 MB flush between iterations; working set > L2"},
             "gpu_launches": int(tbpm.tbpm_total_launch_count() - launches0), "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                          "peak_source": peak_src, "count": count}}
-    if haydock:
+    if ac:
+        line["finite"] = bool(torch.isfinite(out.real).all() and torch.isfinite(out.imag).all())
+    elif haydock:
         a, b = out
         line["finite"] = bool(torch.isfinite(a).all() and torch.isfinite(b).all() and (b > 0).all())
     else:
@@ -512,6 +534,6 @@ def main_next(args):
 
 if __name__ == "__main__":
     a = parse_args()
-    if a.workload.endswith("qe") or a.workload.endswith("haydock"):
+    if a.workload.endswith("qe") or a.workload.endswith("haydock") or a.workload.endswith("ac"):
         sys.exit(main_next(a))
     sys.exit(main_reference(a) if a.impl == "reference" else main_ours(a))

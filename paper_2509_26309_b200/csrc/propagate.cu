@@ -1002,7 +1002,7 @@ extern "C" int tbpm_corr_ac_bytes(const tbpm_ham *H, int n_state, size_t *worksp
 {
     if (!H || n_state < 0 || !workspace_bytes) return TBPM_EINVAL;
     const Plan P = make_plan(H->n_orb, n_state, H->opt_tile);
-    *workspace_bytes = P.vec0_off + 6 * P.full_vec;
+    *workspace_bytes = P.vec0_off + 6 * P.full_vec + pair_extra_bytes(H, P);   // + two vectors where two terms per sweep apply
     return TBPM_OK;
 }
 
@@ -1050,11 +1050,22 @@ int corr_pair(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const double2 *da, const 
                                                                                        n_valid, bt, A[0], B[0]);
         count_launches(1);
         int grid = 1;
+        // two terms per sweep where term_sq2.cu applies and the caller's workspace holds the two extra vectors (behind the six)
+        const bool pairs = H->n_table > 0 && H->opt_kernel == 0 && bt == 8 && pair_sq_supported(bt, mh) &&
+                           workspace_bytes >= P.vec0_off + 8 * P.full_vec;
+        double2 *e1 = reinterpret_cast<double2 *>(base + 6 * P.full_vec), *e2 = reinterpret_cast<double2 *>(base + 7 * P.full_vec);
+        std::vector<StepOp> ops;
         // a Chebyshev series sum_k c_k T_k(H / s) applied to buf[slot]; returns the slot that holds the result
         auto series = [&](double2 **buf, int slot, int K, const std::vector<double> &c) -> int {
             double2 *psi = buf[slot], *t1 = buf[(slot + 1) % 3], *acc = buf[(slot + 2) % 3];
             TermParams tp = mh;
             tp.psi0 = psi;                                // the last term's dot products are not used here
+            if (pairs && K >= 3) {
+                step_pairs(tp, K, c, rescale, psi, t1, acc, e1, e2, ops);
+                for (size_t o = 0; o < ops.size() && !rc; ++o)
+                    rc = ops[o].pair ? launch_pair_sq(ops[o].tp, H->num_sms, st, &grid) : launch_term(bt, true, 0, ops[o].tp, H->num_sms, st, &grid);
+                return (slot + 2) % 3;
+            }
             if (K == 1) {
                 TermParams t0 = tp;
                 t0.x = psi; t0.y = t1; t0.acc = acc; t0.a = 0.0;
