@@ -218,7 +218,8 @@ int tbpm_haydock_ldos(const double *a, const double *b, int n_site, int n_iter, 
  * Ja, Jb: handles built with tbpm_build from the hop lists of the current operators J = i [H, r] (entry <i|J|j> = i <i|H|j>
  * (r_i - r_j), Hermitian, so each conjugate pair once; no onsite), same n_orb and device as H.  f(H) and 1 - f(H) are applied by
  * their Chebyshev series on [-rescale, rescale] (tbpm_fermi_coeff: host only, real coefficients as (re, 0) pairs, truncated after
- * the last |c_k| >= tol; the library uses tol = 1e-13).  Workspace: tbpm_corr_ac_bytes (six vectors of one tile). */
+ * the last |c_k| >= tol; the library uses tol = 1e-13).  Workspace: tbpm_corr_ac_bytes (six vectors of one tile, + two where the two-terms-per-
+ * sweep kernel applies; with only the six the series run one term per sweep). */
 int tbpm_fermi_coeff(double beta, double mu, double rescale, int one_minus, double tol, int kcap, int *K, double *coeff /* host [kcap][2] */);
 int tbpm_corr_ac_bytes(const tbpm_ham *H, int n_state, size_t *workspace_bytes);
 int tbpm_corr_ac(tbpm_ham *H, tbpm_ham *Ja, tbpm_ham *Jb, const double *psi0 /* device [n_state][n_orb][2] */, int n_state, int n_step,
