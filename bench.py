@@ -7,7 +7,7 @@ tbpm_build (hop list -> CSR + kernel layout) followed by tbpm_propagate of ALL t
 tile, per-step correlation + norm).  Inputs are resident in HBM when the timed region starts.
 `value` = n_state * n_block * (K-1) * nnz / step time, summed over ranks.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5|5ldos|3qe|5haydock|4ac] [--block B] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5|5ldos|3qe|4ac|5dp|5haydock] [--block B] [--impl reference]
 
 Default workload: BASELINE.json:configs[4] (cubic 256^3 + Anderson disorder, 16,777,216 orbitals x 32 states): the largest
 single-GPU configuration, one of the >= 16 M-orbital configs `north_star` sets its target on.  The full run length of a
@@ -17,8 +17,8 @@ the line also carries `per_workload`: cfg3, cfg4 and cfg5's 64-site LDOS leg mea
 Multi-GPU: states are independent, so every rank propagates its own batch of seeded states on a replica of
 H (paper_2509_26309_b200/replicas.py); no data-path collective; scaling is weak.
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
-`--workload 3qe` (cfg3 + quasi-eigenstates at 2 energies, NEXT-3), `--workload 4ac` (AC-conductivity correlation on cfg4's lattice,
-NEXT-4) and `--workload 5haydock` (Haydock recursion from cfg5's 64
+`--workload 3qe` (cfg3 + quasi-eigenstates at 2 energies, NEXT-3), `--workload 4ac` / `5dp` (AC-conductivity and dynamic-polarisation
+correlations on cfg4's / cfg5's lattice, NEXT-4) and `--workload 5haydock` (Haydock recursion from cfg5's 64
 sites, NEXT-2) time the two NEXT rows that have kernels of their own (one GPU, one JSON line with `roofline`).
 """
 from __future__ import annotations
@@ -452,6 +452,7 @@ def main_next(args):
     cfg = int(args.workload[0])
     haydock = args.workload.endswith("haydock")
     ac = args.workload.endswith("ac")
+    dp = args.workload.endswith("dp")
     w = W.make_workload(cfg, device=dev)
     H = tbpm.tbpm_build(w.n_orb, w.onsite, w.hop_i, w.hop_j, w.hop_val, 0)
     block = args.block or 8
@@ -475,6 +476,27 @@ def main_next(args):
                 "(k_pair_sq: two Chebyshev terms per launch, as in the filters) with one current-operator product fused with the dot product per step")
         count = ("per H application: matrix bytes of the running kernel's layout + 3 vectors; J_b psi0: current matrix + 2 vectors; per "
                  "<psi2|J_a|psi1>: current matrix + 3 vectors (workspace allocation included in the time)")
+    elif dp:
+        # NEXT-4, second half: dynamic-polarisation correlation <psi2(t)|rho(q)|psi1(t)> on the lattice of cfg5, one tile of 8 states,
+        # q = (2 pi / L)(1, 0, 2); the density operators are diagonal, so there is no second matrix
+        import math
+        n_state, beta, mu, L = 8, 0.5, 1.0, w.meta["L"]
+        psi0 = w.psi0(device=dev, n_state=n_state)
+        idx = torch.arange(w.n_orb, device=dev)
+        ph = (2 * math.pi / L) * (1.0 * (idx % L) + 2.0 * (idx // (L * L))).to(torch.float64)
+        rho = torch.complex(torch.cos(ph), torch.sin(ph))
+        rho_c = rho.conj().resolve_conj().contiguous()
+        run = lambda: tbpm.tbpm_corr_dp(H, rho, rho_c, psi0, block, w.dt, w.rescale, beta, mu)
+        Kf = len(tbpm.tbpm_fermi_coeff(beta, mu, w.rescale, False)); Kg = len(tbpm.tbpm_fermi_coeff(beta, mu, w.rescale, True))
+        apps = (Kf - 1) + (Kg - 1) + 2 * block * (K - 1)
+        units = n_state * apps * H.nnz
+        mat = H.lattice_bytes_per_term if H.lattice_kind in (2, 3) else H.matrix_bytes_per_term
+        vec = 16 * w.n_orb * n_state
+        bytes_step = apps * (mat + 3 * vec) + (16 * w.n_orb + 2 * vec) + (block + 1) * (16 * w.n_orb + 2 * vec)
+        what = (f"dynamic-polarisation correlation: Fermi filters of {Kf} and {Kg} Chebyshev terms, then {block} time steps of two states "
+                "(k_term_l3) with one diagonal density-operator product fused with the dot product per step (k_diag_dot)")
+        count = ("per H application: matrix bytes of the running kernel's layout + 3 vectors; rho_b psi0: diagonal + 2 vectors; per "
+                 "<psi2|rho_a|psi1>: diagonal + 2 vectors (workspace allocation included in the time)")
     elif haydock:
         n_state = w.ldos_n_site
         sites = W.ldos_sites(w.n_orb, n_state)
@@ -513,15 +535,15 @@ def main_next(args):
     clocks = sampler.stop()
     ms = sum(a.elapsed_time(b) for a, b in evs)
     achieved = args.steps * bytes_step / (ms * 1e-3) / 1e9
-    line = {"metric": "Hamiltonian applications*nnz/sec (complex128)" if (haydock or ac) else METRIC, "value": args.steps * units / (ms * 1e-3), "unit": UNIT,
+    line = {"metric": "Hamiltonian applications*nnz/sec (complex128)" if (haydock or ac or dp) else METRIC, "value": args.steps * units / (ms * 1e-3), "unit": UNIT,
             "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "complex128", "data": "synthetic",
-            "config": {"workload": w.name + ("-ac" if ac else "-haydock" if haydock else "-qe"), "n_orb": w.n_orb, "nnz": H.nnz, "n_state": n_state,
+            "config": {"workload": w.name + ("-ac" if ac else "-dp" if dp else "-haydock" if haydock else "-qe"), "n_orb": w.n_orb, "nnz": H.nnz, "n_state": n_state,
                        "n_step_per_bench_step": block, "what": what, "l2": "256 MB flush between iterations; working set > L2"},
             "gpu_launches": int(tbpm.tbpm_total_launch_count() - launches0), "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                          "peak_source": peak_src, "count": count}}
-    if ac:
+    if ac or dp:
         line["finite"] = bool(torch.isfinite(out.real).all() and torch.isfinite(out.imag).all())
     elif haydock:
         a, b = out
@@ -534,6 +556,6 @@ def main_next(args):
 
 if __name__ == "__main__":
     a = parse_args()
-    if a.workload.endswith("qe") or a.workload.endswith("haydock") or a.workload.endswith("ac"):
+    if a.workload.endswith("qe") or a.workload.endswith("haydock") or a.workload.endswith("ac") or a.workload.endswith("dp"):
         sys.exit(main_next(a))
     sys.exit(main_reference(a) if a.impl == "reference" else main_ours(a))
