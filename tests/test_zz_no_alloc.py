@@ -57,6 +57,11 @@ def test_static_workspace_two_calls_in_a_row(dev, oracle_mod):
     w2 = W.make_workload(1, device=dev)
     H2, psi2, cr2, nr2, c2, n2 = both_paths(dev, w2, 1, 16)
     check(cr2, nr2, c2, n2)
+    # a square lattice with flux, 8 states: the two-terms-per-sweep kernel, its two extra vectors inside the static array too
+    w4 = W.make_workload(4, device=dev, Lx=128, Ly=24, phi_den=32)
+    H4, psi4, cr4, nr4, c4, n4 = both_paths(dev, w4, 8, 5)
+    check(cr4, nr4, c4, n4)
+    assert tbpm.tbpm_last_launch_count(H4) == 1 + 5 * 11             # 10 pairs + reduction per time step: the pair path ran
     # call 3: the first model again, three states (a padded tile of 4) over call 2's left-overs, against the oracle itself
     psi3 = w1.psi0(device=dev, n_state=3)
     c3, n3 = tbpm.tbpm_propagate_static(H1, psi3, 5, w1.dt, w1.rescale)
