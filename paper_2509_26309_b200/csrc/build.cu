@@ -757,7 +757,7 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
             }
             // short rows, one real value: 16-bit column offsets for term_n16.cu (every entry checked)
             const int n_off_max = H->max_row_nnz - (has_onsite ? 1 : 0);
-            if (H->single_real && n_off_max >= 1 && n_off_max <= kNear16MaxW + 2) {
+            if (H->single_real && n_off_max >= 1 && n_off_max <= kNear16MaxW + 2 && H->halo_rows <= 32767) {   // halo_rows: widest circular |col - row|
                 k_near16<<<gr, kThreads, 0, st>>>(n_orb, 0, 0, H->orp, H->ocol, H->d16, H->status);
                 int32_t back16[2] = {0, 0};                 // ST_N16_BAD, ST_N16_WF are neighbours
                 TRY_OR_FAIL(cudaMemcpyAsync(back16, H->status + ST_N16_BAD, sizeof(back16), cudaMemcpyDeviceToHost, st));
