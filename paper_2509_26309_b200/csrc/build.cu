@@ -493,7 +493,7 @@ __device__ __forceinline__ int64_t sq8_neighbour(int64_t x, int64_t y, int64_t W
 // status[ST_SQ8_BAD] counts the warps holding a row that fails.  When it stays 0 the lattice kernel needs neither the column
 // words nor the per-entry value indices: the whole matrix is the W x 8 table dline + the value table.
 __global__ void k_sq8(int64_t n_orb, int64_t W, const int32_t *__restrict__ ocol, const uint16_t *__restrict__ oidx, int pass, uint16_t *dline,
-                      int32_t *status)
+                      const double2 *__restrict__ vtab, int32_t *status)
 {
     const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     bool bad = false;
@@ -508,7 +508,11 @@ __global__ void k_sq8(int64_t n_orb, int64_t W, const int32_t *__restrict__ ocol
             for (int j = 0; j < 8; ++j)
                 if ((int64_t)c[j] == nb) found = j;
             if (found < 0) { bad = true; continue; }
-            if (pass == 0) dline[x * 8 + k] = id[found];
+            if (pass == 0) {
+                dline[x * 8 + k] = id[found];
+                // hops along the line (directions 3, 4): real in the Landau gauge -- the pair kernel then spends 2 FMAs on them, not 4
+                if ((k == 3 || k == 4) && vtab[id[found] & 0x7fff].y != 0.0) atomicAdd(&status[ST_SQ8_CPLX], 1);
+            }
             else bad = bad || dline[x * 8 + k] != id[found];
         }
     }
@@ -802,15 +806,16 @@ extern "C" int tbpm_build(int64_t n_orb, const double *onsite, int64_t n_hop, co
                                  dl.d[0] == -Wq - 1 && dl.d[1] == -Wq && dl.d[2] == -Wq + 1 && dl.d[3] == -1 && dl.d[4] == 1 && dl.d[5] == Wq - 1 &&
                                  dl.d[7] == Wq + 1;
                 if (sq8) {
-                    k_sq8<<<blocks_for(Wq, kThreads), kThreads, 0, st>>>(n_orb, Wq, H->ocol, H->oidx, 0, H->dline, H->status);
-                    k_sq8<<<gr, kThreads, 0, st>>>(n_orb, Wq, H->ocol, H->oidx, 1, H->dline, H->status);
+                    k_sq8<<<blocks_for(Wq, kThreads), kThreads, 0, st>>>(n_orb, Wq, H->ocol, H->oidx, 0, H->dline, H->vtab, H->status);
+                    k_sq8<<<gr, kThreads, 0, st>>>(n_orb, Wq, H->ocol, H->oidx, 1, H->dline, H->vtab, H->status);
                     count_launches(2);
                 }
-                int32_t back[2] = {0, 0};                   // ST_NREG, ST_SQ8_BAD are neighbours
+                int32_t back[5] = {0, 0, 0, 0, 0};          // ST_NREG, ST_SQ8_BAD, (near16: 2 words), ST_SQ8_CPLX
                 TRY_OR_FAIL(cudaMemcpyAsync(back, H->status + ST_NREG, sizeof(back), cudaMemcpyDeviceToHost, st));
                 TRY_OR_FAIL(cudaStreamSynchronize(st));
                 H->n_regular = back[0];
                 H->sq8_line = (sq8 && back[1] == 0) ? Wq : 0;
+                H->sq8_real_x = H->sq8_line > 0 && back[4] == 0;
             }
         }
     }

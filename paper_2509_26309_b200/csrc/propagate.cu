@@ -690,7 +690,7 @@ TermParams matrix_params(const tbpm_ham *H, double *partial)
     mp.lat_flags = H->lat_flags;
     mp.n_regular = H->n_regular;
     mp.lat_periodic3 = H->lat_periodic3;
-    mp.sq8_line = H->sq8_line; mp.dline = H->dline;
+    mp.sq8_line = H->sq8_line; mp.dline = H->dline; mp.sq8_real_x = H->sq8_real_x;
     mp.d16 = H->near16_w > 0 ? H->d16 : nullptr; mp.n16_w = H->near16_w;
     mp.uniform = H->n_orb > 0 && H->min_row_nnz == H->max_row_nnz;
     mp.max_row_off = std::max(0, H->max_row_nnz - (H->has_onsite ? 1 : 0));

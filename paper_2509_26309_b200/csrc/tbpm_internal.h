@@ -46,7 +46,8 @@ enum StatusWord {
     ST_NREG = 8,         // rows whose entries sit exactly at the lattice offsets (k_lat_flags)
     ST_SQ8_BAD = 9,      // warps with a row that is not a site of the periodic square lattice with in-line hoppings (k_sq8)
     ST_N16_BAD = 10,     // warps with an entry further than 32767 rows from its row, also round the boundary (k_near16)
-    ST_N16_WF = 11       // most entries of a row that are not at row +- 1 (k_near16)
+    ST_N16_WF = 11,      // most entries of a row that are not at row +- 1 (k_near16)
+    ST_SQ8_CPLX = 12     // k_sq8: in-line hops (directions 3, 4) whose value has a non-zero imaginary part
 };
 
 // What the last tbpm_propagate / tbpm_ldos call of a handle left in a workspace (read by tbpm_get_state).
@@ -74,6 +75,7 @@ struct tbpm_ham {
     int64_t lat_off[16] = {0};
     int64_t lat_delta[16] = {0};   // the same offsets signed, in the order of the sample row's entries (slot j -> col - row)
     int64_t n_regular = 0;         // rows that follow lat_delta exactly (bits of lat_flags)
+    int32_t sq8_real_x = 0;        // sq8_line > 0: the in-line hops (x direction) are all real (Landau gauge along the line)
     int64_t sq8_line = 0;          // > 0: periodic square lattice + next-nearest neighbours, line of this many rows, hoppings = dline
     int32_t near16_w = 0;          // > 0: d16 holds a flag word and this many far column offsets per row (term_n16.cu)
     int32_t lat_periodic3 = 0;     // the bits were computed for the periodic three-dimensional lattice (wrapped neighbours count)

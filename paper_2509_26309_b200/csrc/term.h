@@ -54,6 +54,7 @@ struct TermParams {
     const uint32_t *lat_flags;  // bit r: row r follows lat_delta exactly (build.cu, k_lat_flags)
     int64_t n_regular;     // number of such rows
     int64_t sq8_line;      // > 0: periodic square lattice with next-nearest neighbours whose hoppings depend on the in-line position
+    int sq8_real_x;        // the hops along the line (directions 3, 4 of dline) are real
     const uint16_t *dline; // only (build.cu, k_sq8): line length in rows and the [x][8] table of value indices by direction
     const int16_t *d16;    // short rows, one real value (build.cu, k_near16): [row / 32][word][row % 32], +-1 flags | far offsets
     int n16_w;             // far offsets per row of d16 (1, 2 or 4), 0: none

@@ -83,6 +83,9 @@ struct Out4 { double2 Aa, Ab, Ba, Bb; };                   // rows A and B, slot
 
 // H * v on the thread's two rows from three consecutive lines held in 132-row slots (bp / bo / bn: address of slot row 2p of the
 // line above / the own line / the line below); xA, xB return the own rows of the middle line.
+// RX: the two in-line hops (directions 3, 4) are REAL (Landau gauge along the line, certified by the builder): 2 FMAs instead of 4;
+// the result is the same bit for bit, the dropped FMAs would add 0 * x.
+template <bool RX>
 __device__ __forceinline__ void apply_h(uint32_t bp, uint32_t bo, uint32_t bn, uint32_t oa, uint32_t ob, const double2 (&vA)[kCH],
                                         const double2 (&vB)[kCH], Out4 &h, Row2 &xA, Row2 &xB)
 {
@@ -99,10 +102,13 @@ __device__ __forceinline__ void apply_h(uint32_t bp, uint32_t bo, uint32_t bn, u
         cfma(h.Ba, vB[k], r[k + 1].a); cfma(h.Bb, vB[k], r[k + 1].b);
     }
     load4(bo);                                             // own line: directions 3, 4 = -1, +1; r[1], r[2] are the own rows
-    cfma(h.Aa, vA[3], r[0].a); cfma(h.Ab, vA[3], r[0].b);
-    cfma(h.Ba, vB[3], r[1].a); cfma(h.Bb, vB[3], r[1].b);
-    cfma(h.Aa, vA[4], r[2].a); cfma(h.Ab, vA[4], r[2].b);
-    cfma(h.Ba, vB[4], r[3].a); cfma(h.Bb, vB[4], r[3].b);
+    auto hop = [](double2 &acc, double2 v, double2 x) {
+        if (RX) { acc.x = fma(v.x, x.x, acc.x); acc.y = fma(v.x, x.y, acc.y); } else cfma(acc, v, x);
+    };
+    hop(h.Aa, vA[3], r[0].a); hop(h.Ab, vA[3], r[0].b);
+    hop(h.Ba, vB[3], r[1].a); hop(h.Bb, vB[3], r[1].b);
+    hop(h.Aa, vA[4], r[2].a); hop(h.Ab, vA[4], r[2].b);
+    hop(h.Ba, vB[4], r[3].a); hop(h.Bb, vB[4], r[3].b);
     xA = r[1]; xB = r[2];
     load4(bn);                                             // line below: directions 5, 6, 7
 #pragma unroll
@@ -112,7 +118,7 @@ __device__ __forceinline__ void apply_h(uint32_t bp, uint32_t bo, uint32_t bn, u
     }
 }
 
-template <bool FLUSH, bool REDUCE, bool DIAG>
+template <bool FLUSH, bool REDUCE, bool DIAG, bool RX>
 __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, const Geom g)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -325,7 +331,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
             {   // ---- stage 1: T_k = a1 * H * T_{k-1} - T_{k-2} on rows A, B of line line0 - 1 + i
                 Out4 h;
                 Row2 xA, xB;
-                apply_h(sa0, sa1, sa2, oa, ob, vA, vB, h, xA, xB);
+                apply_h<RX>(sa0, sa1, sa2, oa, ob, vA, vB, h, xA, xB);
                 if (DIAG) {                                // diagonal of rows A, B of this line (stage index = tile row + 2); kept for stage 2 of the next line
                     const uint32_t sd = stage0 + (uint32_t)s * stb + kYBytes + (uint32_t)(2 * pr + 2) * 8u;
                     dA = lds_f64(sd); dB = lds_f64(sd + 8u);
@@ -361,7 +367,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_pair_sq(const TermParams p, con
                                sb2 = ringB0 + (it % kNB) * kSlotBytes + rows2p;
                 Out4 h;
                 Row2 tA, tB, xA, xB;                       // T_k and T_{k-1} on the own rows
-                apply_h(sb0, sb1, sb2, oa, ob, vA, vB, h, tA, tB);
+                apply_h<RX>(sb0, sb1, sb2, oa, ob, vA, vB, h, tA, tB);
                 if (DIAG) {
                     h.Aa.x = fma(dPA, tA.a.x, h.Aa.x); h.Aa.y = fma(dPA, tA.a.y, h.Aa.y); h.Ab.x = fma(dPA, tA.b.x, h.Ab.x); h.Ab.y = fma(dPA, tA.b.y, h.Ab.y);
                     h.Ba.x = fma(dPB, tB.a.x, h.Ba.x); h.Ba.y = fma(dPB, tB.a.y, h.Ba.y); h.Bb.x = fma(dPB, tB.b.x, h.Bb.x); h.Bb.y = fma(dPB, tB.b.y, h.Bb.y);
@@ -474,11 +480,11 @@ bool make_geom(const TermParams &p, Geom &g)
     return (size_t)(g.n_ring + kNB) * kSlotBytes + (size_t)g.n_stage * g.stage_bytes <= kSmemMax - 4096;
 }
 
-template <bool FLUSH, bool REDUCE, bool DIAG>
+template <bool FLUSH, bool REDUCE, bool DIAG, bool RX>
 int launch_one(const TermParams &p, const Geom &g, int num_sms, cudaStream_t st, int *grid_out)
 {
     const size_t dyn = (size_t)(g.n_ring + kNB) * kSlotBytes + (size_t)g.n_stage * g.stage_bytes;
-    auto kern = k_pair_sq<FLUSH, REDUCE, DIAG>;
+    auto kern = k_pair_sq<FLUSH, REDUCE, DIAG, RX>;
     static size_t configured[kMaxDevices] = {0};
     if (p.device < 0 || p.device >= kMaxDevices) return TBPM_EINVAL;
     if (dyn > configured[p.device]) {
@@ -512,14 +518,13 @@ int launch_pair_sq(const TermParams &p, int num_sms, cudaStream_t st, int *grid_
     if (!sq2::make_geom(p, g) || !p.out1 || !p.out2) return TBPM_EINVAL;
     const bool red = p.flags & F_REDUCE;
     if (red && p.n_acc <= 0) return TBPM_EINVAL;
-    if (p.diag) {
-        if (red) return sq2::launch_one<true, true, true>(p, g, num_sms, st, grid_out);
-        if (p.n_acc > 0) return sq2::launch_one<true, false, true>(p, g, num_sms, st, grid_out);
-        return sq2::launch_one<false, false, true>(p, g, num_sms, st, grid_out);
-    }
-    if (red) return sq2::launch_one<true, true, false>(p, g, num_sms, st, grid_out);
-    if (p.n_acc > 0) return sq2::launch_one<true, false, false>(p, g, num_sms, st, grid_out);
-    return sq2::launch_one<false, false, false>(p, g, num_sms, st, grid_out);
+    const int shape = red ? 2 : (p.n_acc > 0 ? 1 : 0);    // plain pair / pair with psi' update / last pair
+#define TBPM_PAIR(D, R)                                                                                         \
+    (shape == 2 ? sq2::launch_one<true, true, D, R>(p, g, num_sms, st, grid_out)                                  \
+                : shape == 1 ? sq2::launch_one<true, false, D, R>(p, g, num_sms, st, grid_out) : sq2::launch_one<false, false, D, R>(p, g, num_sms, st, grid_out))
+    if (p.diag) return p.sq8_real_x ? TBPM_PAIR(true, true) : TBPM_PAIR(true, false);
+    return p.sq8_real_x ? TBPM_PAIR(false, true) : TBPM_PAIR(false, false);
+#undef TBPM_PAIR
 }
 
 }  // namespace tbpm_detail

@@ -274,6 +274,20 @@ def test_two_terms_per_sweep_with_diagonal(dev, oracle_mod, tau_scale, Lx, Ly, p
     assert (c1 - corr).abs().max().item() <= 1e-13 and (n1 - norm2).abs().max().item() <= 1e-13
 
 
+def test_two_terms_per_sweep_complex_inline_hops(dev, oracle_mod):
+    """The builder certifies whether the hops ALONG a line are real (Landau gauge: they are; the pair kernel then spends two FMAs on
+    them instead of four).  Here they carry a constant phase -- still a function of the in-line position only, so the square-lattice
+    kernels run, but on their general (complex) variant; with and without diagonal."""
+    n, hi, hj, hv = W.square_peierls_hops(256, 40, -1.0, 0.2, 1, 64, dev)
+    inline = (hi // 256) == (hj // 256)
+    hv = torch.where(inline, hv * torch.exp(torch.tensor(0.3j, dtype=torch.complex128, device=dev)), hv)
+    for onsite in (None, W.anderson_onsite(n, 2.0, device=dev)):
+        w = W.Workload("square-flux-twisted", n, hi, hj, hv, onsite, 8, 5, 6.0)
+        H, psi0, corr, norm2 = run_parity(dev, oracle_mod, w, 8, 5)
+        assert H.lattice_kind == tbpm.TBPM_LATTICE_SQUARE8
+        assert tbpm.tbpm_last_launch_count(H) == 1 + 5 * 11
+
+
 def test_two_terms_per_sweep_ldos_and_determinism(dev, oracle_mod):
     """The pair path under tbpm_ldos (unit initial vectors) and twice in a row: bit-identical."""
     w = W.make_workload(4, device=dev, Lx=128, Ly=40, phi_den=32)
